@@ -1,0 +1,338 @@
+"""bench.py -- throughput of the gauge-fixing hot path (arXiv 1210.8018, Algorithm 1) on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload 32^4] [--impl ours|reference]
+
+A step is one execution of the loop body of Algorithm 1 (FFT filter of Delta, g build, link
+update, measure) on one lattice.  Default workload: BASELINE.json configs[2], the headline
+32^4 FP64 lattice with 12-real links.  Metric: site-iterations/s = V * steps / time.
+With N > 1 (torchrun) every rank fixes its own lattice (replicas, no data-path collective:
+DESIGN.md section 9), `value` is the sum over ranks / max time over ranks.
+
+One JSON line on stdout (rank 0).  `value` is device-resident; `e2e` goes through the C ABI
+with pinned HOST buffers (load links, iterate, read the result) every step.
+`--impl reference` times the CPU oracle (oracle/) instead, as it stands, on the host cores.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "gauge-fix site-iterations/s"
+UNIT = "site-iterations/s"
+ALPHA = 0.08
+
+# workload name -> (extents, sigma, seed offset, precision, recon)   (BASELINE.json `configs`)
+WORKLOADS = {
+    "8^4": ((8,) * 4, 0.3, 8, "fp64", 18),
+    "16^4": ((16,) * 4, 0.5, 16, "fp64", 18),
+    "32^4": ((32,) * 4, 0.5, 32, "fp64", 12),
+    "48^4": ((48,) * 4, 0.5, 48, "fp32", 18),
+    "64^4": ((64,) * 4, 0.6, 64, "fp64", 18),
+}
+
+
+def algorithmic_bytes(recon, nfields, real_bytes, tiled):
+    """Bytes per site each kernel must move once:
+    L = link bytes per site, W = field bytes per site."""
+    L = 4 * recon * real_bytes
+    W = nfields * 2 * real_bytes
+    per = {"measure": L + W, "update": W + 2 * L}
+    if tiled:
+        per.update({"fft_xy_fwd": 2 * W, "fft_zt": 2 * W, "fft_xy_inv": 2 * W})
+    else:
+        per["fft_generic"] = 2 * W       # per launch (8 launches per iteration)
+    return per
+
+
+class ClockSampler:
+    """nvidia-smi clocks and throttle reasons during the timed region (B200_PROFILING.md)."""
+
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index = index
+        self.rows = []
+        self.proc = None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "50"],
+                stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True)
+            self.t.start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append((time.time(), [x.strip() for x in line.split(",")]))
+
+    def mark(self):
+        return time.time()
+
+    def stop(self, t0, t1):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.12)
+        self.proc.terminate()
+        rows = [r for (t, r) in self.rows if t0 - 0.05 <= t <= t1 + 0.1] or [r for (_, r) in self.rows]
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in rows:
+            try:
+                sm.append(float(r[0])); mx.append(float(r[1]))
+            except (ValueError, IndexError):
+                continue
+            for nm, v in zip(names, r[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(nm)
+        sm.sort()
+        return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        return float(json.load(open(p))["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+def time_oracle(N, sigma, seed, iters):
+    """The oracle as it stands, single thread: site-iterations/s over `iters` iterations."""
+    import gen
+    import oracle
+
+    U = gen.gen_links(N, sigma, seed)
+    oracle.measure(N, U, want_delta=False)          # page everything in
+    t = time.perf_counter()
+    oracle.iterate(N, U, ALPHA, iters)
+    dt = time.perf_counter() - t
+    V = N[0] * N[1] * N[2] * N[3]
+    return V * iters / dt, dt
+
+
+def run_reference(args):
+    """--impl reference: the CPU oracle on the host cores, one bounded sample per step."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    import gen
+
+    N, sigma, soff, prec, recon = WORKLOADS[args.workload]
+    # a step = one oracle iteration on a lattice of the same generator, bounded to 16^4 sites so
+    # that K + W steps end within minutes (a 32^4 oracle iteration takes several seconds)
+    Ns = tuple(min(n, 16) for n in N)
+    seed = gen.BASE_SEED + soff
+    import oracle
+
+    U = gen.gen_links(Ns, sigma, seed)
+    Vs = Ns[0] * Ns[1] * Ns[2] * Ns[3]
+    for _ in range(args.warmup):
+        oracle.iterate(Ns, U, ALPHA, 1)
+    t = time.perf_counter()
+    for _ in range(args.steps):
+        oracle.iterate(Ns, U, ALPHA, 1)
+    dt = time.perf_counter() - t
+    val = Vs * args.steps / dt
+    sample = f"{args.steps} single-thread oracle iterations on {'x'.join(map(str, Ns))} (same generator, sigma={sigma})"
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": args.workload, "sample": sample},
+        "cpu_baseline": {"value": val, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+        "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }), flush=True)
+
+
+def run_ours(args):
+    import numpy as np
+    import torch
+    import torch.distributed as dist
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; liblgf has no CPU fallback")
+    torch.cuda.set_device(local)
+    if world > 1:
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    from paper_1210_8018_b200 import build as lgf_build
+    from paper_1210_8018_b200 import lgf
+
+    if rank == 0:
+        lgf_build.build()
+    if world > 1:
+        dist.barrier()
+    import gen
+
+    N, sigma, soff, prec, recon = WORKLOADS[args.workload]
+    if args.recon:
+        recon = args.recon
+    V = N[0] * N[1] * N[2] * N[3]
+    seed = gen.BASE_SEED + soff + 7919 * rank           # every rank its own lattice (replicas)
+    U = gen.gen_links(N, sigma, seed)
+    cdt = np.complex128 if prec == "fp64" else np.complex64
+    tdt = torch.complex128 if prec == "fp64" else torch.complex64
+    U = U.astype(cdt, copy=False)
+    host = torch.empty((V, 4, 3, 3), dtype=tdt).pin_memory()
+    host.copy_(torch.from_numpy(U))
+    dev = host.to(f"cuda:{local}")
+    torch.cuda.synchronize()
+
+    gf = lgf.GaugeFixer(N, precision=prec, recon=recon, fft_batch=args.fft_batch, fft_path=args.fft_path,
+                        device=f"cuda:{local}")
+    K, W = args.steps, args.warmup
+    stream = gf.stream
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+            torch.cuda.synchronize()
+
+    def timed_iterations(profile):
+        """W untimed + K timed iterations from the freshly loaded links; returns (ms, launches)."""
+        gf.set_option(lgf.OPT_PROFILE, 0)
+        gf.load_links(dev)
+        gf.iterate(ALPHA, W)
+        gf.load_links(dev)                      # timed window = iterations 1..K of Algorithm 1
+        gf.set_option(lgf.OPT_PROFILE, 1 if profile else 0)
+        gf.reset_counters()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        barrier()
+        with torch.cuda.stream(stream):
+            e0.record(stream)
+            gf.iterate(ALPHA, K, sync=False)
+            e1.record(stream)
+        barrier()
+        return e0.elapsed_time(e1), gf.launch_count()
+
+    # ---- device-resident timing (the headline `value`)
+    sampler = ClockSampler(local) if rank == 0 else None
+    if sampler:
+        sampler.start()
+        time.sleep(0.15)
+    t0 = time.time()
+    ms, launches = timed_iterations(profile=False)
+    t1 = time.time()
+    r_end = gf.iterate(ALPHA, 0)
+
+    # ---- the same window with every launch bracketed by CUDA events on the library's stream
+    ms_prof, _ = timed_iterations(profile=True)
+    ktimes = gf.kernel_times()
+    gf.set_option(lgf.OPT_PROFILE, 0)
+
+    # ---- end to end through the C ABI with pinned host buffers, copies inside the timed region
+    e2e_steps = K
+    gf.load_links(host.numpy())
+    barrier()
+    te = time.perf_counter()
+    for _ in range(e2e_steps):
+        gf.load_links(host.numpy())             # H2D of the step's input (36 complex per site)
+        gf.iterate(ALPHA, 1)                    # one iteration + D2H of (iterations, F, theta)
+    torch.cuda.synchronize()
+    e2e_s = time.perf_counter() - te
+    clocks = sampler.stop(t0, t1) if sampler else None
+
+    tmax = torch.tensor([ms, e2e_s], dtype=torch.float64, device=f"cuda:{local}")
+    if world > 1:
+        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
+    ms_all, e2e_all = float(tmax[0]), float(tmax[1])
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    real_bytes = 8 if prec == "fp64" else 4
+    tiled = gf.uses_tiled_fft()
+    per = algorithmic_bytes(recon, args.fft_batch, real_bytes, tiled)
+    peak, peak_src = peaks()
+    kern = {k: {"ms_total": v[0], "launches": v[1], "us_per_launch": 1e3 * v[0] / v[1]}
+            for k, v in ktimes.items() if v[1] and k in per}
+    for k in kern:
+        kern[k]["bytes_per_site"] = per[k]
+        kern[k]["GBps"] = per[k] * V / (kern[k]["us_per_launch"] * 1e-6) / 1e9
+        kern[k]["share"] = kern[k]["ms_total"] / sum(v[0] for kk, v in ktimes.items() if kk in per)
+    dom = max(kern, key=lambda k: kern[k]["ms_total"])
+    iter_bytes = sum(per[k] * (8 if k == "fft_generic" else 1) for k in per)
+    value = world * V * K / (ms_all * 1e-3)
+    e2e_val = world * V * e2e_steps / e2e_all
+    h2d = V * 36 * 2 * real_bytes
+
+    # ---- CPU baseline: the oracle as it stands on a bounded sample of the same workload
+    cpu = None
+    if not args.no_cpu_baseline:
+        Ns = N if V <= 32 ** 4 else tuple(min(n, 32) for n in N)
+        iters = {True: 3}.get(Ns[0] >= 32, 20 if Ns[0] >= 16 else 200)
+        v, dt = time_oracle(Ns, sigma, gen.BASE_SEED + soff, iters)
+        cpu = {"value": v, "unit": UNIT, "cores": 1, "kind": "oracle",
+               "sample": f"{iters} oracle iterations on {'x'.join(map(str, Ns))} ({dt:.1f} s, single thread, "
+                         f"{os.cpu_count()} cores on the box)"}
+
+    out = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
+        "ms_per_step": ms_all / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f64" if prec == "fp64" else "f32", "data": "synthetic",
+        "config": {"workload": f"{args.workload} periodic SU(3), {prec}, {recon}-real links, {args.fft_batch} FFT fields, "
+                               f"alpha={ALPHA}, gen seed {gen.BASE_SEED + soff}, sigma={sigma}",
+                   "fft": "tiled register FFT, 3 passes" if tiled else "generic per-axis transform, 8 passes",
+                   "l2": "working set (links + fields) exceeds the 126 MB L2" if V >= 32 ** 4 else
+                         "working set fits in L2; latency/L2-bound by design (DESIGN.md section 6)",
+                   "parallelism": "replicas" if world > 1 else "single GPU",
+                   "final": {"iterations": int(r_end.iterations), "F": r_end.F, "theta": r_end.theta}},
+        "clocks": clocks,
+        "e2e": {"value": e2e_val, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": 32,
+                "ms_per_step": 1e3 * e2e_all / e2e_steps,
+                "what": "lgf_load_links(pinned host) + lgf_iterate(1) + result readback, every step"},
+        "gpu_launches": int(launches),
+        "roofline": {"bound": "hbm", "kernel": dom, "achieved": kern[dom]["GBps"], "peak": peak, "unit": "GB/s",
+                     "frac": kern[dom]["GBps"] / peak, "traffic": None, "peak_source": peak_src,
+                     "bytes_per_site": per[dom],
+                     "iteration": {"bytes_per_site": iter_bytes, "GBps": iter_bytes * V * K / (ms_all * 1e-3) / 1e9,
+                                   "frac": iter_bytes * V * K / (ms_all * 1e-3) / 1e9 / peak,
+                                   "ms_profiled": ms_prof / K},
+                     "kernels": kern},
+        "cpu_baseline": cpu,
+    }
+    print(json.dumps(out), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="32^4", choices=sorted(WORKLOADS))
+    ap.add_argument("--recon", type=int, default=0, choices=[0, 12, 18])
+    ap.add_argument("--fft-batch", type=int, default=4, choices=[4, 9])
+    ap.add_argument("--fft-path", type=int, default=0, choices=[0, 1])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

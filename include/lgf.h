@@ -1,0 +1,174 @@
+/*
+ * lgf.h -- C ABI of liblgf.so: Fourier-accelerated steepest-descent SU(3) Landau gauge
+ * fixing on a periodic 4D lattice (arXiv 1210.8018, Algorithm 1), on one
+ * NVIDIA B200 (sm_100a).
+ *
+ * Conventions
+ *   - Every function returns an int status: LGF_OK (0) or a negative LGF_ERR_* code.  No
+ *     exception, exit() or abort() crosses this boundary.  lgf_last_error(ctx) gives text.
+ *   - "host" / "device" is stated for every pointer.  Device pointers are plain CUDA device
+ *     addresses on the current device; the library never takes ownership of a caller buffer.
+ *   - The library allocates no device memory: the caller (PyTorch in this repo) hands it ONE
+ *     device workspace of lgf_workspace_bytes() bytes and a CUDA stream with lgf_bind().
+ *   - Not thread-safe per context; distinct contexts are independent.
+ *
+ * Lattice and layouts
+ *   extents N[0..3] = Nx, Ny, Nz, Nt;  V = Nx*Ny*Nz*Nt;  direction mu = 0..3 <-> x, y, z, t;
+ *   site index s = ix + Nx*(iy + Ny*(iz + Nz*it))  (x fastest, lexicographic).
+ *   Interchange layout of a link field (LGF_LAYOUT_AOS, the only one defined):
+ *       real[((((s*4 + mu)*3 + row)*3 + col)*2 + {0:re, 1:im}],   18 reals per link,
+ *   and of a site field (Delta, w, g):  real[(((s*3 + row)*3 + col)*2 + {re,im}].
+ *   `real` is double for LGF_PREC_FP64 contexts and float for LGF_PREC_FP32 contexts.
+ *   Inside the workspace links live as complex SoA arrays (one array over sites per matrix
+ *   element), 9 or 6 elements per link (12-real compression).
+ */
+#ifndef LGF_H
+#define LGF_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct lgf_ctx lgf_ctx;
+
+/* Result of lgf_iterate / lgf_fix.  F and theta are those of the final links. */
+typedef struct lgf_result {
+    int64_t iterations; /* executions of the loop body of Algorithm 1 (= link updates) in this call */
+    double F;           /* eq. 1.1 at g = 1 on the current links */
+    double theta;       /* eq. 1.4 */
+    int converged;      /* 1 if theta <= eps was reached (lgf_fix), else 0 */
+} lgf_result;
+
+enum {
+    LGF_OK = 0,
+    LGF_ERR_INVALID_ARG = -1,
+    LGF_ERR_UNSUPPORTED_SIZE = -2,
+    LGF_ERR_NOT_BOUND = -3,
+    LGF_ERR_NOT_LOADED = -4,
+    LGF_ERR_WORKSPACE_TOO_SMALL = -5,
+    LGF_ERR_CUDA = -6,
+    LGF_ERR_NOT_CONVERGED = -7,
+    LGF_ERR_NUMERIC = -8
+};
+
+enum { LGF_PREC_FP64 = 0, LGF_PREC_FP32 = 1 };
+enum { LGF_LAYOUT_AOS = 0 };
+
+/* lgf_set_option keys.  Options must be set before lgf_workspace_bytes / lgf_bind. */
+enum {
+    LGF_OPT_RECON = 1,          /* 18 (default) or 12 reals stored per link */
+    LGF_OPT_FFT_BATCH = 2,      /* 4 (default): Delta packed into 4 complex fields; 9: one FFT per
+                                   element of the Delta matrix as in Alg. 1 line 3 */
+    LGF_OPT_MAX_ITER = 3,       /* iteration cap of lgf_fix, default 100000 */
+    LGF_OPT_CHECK_INTERVAL = 4, /* iterations launched between two host polls of the device
+                                   `done` flag in lgf_fix, default 8.  Does not change results:
+                                   kernels launched after convergence exit at once. */
+    LGF_OPT_FFT_PATH = 5,       /* 0 (default): tiled register FFT when the extents allow it,
+                                   1: always the generic per-axis transform */
+    LGF_OPT_PROFILE = 6         /* 1: bracket every kernel launch with CUDA events on the bound
+                                   stream so that lgf_kernel_time works; default 0 */
+};
+
+/* lgf_get_field / lgf_set_field selectors */
+enum {
+    LGF_FIELD_DELTA = 0, /* Delta(x) of the current links, eq. 1.5 (valid after a measure) */
+    LGF_FIELD_W = 1,     /* w(x) = F^-1 (p_max^2/p^2) F Delta, normalised (valid after LGF_STAGE_FOURIER) */
+    LGF_FIELD_G = 2      /* g(x) = reunit(1 + (alpha/2) w(x)) built from the current w (get only) */
+};
+
+/* lgf_stage selectors: the three kernels of one iteration, for per-kernel parity tests */
+enum {
+    LGF_STAGE_MEASURE = 0, /* kernel (a): Delta, F, theta from the links */
+    LGF_STAGE_FOURIER = 1, /* kernel (b): Delta -> w in place (Alg. 1 lines 3-8) */
+    LGF_STAGE_UPDATE = 2   /* kernel (c): g(x), U_mu(x) <- g(x) U_mu(x) g^dagger(x+mu) */
+};
+
+/* kernel kinds for lgf_kernel_time */
+enum {
+    LGF_KERNEL_MEASURE = 0,
+    LGF_KERNEL_FFT_XY_FWD = 1,
+    LGF_KERNEL_FFT_ZT = 2,
+    LGF_KERNEL_FFT_XY_INV = 3,
+    LGF_KERNEL_UPDATE = 4,
+    LGF_KERNEL_FFT_GENERIC = 5,
+    LGF_KERNEL_LAYOUT = 6,
+    LGF_KERNEL_KINDS = 7
+};
+
+/* Create a context for an Nx*Ny*Nz*Nt lattice.  host call; allocates host memory only.
+ * Each extent must be even, 4 <= N <= 64, of the form 2^a 3^b; else LGF_ERR_UNSUPPORTED_SIZE.
+ * precision: LGF_PREC_FP64, or LGF_PREC_FP32 (storage, FFT and matrix arithmetic in float,
+ * F and theta accumulated in double).  *out (host) receives the context. */
+int lgf_create(int Nx, int Ny, int Nz, int Nt, int precision, lgf_ctx **out);
+
+/* Set an option (see LGF_OPT_*).  Must precede lgf_bind, except MAX_ITER, CHECK_INTERVAL, PROFILE. */
+int lgf_set_option(lgf_ctx *ctx, int key, int64_t value);
+
+/* Bytes of device workspace this context needs with its current options (0 on NULL). */
+size_t lgf_workspace_bytes(const lgf_ctx *ctx);
+
+/* Hand the context its device workspace (device pointer, 256-byte aligned, owned by the
+ * caller, must outlive the context's use) and the CUDA stream (a cudaStream_t passed as
+ * void*, may be NULL for the default stream) on which every kernel and copy is issued.
+ * Uploads the small tables (momentum tables 4 sin^2(pi k/N), twiddles). */
+int lgf_bind(lgf_ctx *ctx, void *dev_workspace, size_t bytes, void *cuda_stream);
+
+/* Load a link field in the interchange layout from host (src_is_device = 0) or device memory
+ * into the internal SoA arrays (dropping row 2 if RECON = 12), then run kernel (a) so that
+ * Delta, F, theta of the loaded links are available.  The source is not retained.
+ * Synchronises the stream before returning when the source is host memory. */
+int lgf_load_links(lgf_ctx *ctx, const void *src, int src_is_device, int src_layout);
+
+/* Inverse conversion into dst (host or device), third row rebuilt if RECON = 12.  Synchronous. */
+int lgf_get_links(lgf_ctx *ctx, void *dst, int dst_is_device, int dst_layout);
+
+/* Kernel (a) only: F and theta of the current links (host out pointers, may be NULL). Synchronous. */
+int lgf_measure(lgf_ctx *ctx, double *F, double *theta);
+
+/* Exactly n iterations of the loop body of Algorithm 1 with step alpha, never looking at
+ * theta (timed windows).  Asynchronous on the bound stream when out == NULL; otherwise
+ * synchronises and fills *out (host). */
+int lgf_iterate(lgf_ctx *ctx, double alpha, int64_t n, lgf_result *out);
+
+/* Algorithm 1: iterate while theta > eps (stop when theta <= eps).
+ * out->iterations = 0 if the loaded links already satisfy theta <= eps.  When MAX_ITER is
+ * reached returns LGF_ERR_NOT_CONVERGED with *out filled; NaN/Inf in theta returns
+ * LGF_ERR_NUMERIC.  The stop decision is taken on the device; the host polls it every
+ * CHECK_INTERVAL iterations. */
+int lgf_fix(lgf_ctx *ctx, double alpha, double eps, lgf_result *out);
+
+/* Run one kernel of the iteration (per-kernel parity).  alpha is used by LGF_STAGE_UPDATE only. */
+int lgf_stage(lgf_ctx *ctx, int stage, double alpha);
+
+/* Copy a site field in the interchange layout ([V][3][3] complex of the context's precision)
+ * out of / into the context.  LGF_FIELD_G needs alpha (ignored otherwise).  Synchronous. */
+int lgf_get_field(lgf_ctx *ctx, int which, double alpha, void *dst, int dst_is_device);
+int lgf_set_field(lgf_ctx *ctx, int which, const void *src, int src_is_device);
+
+/* (F, theta) after the initial measure and after each iteration of the last lgf_fix /
+ * lgf_iterate call: up to cap pairs into host arrays F[], theta[]; *n (host) = pairs written. */
+int lgf_history(lgf_ctx *ctx, double *F, double *theta, int cap, int *n);
+
+/* With LGF_OPT_PROFILE = 1: total milliseconds and launch count of one kernel kind since
+ * the last lgf_reset_counters, from CUDA events on the bound stream.  Synchronises. */
+int lgf_kernel_time(lgf_ctx *ctx, int kind, double *ms, int64_t *launches);
+/* Kernel launches issued by this context since the last reset (always counted). */
+int64_t lgf_launch_count(const lgf_ctx *ctx);
+int lgf_reset_counters(lgf_ctx *ctx);
+
+/* 1 if this context takes the tiled register-FFT path, 0 if the generic one. */
+int lgf_uses_tiled_fft(const lgf_ctx *ctx);
+
+/* Text of the last error of this context (or of lgf_create when ctx == NULL). Never NULL. */
+const char *lgf_last_error(const lgf_ctx *ctx);
+
+/* Free the context (host memory, events).  Caller buffers are never freed.  NULL is a no-op. */
+int lgf_destroy(lgf_ctx *ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* LGF_H */

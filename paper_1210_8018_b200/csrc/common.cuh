@@ -1,0 +1,65 @@
+// common.cuh -- shared device-side types of liblgf (CUDA path only; shares nothing with oracle/).
+//
+// Notation follows arXiv 1210.8018: V sites, N_c = 3, links U_mu(x), Delta(x) (eq. 1.5),
+// F (eq. 1.1), theta (eq. 1.4).  Site index s = ix + Nx*(iy + Ny*(iz + Nz*it)).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace lgf {
+
+// ---------------------------------------------------------------- complex numbers
+template <typename T> struct C2;
+template <> struct C2<double> { typedef double2 type; };
+template <> struct C2<float> { typedef float2 type; };
+template <typename T> using cx = typename C2<T>::type;
+
+template <typename T> __host__ __device__ __forceinline__ cx<T> mk(T re, T im) { cx<T> r; r.x = re; r.y = im; return r; }
+__device__ __forceinline__ double2 operator+(double2 a, double2 b) { return make_double2(a.x + b.x, a.y + b.y); }
+__device__ __forceinline__ double2 operator-(double2 a, double2 b) { return make_double2(a.x - b.x, a.y - b.y); }
+__device__ __forceinline__ float2 operator+(float2 a, float2 b) { return make_float2(a.x + b.x, a.y + b.y); }
+__device__ __forceinline__ float2 operator-(float2 a, float2 b) { return make_float2(a.x - b.x, a.y - b.y); }
+// a*b
+template <typename V> __device__ __forceinline__ V cmul(V a, V b) { V r; r.x = a.x * b.x - a.y * b.y; r.y = a.x * b.y + a.y * b.x; return r; }
+// a*conj(b)
+template <typename V> __device__ __forceinline__ V cmulc(V a, V b) { V r; r.x = a.x * b.x + a.y * b.y; r.y = a.y * b.x - a.x * b.y; return r; }
+// conj(a)*b
+template <typename V> __device__ __forceinline__ V cconjmul(V a, V b) { V r; r.x = a.x * b.x + a.y * b.y; r.y = a.x * b.y - a.y * b.x; return r; }
+// acc + a*b
+template <typename V> __device__ __forceinline__ V cfma(V a, V b, V acc) { acc.x += a.x * b.x - a.y * b.y; acc.y += a.x * b.y + a.y * b.x; return acc; }
+// acc + a*conj(b)
+template <typename V> __device__ __forceinline__ V cfmac(V a, V b, V acc) { acc.x += a.x * b.x + a.y * b.y; acc.y += a.y * b.x - a.x * b.y; return acc; }
+template <typename V> __device__ __forceinline__ V cconj(V a) { a.y = -a.y; return a; }
+template <typename V> __device__ __forceinline__ auto cnorm2(V a) -> decltype(a.x) { return a.x * a.x + a.y * a.y; }
+template <typename V, typename T> __device__ __forceinline__ V cscale(V a, T s) { a.x *= s; a.y *= s; return a; }
+
+// ---------------------------------------------------------------- lattice geometry
+struct Geom {
+    int N[4];        // Nx, Ny, Nz, Nt
+    int64_t V;       // sites
+    int64_t st[4];   // site-index stride of each direction: 1, Nx, Nx*Ny, Nx*Ny*Nz
+};
+
+__device__ __forceinline__ void site_coords(const Geom &g, int64_t s, int c[4])
+{
+    c[0] = (int)(s % g.N[0]); s /= g.N[0];
+    c[1] = (int)(s % g.N[1]); s /= g.N[1];
+    c[2] = (int)(s % g.N[2]); s /= g.N[2];
+    c[3] = (int)s;
+}
+
+// ---------------------------------------------------------------- device control block
+// One per context, in the workspace.  The stop decision of Algorithm 1 is
+// taken by the last block of kernel (a) and kept here, so that the host need not read
+// theta back after every iteration.
+#define LGF_HIST_CAP 4096
+struct Ctrl {
+    double F;                 // eq. 1.1 of the current links
+    double theta;             // eq. 1.4
+    long long iter;           // loop-body executions since the last reset
+    int done;                 // 0 running, 1 theta <= eps reached, 2 theta is NaN/Inf
+    unsigned int ticket;      // block counter of the fixed-order final reduction
+    int pad[2];
+};
+
+} // namespace lgf

@@ -1,0 +1,52 @@
+// launch.h -- internal interface between the host C-ABI (lgf_api.cu) and the kernel files.
+#pragma once
+#include "common.cuh"
+
+namespace lgf {
+
+struct SiteArgs {
+    Geom geo;
+    void *links;        // device: cx<T> [4][NE][V]
+    void *w;            // device: cx<T> [PACK][V]   (Delta, then w, in place)
+    Ctrl *ctrl;         // device
+    double *partials;   // device: 2 doubles per block of kernel (a)
+    double2 *hist;      // device: LGF_HIST_CAP pairs (F, theta)
+    int prec;           // 0 = FP64, 1 = FP32
+    int recon;          // 18 or 12
+    int pack;           // 4 or 9
+};
+
+// kernel (a): Delta, F, theta (eq. 1.5, 1.1, 1.4).  eps < 0: never raise `done`.
+void launch_measure(const SiteArgs &a, double eps, int count_iter, cudaStream_t st);
+int measure_blocks(int64_t V);
+// kernel (c): g(x) = reunit(1 + (alpha/2) w), U_mu(x) <- g(x) U_mu(x) g^dagger(x+mu)
+void launch_update(const SiteArgs &a, double alpha, cudaStream_t st);
+// iter = 0, hist[0] = (F, theta), done = (theta <= eps)
+void launch_ctrl_reset(const SiteArgs &a, double eps, cudaStream_t st);
+
+// interchange layout <-> SoA, for `count` sites starting at site s0; aos points at site s0
+void launch_aos_to_soa(const SiteArgs &a, const void *aos, int64_t s0, int64_t count, cudaStream_t st);
+void launch_soa_to_aos(const SiteArgs &a, void *aos, int64_t s0, int64_t count, cudaStream_t st);
+// site-field taps ([count][3][3] complex); which: 0 Delta / 1 w (same unpacking), 2 g
+void launch_field_get(const SiteArgs &a, int which, double alpha, void *aos, int64_t s0, int64_t count, cudaStream_t st);
+void launch_field_set(const SiteArgs &a, const void *aos, int64_t s0, int64_t count, cudaStream_t st);
+
+// ---- Fourier acceleration (Alg. 1 lines 3-8): w <- F^-1 [p_max^2/(p^2 V)] F w, zero mode -> 0
+struct FftArgs {
+    Geom geo;
+    void *w;            // device: cx<T> [nfields][V]
+    int nfields;
+    int prec;
+    const double *ptab; // device: 4 sin^2(pi k/N_mu), the four tables back to back (N0+N1+N2+N3)
+    double pmax2;       // max_k p^2(k)
+    const void *tw;     // device: cx<T> forward twiddles exp(-2 pi i k/N_mu), four tables back to back
+    const Ctrl *ctrl;
+};
+// generic per-axis transform: any extent, O(N^2) per line.  Returns launches issued.
+int launch_fft_generic(const FftArgs &a, cudaStream_t st);
+// tiled register FFT: three passes.  which = 0 (x,y) forward, 1 (z,t) forward*mask*inverse, 2 (x,y) inverse
+bool fft_tiled_supported(const int N[4], int prec);
+void launch_fft_tiled(const FftArgs &a, int which, cudaStream_t st);
+int fft_tiled_setup(const int N[4], int prec); // sets kernel attributes (smem opt-in); 0 on success
+
+} // namespace lgf

@@ -1,0 +1,553 @@
+// lgf_api.cu -- host side of liblgf.so: the C ABI declared in include/lgf.h.
+// Owns no device memory: carves the caller's workspace, launches the kernels of
+// kernels_site.cu / fft_tiled.cu / fft_generic.cu on the caller's stream, and keeps the
+// loop of Algorithm 1 on the device between polls of the `done` flag.
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "../../include/lgf.h"
+#include "launch.h"
+
+using namespace lgf;
+
+namespace {
+
+const double kTwoPi = 6.283185307179586476925286766559;
+std::string g_create_err = "";
+
+struct EvPair { cudaEvent_t a, b; int kind; };
+
+size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+
+struct Layout {
+    size_t links, w, partials, ctrl, hist, ptab, tw, staging, total;
+    int64_t staging_sites;
+};
+
+} // namespace
+
+struct lgf_ctx {
+    int N[4];
+    int64_t V;
+    int prec;
+    int recon = 18, pack = 4, check_interval = 8, fft_path = 0, profile = 0;
+    int64_t max_iter = 100000;
+    bool bound = false, loaded = false;
+    int wstate = 0; // 0 invalid, 1 holds Delta of the current links, 2 holds w
+    cudaStream_t st = nullptr;
+    char *base = nullptr;
+    Layout lay{};
+    SiteArgs sa{};
+    FftArgs fa{};
+    bool tiled = false;
+    std::vector<double> ptab_h;
+    double pmax2 = 0;
+    int64_t launches = 0;
+    std::vector<EvPair> evs;
+    size_t ev_used = 0;
+    double kms[LGF_KERNEL_KINDS] = {0};
+    int64_t kcount[LGF_KERNEL_KINDS] = {0};
+    std::string err;
+};
+
+namespace {
+
+size_t elem_bytes(const lgf_ctx *c) { return c->prec == LGF_PREC_FP64 ? 16 : 8; }
+int sum_n(const lgf_ctx *c) { return c->N[0] + c->N[1] + c->N[2] + c->N[3]; }
+
+Layout make_layout(const lgf_ctx *c)
+{
+    Layout L{};
+    const size_t e = elem_bytes(c);
+    const int ne = c->recon == 12 ? 6 : 9;
+    size_t off = 0;
+    L.links = off; off = align_up(off + (size_t)4 * ne * c->V * e, 256);
+    L.w = off; off = align_up(off + (size_t)c->pack * c->V * e, 256);
+    L.partials = off; off = align_up(off + (size_t)2 * measure_blocks(c->V) * sizeof(double), 256);
+    L.ctrl = off; off = align_up(off + sizeof(Ctrl), 256);
+    L.hist = off; off = align_up(off + (size_t)LGF_HIST_CAP * sizeof(double2), 256);
+    L.ptab = off; off = align_up(off + (size_t)sum_n(c) * sizeof(double), 256);
+    L.tw = off; off = align_up(off + (size_t)sum_n(c) * e, 256);
+    L.staging_sites = c->V < (1 << 17) ? c->V : (1 << 17);
+    L.staging = off; off = align_up(off + (size_t)L.staging_sites * 36 * e, 256);
+    L.total = off;
+    return L;
+}
+
+int fail(lgf_ctx *c, int code, const std::string &msg)
+{
+    if (c) c->err = msg; else g_create_err = msg;
+    return code;
+}
+
+int cuda_fail(lgf_ctx *c, cudaError_t e, const char *what)
+{
+    return fail(c, LGF_ERR_CUDA, std::string(what) + ": " + cudaGetErrorString(e));
+}
+
+#define CK(call)                                                   \
+    do {                                                           \
+        cudaError_t e_ = (call);                                   \
+        if (e_ != cudaSuccess) return cuda_fail(ctx, e_, #call);   \
+    } while (0)
+
+bool smooth23(int n)
+{
+    while (n % 2 == 0) n /= 2;
+    while (n % 3 == 0) n /= 3;
+    return n == 1;
+}
+
+// bracket a launch with events when profiling
+template <typename F> void run_kernel(lgf_ctx *c, int kind, int nlaunch, F f)
+{
+    if (c->profile) {
+        if (c->ev_used == c->evs.size()) {
+            EvPair p;
+            cudaEventCreate(&p.a);
+            cudaEventCreate(&p.b);
+            p.kind = kind;
+            c->evs.push_back(p);
+        }
+        EvPair &p = c->evs[c->ev_used++];
+        p.kind = kind;
+        cudaEventRecord(p.a, c->st);
+        f();
+        cudaEventRecord(p.b, c->st);
+    } else {
+        f();
+    }
+    c->launches += nlaunch;
+    c->kcount[kind] += nlaunch;
+}
+
+void flush_events(lgf_ctx *c)
+{
+    if (!c->ev_used) return;
+    cudaStreamSynchronize(c->st);
+    for (size_t i = 0; i < c->ev_used; i++) {
+        float ms = 0;
+        if (cudaEventElapsedTime(&ms, c->evs[i].a, c->evs[i].b) == cudaSuccess) c->kms[c->evs[i].kind] += ms;
+    }
+    c->ev_used = 0;
+}
+
+void do_measure(lgf_ctx *c, double eps, int count_iter)
+{
+    run_kernel(c, LGF_KERNEL_MEASURE, 1, [&] { launch_measure(c->sa, eps, count_iter, c->st); });
+    c->wstate = 1;
+}
+
+void do_fourier(lgf_ctx *c)
+{
+    if (c->tiled) {
+        run_kernel(c, LGF_KERNEL_FFT_XY_FWD, 1, [&] { launch_fft_tiled(c->fa, 0, c->st); });
+        run_kernel(c, LGF_KERNEL_FFT_ZT, 1, [&] { launch_fft_tiled(c->fa, 1, c->st); });
+        run_kernel(c, LGF_KERNEL_FFT_XY_INV, 1, [&] { launch_fft_tiled(c->fa, 2, c->st); });
+    } else {
+        run_kernel(c, LGF_KERNEL_FFT_GENERIC, 8, [&] { launch_fft_generic(c->fa, c->st); });
+    }
+    c->wstate = 2;
+}
+
+void do_update(lgf_ctx *c, double alpha)
+{
+    run_kernel(c, LGF_KERNEL_UPDATE, 1, [&] { launch_update(c->sa, alpha, c->st); });
+    c->wstate = 0;
+}
+
+// one execution of the loop body of Algorithm 1 (lines 3-17) on the device
+void do_iteration(lgf_ctx *c, double alpha, double eps)
+{
+    do_fourier(c);
+    do_update(c, alpha);
+    do_measure(c, eps, 1);
+}
+
+int read_ctrl(lgf_ctx *ctx, Ctrl *h)
+{
+    CK(cudaMemcpyAsync(h, ctx->sa.ctrl, sizeof(Ctrl), cudaMemcpyDeviceToHost, ctx->st));
+    CK(cudaStreamSynchronize(ctx->st));
+    CK(cudaGetLastError());
+    return LGF_OK;
+}
+
+int clear_done(lgf_ctx *ctx)
+{
+    CK(cudaMemsetAsync(&ctx->sa.ctrl->done, 0, sizeof(int), ctx->st));
+    return LGF_OK;
+}
+
+int need_loaded(lgf_ctx *ctx)
+{
+    if (!ctx) return LGF_ERR_INVALID_ARG;
+    if (!ctx->bound) return fail(ctx, LGF_ERR_NOT_BOUND, "lgf_bind has not been called");
+    if (!ctx->loaded) return fail(ctx, LGF_ERR_NOT_LOADED, "lgf_load_links has not been called");
+    return LGF_OK;
+}
+
+} // namespace
+
+extern "C" {
+
+int lgf_create(int Nx, int Ny, int Nz, int Nt, int precision, lgf_ctx **out)
+{
+    if (!out) return fail(nullptr, LGF_ERR_INVALID_ARG, "out is NULL");
+    *out = nullptr;
+    if (precision != LGF_PREC_FP64 && precision != LGF_PREC_FP32)
+        return fail(nullptr, LGF_ERR_INVALID_ARG, "precision must be LGF_PREC_FP64 or LGF_PREC_FP32");
+    const int N[4] = {Nx, Ny, Nz, Nt};
+    for (int d = 0; d < 4; d++)
+        if (N[d] < 4 || N[d] > 64 || (N[d] & 1) || !smooth23(N[d]))
+            return fail(nullptr, LGF_ERR_UNSUPPORTED_SIZE, "each extent must be even, 4 <= N <= 64, of the form 2^a 3^b");
+    lgf_ctx *c = new (std::nothrow) lgf_ctx;
+    if (!c) return fail(nullptr, LGF_ERR_INVALID_ARG, "out of host memory");
+    for (int d = 0; d < 4; d++) c->N[d] = N[d];
+    c->V = (int64_t)Nx * Ny * Nz * Nt;
+    c->prec = precision;
+    // s_mu[k] = 4 sin^2(pi k/N_mu): eigenvalues of minus the lattice second difference
+    // (reading R5); p_max^2 = sum_mu max_k s_mu[k] (reading R6).
+    c->pmax2 = 0;
+    for (int d = 0; d < 4; d++) {
+        double m = 0;
+        for (int k = 0; k < N[d]; k++) {
+            const double sn = std::sin(0.5 * kTwoPi * (double)k / (double)N[d]);
+            const double v = 4.0 * sn * sn;
+            c->ptab_h.push_back(v);
+            if (v > m) m = v;
+        }
+        c->pmax2 += m;
+    }
+    *out = c;
+    return LGF_OK;
+}
+
+int lgf_set_option(lgf_ctx *ctx, int key, int64_t value)
+{
+    if (!ctx) return LGF_ERR_INVALID_ARG;
+    const bool layout_key = (key == LGF_OPT_RECON || key == LGF_OPT_FFT_BATCH || key == LGF_OPT_FFT_PATH);
+    if (layout_key && ctx->bound) return fail(ctx, LGF_ERR_INVALID_ARG, "this option must be set before lgf_bind");
+    switch (key) {
+    case LGF_OPT_RECON:
+        if (value != 12 && value != 18) return fail(ctx, LGF_ERR_INVALID_ARG, "RECON must be 12 or 18");
+        ctx->recon = (int)value; break;
+    case LGF_OPT_FFT_BATCH:
+        if (value != 4 && value != 9) return fail(ctx, LGF_ERR_INVALID_ARG, "FFT_BATCH must be 4 or 9");
+        ctx->pack = (int)value; break;
+    case LGF_OPT_MAX_ITER:
+        if (value < 0) return fail(ctx, LGF_ERR_INVALID_ARG, "MAX_ITER must be >= 0");
+        ctx->max_iter = value; break;
+    case LGF_OPT_CHECK_INTERVAL:
+        if (value < 1 || value > 1024) return fail(ctx, LGF_ERR_INVALID_ARG, "CHECK_INTERVAL must be in 1..1024");
+        ctx->check_interval = (int)value; break;
+    case LGF_OPT_FFT_PATH:
+        if (value != 0 && value != 1) return fail(ctx, LGF_ERR_INVALID_ARG, "FFT_PATH must be 0 or 1");
+        ctx->fft_path = (int)value; break;
+    case LGF_OPT_PROFILE:
+        if (ctx->bound) flush_events(ctx);
+        ctx->profile = value ? 1 : 0; break;
+    default:
+        return fail(ctx, LGF_ERR_INVALID_ARG, "unknown option key");
+    }
+    return LGF_OK;
+}
+
+size_t lgf_workspace_bytes(const lgf_ctx *ctx)
+{
+    if (!ctx) return 0;
+    return make_layout(ctx).total;
+}
+
+int lgf_bind(lgf_ctx *ctx, void *dev_workspace, size_t bytes, void *cuda_stream)
+{
+    if (!ctx) return LGF_ERR_INVALID_ARG;
+    if (!dev_workspace) return fail(ctx, LGF_ERR_INVALID_ARG, "dev_workspace is NULL");
+    if (((uintptr_t)dev_workspace) & 255) return fail(ctx, LGF_ERR_INVALID_ARG, "dev_workspace must be 256-byte aligned");
+    const Layout L = make_layout(ctx);
+    if (bytes < L.total) return fail(ctx, LGF_ERR_WORKSPACE_TOO_SMALL, "workspace smaller than lgf_workspace_bytes()");
+    ctx->lay = L;
+    ctx->base = (char *)dev_workspace;
+    ctx->st = (cudaStream_t)cuda_stream;
+    Geom g{};
+    for (int d = 0; d < 4; d++) g.N[d] = ctx->N[d];
+    g.V = ctx->V;
+    g.st[0] = 1; g.st[1] = g.N[0]; g.st[2] = (int64_t)g.N[0] * g.N[1]; g.st[3] = (int64_t)g.N[0] * g.N[1] * g.N[2];
+    SiteArgs &s = ctx->sa;
+    s.geo = g;
+    s.links = ctx->base + L.links;
+    s.w = ctx->base + L.w;
+    s.partials = (double *)(ctx->base + L.partials);
+    s.ctrl = (Ctrl *)(ctx->base + L.ctrl);
+    s.hist = (double2 *)(ctx->base + L.hist);
+    s.prec = ctx->prec; s.recon = ctx->recon; s.pack = ctx->pack;
+    FftArgs &f = ctx->fa;
+    f.geo = g; f.w = s.w; f.nfields = ctx->pack; f.prec = ctx->prec;
+    f.ptab = (const double *)(ctx->base + L.ptab);
+    f.pmax2 = ctx->pmax2;
+    f.tw = ctx->base + L.tw;
+    f.ctrl = s.ctrl;
+    // tables: momentum tables and forward twiddles exp(-2 pi i k/N), computed in FP64, rounded once (R19)
+    const int sn = sum_n(ctx);
+    CK(cudaMemcpyAsync(ctx->base + L.ptab, ctx->ptab_h.data(), sizeof(double) * sn, cudaMemcpyHostToDevice, ctx->st));
+    std::vector<double> twd(2 * sn);
+    std::vector<float> twf(2 * sn);
+    int o = 0;
+    for (int d = 0; d < 4; d++)
+        for (int k = 0; k < ctx->N[d]; k++, o++) {
+            const double ang = kTwoPi * (double)k / (double)ctx->N[d];
+            twd[2 * o] = std::cos(ang); twd[2 * o + 1] = -std::sin(ang);
+            twf[2 * o] = (float)twd[2 * o]; twf[2 * o + 1] = (float)twd[2 * o + 1];
+        }
+    if (ctx->prec == LGF_PREC_FP64) CK(cudaMemcpyAsync(ctx->base + L.tw, twd.data(), sizeof(double) * 2 * sn, cudaMemcpyHostToDevice, ctx->st));
+    else CK(cudaMemcpyAsync(ctx->base + L.tw, twf.data(), sizeof(float) * 2 * sn, cudaMemcpyHostToDevice, ctx->st));
+    CK(cudaMemsetAsync(s.ctrl, 0, sizeof(Ctrl), ctx->st));
+    CK(cudaMemsetAsync(s.hist, 0, sizeof(double2) * LGF_HIST_CAP, ctx->st));
+    CK(cudaStreamSynchronize(ctx->st)); // the host vectors above go out of scope
+    ctx->tiled = (ctx->fft_path == 0) && fft_tiled_supported(ctx->N, ctx->prec);
+    if (ctx->tiled && fft_tiled_setup(ctx->N, ctx->prec) != 0) {
+        cudaError_t e = cudaGetLastError();
+        return cuda_fail(ctx, e, "fft_tiled_setup");
+    }
+    ctx->bound = true;
+    ctx->loaded = false;
+    ctx->wstate = 0;
+    return LGF_OK;
+}
+
+int lgf_load_links(lgf_ctx *ctx, const void *src, int src_is_device, int src_layout)
+{
+    if (!ctx) return LGF_ERR_INVALID_ARG;
+    if (!ctx->bound) return fail(ctx, LGF_ERR_NOT_BOUND, "lgf_bind has not been called");
+    if (!src) return fail(ctx, LGF_ERR_INVALID_ARG, "src is NULL");
+    if (src_layout != LGF_LAYOUT_AOS) return fail(ctx, LGF_ERR_INVALID_ARG, "unknown layout");
+    const size_t e = elem_bytes(ctx);
+    if (src_is_device) {
+        run_kernel(ctx, LGF_KERNEL_LAYOUT, 1, [&] { launch_aos_to_soa(ctx->sa, src, 0, ctx->V, ctx->st); });
+    } else {
+        char *stg = ctx->base + ctx->lay.staging;
+        for (int64_t s0 = 0; s0 < ctx->V; s0 += ctx->lay.staging_sites) {
+            const int64_t n = std::min<int64_t>(ctx->lay.staging_sites, ctx->V - s0);
+            CK(cudaMemcpyAsync(stg, (const char *)src + (size_t)s0 * 36 * e, (size_t)n * 36 * e, cudaMemcpyHostToDevice, ctx->st));
+            run_kernel(ctx, LGF_KERNEL_LAYOUT, 1, [&] { launch_aos_to_soa(ctx->sa, stg, s0, n, ctx->st); });
+        }
+    }
+    int rc = clear_done(ctx);
+    if (rc) return rc;
+    do_measure(ctx, -1.0, 0);
+    CK(cudaGetLastError());
+    if (!src_is_device) CK(cudaStreamSynchronize(ctx->st));
+    ctx->loaded = true;
+    return LGF_OK;
+}
+
+int lgf_get_links(lgf_ctx *ctx, void *dst, int dst_is_device, int dst_layout)
+{
+    int rc = need_loaded(ctx);
+    if (rc) return rc;
+    if (!dst) return fail(ctx, LGF_ERR_INVALID_ARG, "dst is NULL");
+    if (dst_layout != LGF_LAYOUT_AOS) return fail(ctx, LGF_ERR_INVALID_ARG, "unknown layout");
+    const size_t e = elem_bytes(ctx);
+    if (dst_is_device) {
+        run_kernel(ctx, LGF_KERNEL_LAYOUT, 1, [&] { launch_soa_to_aos(ctx->sa, dst, 0, ctx->V, ctx->st); });
+    } else {
+        char *stg = ctx->base + ctx->lay.staging;
+        for (int64_t s0 = 0; s0 < ctx->V; s0 += ctx->lay.staging_sites) {
+            const int64_t n = std::min<int64_t>(ctx->lay.staging_sites, ctx->V - s0);
+            run_kernel(ctx, LGF_KERNEL_LAYOUT, 1, [&] { launch_soa_to_aos(ctx->sa, stg, s0, n, ctx->st); });
+            CK(cudaMemcpyAsync((char *)dst + (size_t)s0 * 36 * e, stg, (size_t)n * 36 * e, cudaMemcpyDeviceToHost, ctx->st));
+        }
+    }
+    CK(cudaStreamSynchronize(ctx->st));
+    CK(cudaGetLastError());
+    return LGF_OK;
+}
+
+int lgf_measure(lgf_ctx *ctx, double *F, double *theta)
+{
+    int rc = need_loaded(ctx);
+    if (rc) return rc;
+    if ((rc = clear_done(ctx))) return rc;
+    do_measure(ctx, -1.0, 0);
+    Ctrl h;
+    if ((rc = read_ctrl(ctx, &h))) return rc;
+    if (F) *F = h.F;
+    if (theta) *theta = h.theta;
+    return LGF_OK;
+}
+
+int lgf_iterate(lgf_ctx *ctx, double alpha, int64_t n, lgf_result *out)
+{
+    int rc = need_loaded(ctx);
+    if (rc) return rc;
+    if (n < 0) return fail(ctx, LGF_ERR_INVALID_ARG, "n must be >= 0");
+    if (ctx->wstate != 1) {
+        if ((rc = clear_done(ctx))) return rc;
+        do_measure(ctx, -1.0, 0);
+    }
+    run_kernel(ctx, LGF_KERNEL_LAYOUT, 1, [&] { launch_ctrl_reset(ctx->sa, -1.0, ctx->st); });
+    for (int64_t i = 0; i < n; i++) do_iteration(ctx, alpha, -1.0);
+    CK(cudaGetLastError());
+    if (out) {
+        Ctrl h;
+        if ((rc = read_ctrl(ctx, &h))) return rc;
+        out->iterations = h.iter; out->F = h.F; out->theta = h.theta; out->converged = 0;
+        if (h.done == 2) return fail(ctx, LGF_ERR_NUMERIC, "theta is NaN or Inf");
+    }
+    return LGF_OK;
+}
+
+int lgf_fix(lgf_ctx *ctx, double alpha, double eps, lgf_result *out)
+{
+    int rc = need_loaded(ctx);
+    if (rc) return rc;
+    if (!(eps >= 0)) return fail(ctx, LGF_ERR_INVALID_ARG, "eps must be >= 0");
+    if (ctx->wstate != 1) {
+        if ((rc = clear_done(ctx))) return rc;
+        do_measure(ctx, -1.0, 0);
+    }
+    run_kernel(ctx, LGF_KERNEL_LAYOUT, 1, [&] { launch_ctrl_reset(ctx->sa, eps, ctx->st); });
+    Ctrl h;
+    if ((rc = read_ctrl(ctx, &h))) return rc;
+    int64_t launched = 0;
+    while (!h.done && launched < ctx->max_iter) {
+        const int64_t n = std::min<int64_t>(ctx->check_interval, ctx->max_iter - launched);
+        for (int64_t i = 0; i < n; i++) do_iteration(ctx, alpha, eps);
+        launched += n;
+        CK(cudaGetLastError());
+        if ((rc = read_ctrl(ctx, &h))) return rc;
+    }
+    ctx->wstate = 1; // kernels after `done` exited at once: w still holds Delta of the final links
+    if (out) { out->iterations = h.iter; out->F = h.F; out->theta = h.theta; out->converged = (h.done == 1); }
+    if (h.done == 2) return fail(ctx, LGF_ERR_NUMERIC, "theta is NaN or Inf");
+    if (!h.done) return fail(ctx, LGF_ERR_NOT_CONVERGED, "MAX_ITER reached before theta <= eps");
+    return LGF_OK;
+}
+
+int lgf_stage(lgf_ctx *ctx, int stage, double alpha)
+{
+    int rc = need_loaded(ctx);
+    if (rc) return rc;
+    if ((rc = clear_done(ctx))) return rc;
+    switch (stage) {
+    case LGF_STAGE_MEASURE: do_measure(ctx, -1.0, 0); break;
+    case LGF_STAGE_FOURIER:
+        if (ctx->wstate != 1) return fail(ctx, LGF_ERR_INVALID_ARG, "FOURIER needs Delta in the field buffer (run MEASURE or set DELTA)");
+        do_fourier(ctx); break;
+    case LGF_STAGE_UPDATE:
+        if (ctx->wstate != 2) return fail(ctx, LGF_ERR_INVALID_ARG, "UPDATE needs w in the field buffer (run FOURIER or set W)");
+        do_update(ctx, alpha); break;
+    default: return fail(ctx, LGF_ERR_INVALID_ARG, "unknown stage");
+    }
+    CK(cudaStreamSynchronize(ctx->st));
+    CK(cudaGetLastError());
+    return LGF_OK;
+}
+
+int lgf_get_field(lgf_ctx *ctx, int which, double alpha, void *dst, int dst_is_device)
+{
+    int rc = need_loaded(ctx);
+    if (rc) return rc;
+    if (!dst) return fail(ctx, LGF_ERR_INVALID_ARG, "dst is NULL");
+    if (which == LGF_FIELD_DELTA) { if (ctx->wstate != 1) return fail(ctx, LGF_ERR_INVALID_ARG, "field buffer does not hold Delta"); }
+    else if (which == LGF_FIELD_W || which == LGF_FIELD_G) { if (ctx->wstate != 2) return fail(ctx, LGF_ERR_INVALID_ARG, "field buffer does not hold w"); }
+    else return fail(ctx, LGF_ERR_INVALID_ARG, "unknown field");
+    const size_t e = elem_bytes(ctx);
+    if (dst_is_device) {
+        run_kernel(ctx, LGF_KERNEL_LAYOUT, 1, [&] { launch_field_get(ctx->sa, which, alpha, dst, 0, ctx->V, ctx->st); });
+    } else {
+        char *stg = ctx->base + ctx->lay.staging;
+        for (int64_t s0 = 0; s0 < ctx->V; s0 += ctx->lay.staging_sites) {
+            const int64_t n = std::min<int64_t>(ctx->lay.staging_sites, ctx->V - s0);
+            run_kernel(ctx, LGF_KERNEL_LAYOUT, 1, [&] { launch_field_get(ctx->sa, which, alpha, stg, s0, n, ctx->st); });
+            CK(cudaMemcpyAsync((char *)dst + (size_t)s0 * 9 * e, stg, (size_t)n * 9 * e, cudaMemcpyDeviceToHost, ctx->st));
+        }
+    }
+    CK(cudaStreamSynchronize(ctx->st));
+    CK(cudaGetLastError());
+    return LGF_OK;
+}
+
+int lgf_set_field(lgf_ctx *ctx, int which, const void *src, int src_is_device)
+{
+    int rc = need_loaded(ctx);
+    if (rc) return rc;
+    if (!src) return fail(ctx, LGF_ERR_INVALID_ARG, "src is NULL");
+    if (which != LGF_FIELD_DELTA && which != LGF_FIELD_W) return fail(ctx, LGF_ERR_INVALID_ARG, "only DELTA and W can be set");
+    const size_t e = elem_bytes(ctx);
+    if (src_is_device) {
+        run_kernel(ctx, LGF_KERNEL_LAYOUT, 1, [&] { launch_field_set(ctx->sa, src, 0, ctx->V, ctx->st); });
+    } else {
+        char *stg = ctx->base + ctx->lay.staging;
+        for (int64_t s0 = 0; s0 < ctx->V; s0 += ctx->lay.staging_sites) {
+            const int64_t n = std::min<int64_t>(ctx->lay.staging_sites, ctx->V - s0);
+            CK(cudaMemcpyAsync(stg, (const char *)src + (size_t)s0 * 9 * e, (size_t)n * 9 * e, cudaMemcpyHostToDevice, ctx->st));
+            run_kernel(ctx, LGF_KERNEL_LAYOUT, 1, [&] { launch_field_set(ctx->sa, stg, s0, n, ctx->st); });
+        }
+    }
+    CK(cudaStreamSynchronize(ctx->st));
+    CK(cudaGetLastError());
+    ctx->wstate = (which == LGF_FIELD_DELTA) ? 1 : 2;
+    return LGF_OK;
+}
+
+int lgf_history(lgf_ctx *ctx, double *F, double *theta, int cap, int *n)
+{
+    int rc = need_loaded(ctx);
+    if (rc) return rc;
+    if (!n || cap < 0) return fail(ctx, LGF_ERR_INVALID_ARG, "bad arguments");
+    Ctrl h;
+    if ((rc = read_ctrl(ctx, &h))) return rc;
+    int64_t cnt = h.iter + 1;
+    if (cnt > LGF_HIST_CAP) cnt = LGF_HIST_CAP;
+    if (cnt > cap) cnt = cap;
+    std::vector<double2> tmp((size_t)cnt);
+    if (cnt) {
+        CK(cudaMemcpyAsync(tmp.data(), ctx->sa.hist, sizeof(double2) * (size_t)cnt, cudaMemcpyDeviceToHost, ctx->st));
+        CK(cudaStreamSynchronize(ctx->st));
+    }
+    for (int64_t i = 0; i < cnt; i++) {
+        if (F) F[i] = tmp[(size_t)i].x;
+        if (theta) theta[i] = tmp[(size_t)i].y;
+    }
+    *n = (int)cnt;
+    return LGF_OK;
+}
+
+int lgf_kernel_time(lgf_ctx *ctx, int kind, double *ms, int64_t *launches)
+{
+    if (!ctx) return LGF_ERR_INVALID_ARG;
+    if (kind < 0 || kind >= LGF_KERNEL_KINDS) return fail(ctx, LGF_ERR_INVALID_ARG, "unknown kernel kind");
+    if (ctx->bound) flush_events(ctx);
+    if (ms) *ms = ctx->kms[kind];
+    if (launches) *launches = ctx->kcount[kind];
+    return LGF_OK;
+}
+
+int64_t lgf_launch_count(const lgf_ctx *ctx) { return ctx ? ctx->launches : 0; }
+
+int lgf_reset_counters(lgf_ctx *ctx)
+{
+    if (!ctx) return LGF_ERR_INVALID_ARG;
+    if (ctx->bound) flush_events(ctx);
+    ctx->launches = 0;
+    for (int k = 0; k < LGF_KERNEL_KINDS; k++) { ctx->kms[k] = 0; ctx->kcount[k] = 0; }
+    return LGF_OK;
+}
+
+int lgf_uses_tiled_fft(const lgf_ctx *ctx) { return ctx && ctx->tiled ? 1 : 0; }
+
+const char *lgf_last_error(const lgf_ctx *ctx) { return ctx ? ctx->err.c_str() : g_create_err.c_str(); }
+
+int lgf_destroy(lgf_ctx *ctx)
+{
+    if (!ctx) return LGF_OK;
+    for (auto &p : ctx->evs) { cudaEventDestroy(p.a); cudaEventDestroy(p.b); }
+    delete ctx;
+    return LGF_OK;
+}
+
+} // extern "C"

@@ -1,0 +1,103 @@
+// su3.cuh -- 3x3 complex matrix helpers in registers (CUDA path only).
+#pragma once
+#include "common.cuh"
+
+namespace lgf {
+
+// Third row of a special unitary matrix from rows 0, 1: row2 = conj(row0 x row1)
+// (12-real compression; reading R15).  m[0..5] given, m[6..8] written.
+template <typename V> __device__ __forceinline__ void su3_row2(V (&m)[9])
+{
+    m[6] = cconj(cmul(m[1], m[5]) - cmul(m[2], m[4]));
+    m[7] = cconj(cmul(m[2], m[3]) - cmul(m[0], m[5]));
+    m[8] = cconj(cmul(m[0], m[4]) - cmul(m[1], m[3]));
+}
+
+// Load U_mu(s) from the SoA link arrays: element k = 3*row + col of direction mu lives at
+// links[(mu*NE + k)*V + s], NE = 9 (18-real) or 6 (12-real, row 2 rebuilt here).
+template <typename T, int NE>
+__device__ __forceinline__ void load_link(const cx<T> *__restrict__ links, int64_t V, int mu, int64_t s, cx<T> (&u)[9])
+{
+    const cx<T> *p = links + (int64_t)mu * NE * V + s;
+#pragma unroll
+    for (int k = 0; k < NE; k++) u[k] = __ldg(p + (int64_t)k * V);
+    if (NE == 6) su3_row2(u);
+}
+
+template <typename T> __device__ __forceinline__ T rsqrt_t(T x);
+template <> __device__ __forceinline__ double rsqrt_t<double>(double x) { return rsqrt(x); }
+template <> __device__ __forceinline__ float rsqrt_t<float>(float x) { return rsqrtf(x); }
+
+// g = reunit(m): Gram-Schmidt on rows 0, 1 of m, row 2 = conj(row0 x row1)
+// ("followed by a reunitarization"; readings R12, R13).
+// m[0..5] = rows 0, 1 on entry; g[0..8] on exit.
+template <typename T> __device__ __forceinline__ void reunit(cx<T> (&g)[9])
+{
+    T n0 = rsqrt_t<T>(cnorm2(g[0]) + cnorm2(g[1]) + cnorm2(g[2]));
+    g[0] = cscale(g[0], n0); g[1] = cscale(g[1], n0); g[2] = cscale(g[2], n0);
+    // <u, m1> = sum_j conj(u_j) m_1j
+    cx<T> ip = cconjmul(g[0], g[3]);
+    ip = ip + cconjmul(g[1], g[4]);
+    ip = ip + cconjmul(g[2], g[5]);
+    g[3] = g[3] - cmul(ip, g[0]);
+    g[4] = g[4] - cmul(ip, g[1]);
+    g[5] = g[5] - cmul(ip, g[2]);
+    T n1 = rsqrt_t<T>(cnorm2(g[3]) + cnorm2(g[4]) + cnorm2(g[5]));
+    g[3] = cscale(g[3], n1); g[4] = cscale(g[4], n1); g[5] = cscale(g[5], n1);
+    su3_row2(g);
+}
+
+// Rows 0, 1 of w(x) from the field buffer, then g(x) = reunit(1 + (alpha/2) w(x)), a = alpha/2
+// (first order of eq. 1.2).
+// PACK = 9: field k = 3*row+col holds w_rowcol (one FFT per matrix element, Alg. 1 line 3).
+// PACK = 4: w is anti-Hermitian and traceless (the mask is real and even), so its 8 real
+//   degrees of freedom are kept as  f0 = Im w00 + i Im w11,  f1 = w01,  f2 = w02,  f3 = w12;
+//   then w10 = -conj(w01).
+template <typename T, int PACK>
+__device__ __forceinline__ void build_g(const cx<T> *__restrict__ w, int64_t V, int64_t s, T a, cx<T> (&g)[9])
+{
+    if (PACK == 9) {
+#pragma unroll
+        for (int k = 0; k < 6; k++) g[k] = cscale(__ldg(w + (int64_t)k * V + s), a);
+        g[0].x += (T)1; g[4].x += (T)1;
+    } else {
+        cx<T> f0 = __ldg(w + s), f1 = __ldg(w + V + s), f2 = __ldg(w + 2 * V + s), f3 = __ldg(w + 3 * V + s);
+        g[0] = mk<T>((T)1, a * f0.x);
+        g[1] = cscale(f1, a);
+        g[2] = cscale(f2, a);
+        g[3] = mk<T>(-a * f1.x, a * f1.y);
+        g[4] = mk<T>((T)1, a * f0.y);
+        g[5] = cscale(f3, a);
+    }
+    reunit<T>(g);
+}
+
+// rows [0, R) of c = a b
+template <int R, typename V> __device__ __forceinline__ void mul_rows(const V (&a)[9], const V (&b)[9], V (&c)[9])
+{
+#pragma unroll
+    for (int i = 0; i < R; i++)
+#pragma unroll
+        for (int j = 0; j < 3; j++) {
+            V s = cmul(a[3 * i], b[j]);
+            s = cfma(a[3 * i + 1], b[3 + j], s);
+            s = cfma(a[3 * i + 2], b[6 + j], s);
+            c[3 * i + j] = s;
+        }
+}
+
+// rows [0, R) of c = a b^dagger
+template <int R, typename V> __device__ __forceinline__ void mul_rows_dag(const V (&a)[9], const V (&b)[9], V (&c)[9])
+{
+#pragma unroll
+    for (int i = 0; i < R; i++)
+#pragma unroll
+        for (int j = 0; j < 3; j++) {
+            V s = cmulc(a[3 * i], b[3 * j]);
+            s = cfmac(a[3 * i + 1], b[3 * j + 1], s);
+            s = cfmac(a[3 * i + 2], b[3 * j + 2], s);
+            c[3 * i + j] = s;
+        }
+}
+
+} // namespace lgf

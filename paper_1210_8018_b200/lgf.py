@@ -1,0 +1,246 @@
+"""ctypes binding of liblgf.so (include/lgf.h).  Same names as the C ABI; argument marshalling
+only -- every step of the gauge-fixing iteration runs in the CUDA kernels behind the library.
+
+Low level: ``lib()`` returns the loaded CDLL with typed prototypes (``lgf_create`` ...).
+Convenience: ``GaugeFixer`` owns a torch device workspace + stream and forwards to the ABI.
+There is no CPU fallback: a missing or unloadable ``liblgf.so`` raises ``LgfError``.
+"""
+import ctypes
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "liblgf.so")
+
+OK = 0
+ERR_INVALID_ARG, ERR_UNSUPPORTED_SIZE, ERR_NOT_BOUND, ERR_NOT_LOADED = -1, -2, -3, -4
+ERR_WORKSPACE_TOO_SMALL, ERR_CUDA, ERR_NOT_CONVERGED, ERR_NUMERIC = -5, -6, -7, -8
+PREC_FP64, PREC_FP32 = 0, 1
+LAYOUT_AOS = 0
+OPT_RECON, OPT_FFT_BATCH, OPT_MAX_ITER, OPT_CHECK_INTERVAL, OPT_FFT_PATH, OPT_PROFILE = 1, 2, 3, 4, 5, 6
+FIELD_DELTA, FIELD_W, FIELD_G = 0, 1, 2
+STAGE_MEASURE, STAGE_FOURIER, STAGE_UPDATE = 0, 1, 2
+KERNEL_NAMES = ["measure", "fft_xy_fwd", "fft_zt", "fft_xy_inv", "update", "fft_generic", "layout"]
+
+#: every symbol include/lgf.h declares
+SYMBOLS = [
+    "lgf_create", "lgf_set_option", "lgf_workspace_bytes", "lgf_bind", "lgf_load_links", "lgf_get_links",
+    "lgf_measure", "lgf_iterate", "lgf_fix", "lgf_stage", "lgf_get_field", "lgf_set_field", "lgf_history",
+    "lgf_kernel_time", "lgf_launch_count", "lgf_reset_counters", "lgf_uses_tiled_fft", "lgf_last_error",
+    "lgf_destroy",
+]
+
+
+class LgfError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__(f"liblgf error {code}: {msg}")
+        self.code = code
+
+
+class lgf_result(ctypes.Structure):
+    _fields_ = [("iterations", ctypes.c_int64), ("F", ctypes.c_double), ("theta", ctypes.c_double),
+                ("converged", ctypes.c_int)]
+
+
+_lib = None
+
+
+def lib():
+    """Load liblgf.so (no GPU needed to load it) and type its prototypes."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise LgfError(ERR_CUDA, f"{LIB_PATH} is missing: build it with `python -m paper_1210_8018_b200.build` "
+                                 "(there is no CPU fallback)")
+    L = ctypes.CDLL(LIB_PATH)
+    vp, i, i64, d = ctypes.c_void_p, ctypes.c_int, ctypes.c_int64, ctypes.c_double
+    dp = ctypes.POINTER(ctypes.c_double)
+    rp = ctypes.POINTER(lgf_result)
+    L.lgf_create.argtypes = [i, i, i, i, i, ctypes.POINTER(vp)]
+    L.lgf_set_option.argtypes = [vp, i, i64]
+    L.lgf_workspace_bytes.argtypes = [vp]
+    L.lgf_workspace_bytes.restype = ctypes.c_size_t
+    L.lgf_bind.argtypes = [vp, vp, ctypes.c_size_t, vp]
+    L.lgf_load_links.argtypes = [vp, vp, i, i]
+    L.lgf_get_links.argtypes = [vp, vp, i, i]
+    L.lgf_measure.argtypes = [vp, dp, dp]
+    L.lgf_iterate.argtypes = [vp, d, i64, rp]
+    L.lgf_fix.argtypes = [vp, d, d, rp]
+    L.lgf_stage.argtypes = [vp, i, d]
+    L.lgf_get_field.argtypes = [vp, i, d, vp, i]
+    L.lgf_set_field.argtypes = [vp, i, vp, i]
+    L.lgf_history.argtypes = [vp, dp, dp, i, ctypes.POINTER(i)]
+    L.lgf_kernel_time.argtypes = [vp, i, dp, ctypes.POINTER(i64)]
+    L.lgf_launch_count.argtypes = [vp]
+    L.lgf_launch_count.restype = i64
+    L.lgf_reset_counters.argtypes = [vp]
+    L.lgf_uses_tiled_fft.argtypes = [vp]
+    L.lgf_last_error.argtypes = [vp]
+    L.lgf_last_error.restype = ctypes.c_char_p
+    L.lgf_destroy.argtypes = [vp]
+    _lib = L
+    return L
+
+
+def _dims(N):
+    N = (N,) * 4 if isinstance(N, int) else tuple(int(n) for n in N)
+    assert len(N) == 4
+    return N
+
+
+class GaugeFixer:
+    """One lattice on one GPU.  Thin wrapper: allocates the workspace with torch, binds it,
+    and forwards every call to the C ABI.  Host arrays are numpy, complex128 (FP64 contexts)
+    or complex64 (FP32 contexts), links [V,4,3,3], site fields [V,3,3]; device arrays are
+    torch complex tensors of the same shapes."""
+
+    def __init__(self, N, precision="fp64", recon=18, fft_batch=4, fft_path=0, device="cuda:0",
+                 stream=None, max_iter=None, check_interval=None, profile=False):
+        import torch
+
+        self.torch = torch
+        self.N = _dims(N)
+        self.V = self.N[0] * self.N[1] * self.N[2] * self.N[3]
+        self.prec = {"fp64": PREC_FP64, "fp32": PREC_FP32}[precision]
+        self.np_dtype = np.complex128 if self.prec == PREC_FP64 else np.complex64
+        self.torch_dtype = torch.complex128 if self.prec == PREC_FP64 else torch.complex64
+        self.L = lib()
+        self.ctx = ctypes.c_void_p()
+        rc = self.L.lgf_create(*self.N, self.prec, ctypes.byref(self.ctx))
+        if rc:
+            raise LgfError(rc, self.L.lgf_last_error(None).decode())
+        self.set_option(OPT_RECON, recon)
+        self.set_option(OPT_FFT_BATCH, fft_batch)
+        self.set_option(OPT_FFT_PATH, fft_path)
+        if max_iter is not None:
+            self.set_option(OPT_MAX_ITER, max_iter)
+        if check_interval is not None:
+            self.set_option(OPT_CHECK_INTERVAL, check_interval)
+        if profile:
+            self.set_option(OPT_PROFILE, 1)
+        if not torch.cuda.is_available():
+            raise LgfError(ERR_CUDA, "no CUDA device: liblgf has no CPU fallback")
+        self.device = torch.device(device)
+        torch.cuda.set_device(self.device)
+        self.stream = stream if stream is not None else torch.cuda.Stream(device=self.device)
+        nbytes = self.L.lgf_workspace_bytes(self.ctx)
+        self.workspace = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
+        ptr = (self.workspace.data_ptr() + 255) // 256 * 256
+        torch.cuda.synchronize(self.device)
+        self._ck(self.L.lgf_bind(self.ctx, ptr, nbytes, self.stream.cuda_stream))
+
+    # -- plumbing
+    def _ck(self, rc, allow=()):
+        if rc and rc not in allow:
+            raise LgfError(rc, self.L.lgf_last_error(self.ctx).decode())
+        return rc
+
+    def close(self):
+        if getattr(self, "ctx", None) is not None and self.ctx:
+            self.L.lgf_destroy(self.ctx)
+            self.ctx = ctypes.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def _src(self, a, per_site):
+        """(pointer, is_device, keepalive) for a numpy or torch array of V*per_site complex numbers."""
+        torch = self.torch
+        if isinstance(a, torch.Tensor):
+            assert a.dtype == self.torch_dtype and a.is_contiguous() and a.numel() == self.V * per_site
+            if a.is_cuda:
+                # order the library's stream after whatever produced/consumes this tensor
+                self.stream.wait_stream(torch.cuda.current_stream(self.device))
+                return a.data_ptr(), 1, a
+            return a.data_ptr(), 0, a
+        assert isinstance(a, np.ndarray) and a.dtype == self.np_dtype and a.flags.c_contiguous
+        assert a.size == self.V * per_site
+        return a.ctypes.data, 0, a
+
+    # -- the C ABI, same names
+    def set_option(self, key, value):
+        self._ck(self.L.lgf_set_option(self.ctx, key, int(value)))
+
+    def workspace_bytes(self):
+        return self.L.lgf_workspace_bytes(self.ctx)
+
+    def load_links(self, U):
+        p, dev, keep = self._src(U, 36)
+        self._ck(self.L.lgf_load_links(self.ctx, p, dev, LAYOUT_AOS))
+        if dev:
+            self.stream.synchronize()
+
+    def get_links(self, out=None, device=False):
+        if out is None:
+            out = (self.torch.empty((self.V, 4, 3, 3), dtype=self.torch_dtype, device=self.device) if device
+                   else np.empty((self.V, 4, 3, 3), dtype=self.np_dtype))
+        p, dev, keep = self._src(out, 36)
+        self._ck(self.L.lgf_get_links(self.ctx, p, dev, LAYOUT_AOS))
+        return out
+
+    def measure(self):
+        F, th = ctypes.c_double(), ctypes.c_double()
+        self._ck(self.L.lgf_measure(self.ctx, ctypes.byref(F), ctypes.byref(th)))
+        return F.value, th.value
+
+    def iterate(self, alpha, n, sync=True):
+        if not sync:
+            self._ck(self.L.lgf_iterate(self.ctx, float(alpha), int(n), None))
+            return None
+        r = lgf_result()
+        self._ck(self.L.lgf_iterate(self.ctx, float(alpha), int(n), ctypes.byref(r)))
+        return r
+
+    def fix(self, alpha=0.08, eps=1e-15, allow_not_converged=False):
+        r = lgf_result()
+        self._ck(self.L.lgf_fix(self.ctx, float(alpha), float(eps), ctypes.byref(r)),
+                 allow=(ERR_NOT_CONVERGED,) if allow_not_converged else ())
+        return r
+
+    def stage(self, stage, alpha=0.08):
+        self._ck(self.L.lgf_stage(self.ctx, stage, float(alpha)))
+
+    def get_field(self, which, alpha=0.08, device=False):
+        out = (self.torch.empty((self.V, 3, 3), dtype=self.torch_dtype, device=self.device) if device
+               else np.empty((self.V, 3, 3), dtype=self.np_dtype))
+        p, dev, keep = self._src(out, 9)
+        self._ck(self.L.lgf_get_field(self.ctx, which, float(alpha), p, dev))
+        return out
+
+    def set_field(self, which, a):
+        p, dev, keep = self._src(a, 9)
+        self._ck(self.L.lgf_set_field(self.ctx, which, p, dev))
+
+    def history(self, cap=4096):
+        F = np.empty(cap, dtype=np.float64)
+        th = np.empty(cap, dtype=np.float64)
+        n = ctypes.c_int()
+        dp = ctypes.POINTER(ctypes.c_double)
+        self._ck(self.L.lgf_history(self.ctx, F.ctypes.data_as(dp), th.ctypes.data_as(dp), cap, ctypes.byref(n)))
+        return np.stack([F[: n.value], th[: n.value]], axis=1)
+
+    def kernel_times(self):
+        """{kind: (total ms, launches)} since the last reset (needs profile=True for the ms)."""
+        out = {}
+        for k, name in enumerate(KERNEL_NAMES):
+            ms, cnt = ctypes.c_double(), ctypes.c_int64()
+            self._ck(self.L.lgf_kernel_time(self.ctx, k, ctypes.byref(ms), ctypes.byref(cnt)))
+            out[name] = (ms.value, cnt.value)
+        return out
+
+    def launch_count(self):
+        return self.L.lgf_launch_count(self.ctx)
+
+    def reset_counters(self):
+        self._ck(self.L.lgf_reset_counters(self.ctx))
+
+    def uses_tiled_fft(self):
+        return bool(self.L.lgf_uses_tiled_fft(self.ctx))
+
+    def synchronize(self):
+        self.stream.synchronize()

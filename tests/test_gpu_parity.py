@@ -1,0 +1,251 @@
+"""GPU parity: the CUDA path (through the C ABI, liblgf.so) against the CPU oracle, element by
+element, on the same seeded inputs.  Tolerances are BASELINE.json's north_star:
+  after one iteration: links <= 1e-12 max abs, F and theta <= 1e-10 relative;
+  after convergence:   iteration count within +-2 %, final F within 1e-10;
+  FP32: links <= 1e-5 max abs after one iteration, converges to theta <= 1e-12.
+Per-kernel taps use tighter, arithmetic-derived bounds."""
+import os
+
+import numpy as np
+import pytest
+
+import gen
+import oracle
+from test_golden import golden_path, read_golden
+
+pytestmark = pytest.mark.gpu
+
+ALPHA = 0.08
+
+
+@pytest.fixture(scope="module")
+def lgf(cuda_device):
+    from paper_1210_8018_b200 import lgf as m
+
+    m.lib()
+    return m
+
+
+def fixer(lgf, N, **kw):
+    return lgf.GaugeFixer(N, **kw)
+
+
+LATTICES = [
+    # (extents, sigma, seed)            8^4 = BASELINE config 1; mixed extents span ragged tiles
+    ((8, 8, 8, 8), 0.3, gen.BASE_SEED + 8),
+    ((4, 6, 8, 12), 0.5, 77),
+    ((16, 8, 4, 6), 0.5, 78),
+    ((16, 16, 16, 16), 0.5, gen.BASE_SEED + 16),
+]
+VARIANTS = [dict(recon=18, fft_batch=4), dict(recon=12, fft_batch=4), dict(recon=18, fft_batch=9),
+            dict(recon=12, fft_batch=9), dict(recon=18, fft_batch=4, fft_path=1)]
+
+
+def ids(v):
+    return "-".join(f"{k}{x}" for k, x in v.items()) if isinstance(v, dict) else "x".join(map(str, v[0]))
+
+
+@pytest.mark.parametrize("recon", [18, 12])
+def test_links_round_trip(lgf, recon):
+    N = (4, 6, 8, 12)
+    U = gen.gen_links(N, 0.5, 5)
+    gf = fixer(lgf, N, recon=recon)
+    gf.load_links(U)
+    back = gf.get_links()
+    if recon == 18:
+        assert np.array_equal(back, U)
+    else:
+        assert np.array_equal(back[:, :, :2], U[:, :, :2])
+        assert np.abs(back - U).max() < 1e-14            # row 2 rebuilt from unitarity
+    # device-resident source and destination
+    import torch
+    Ud = torch.from_numpy(U).cuda()
+    gf.load_links(Ud)
+    assert np.abs(gf.get_links(device=True).cpu().numpy() - U).max() < 1e-14
+
+
+@pytest.mark.parametrize("lat", LATTICES, ids=ids)
+@pytest.mark.parametrize("var", VARIANTS, ids=ids)
+def test_measure_matches_oracle(lgf, lat, var):
+    N, sigma, seed = lat
+    U = gen.gen_links(N, sigma, seed)
+    D, F, th = oracle.measure(N, U)
+    gf = fixer(lgf, N, **var)
+    gf.load_links(U)
+    F2, th2 = gf.measure()
+    D2 = gf.get_field(lgf.FIELD_DELTA)
+    assert np.abs(D2 - D).max() < 1e-13
+    assert abs(F2 - F) <= 1e-12 * max(abs(F), 1e-3) + 1e-15
+    assert abs(th2 - th) <= 1e-12 * th
+
+
+@pytest.mark.parametrize("lat", LATTICES, ids=ids)
+@pytest.mark.parametrize("var", VARIANTS, ids=ids)
+def test_fourier_matches_oracle(lgf, lat, var):
+    N, sigma, seed = lat
+    U = gen.gen_links(N, sigma, seed)
+    D, _, _ = oracle.measure(N, U)
+    w = oracle.fourier_accelerate(N, D)
+    gf = fixer(lgf, N, **var)
+    gf.load_links(U)
+    gf.set_field(lgf.FIELD_DELTA, D)
+    gf.stage(lgf.STAGE_FOURIER)
+    w2 = gf.get_field(lgf.FIELD_W)
+    scale = np.abs(w).max()
+    # row 2 of w is not needed by g (pin P15); the packed mode rebuilds it from anti-Hermiticity
+    assert np.abs(w2 - w).max() < 2e-13 * scale
+
+
+@pytest.mark.parametrize("var", VARIANTS[:4], ids=ids)
+def test_g_and_update_match_oracle(lgf, var):
+    N, sigma, seed = (4, 6, 8, 12), 0.5, 91
+    U = gen.gen_links(N, sigma, seed)
+    D, _, _ = oracle.measure(N, U)
+    w = oracle.fourier_accelerate(N, D)
+    g = oracle.build_g(w, ALPHA)
+    gf = fixer(lgf, N, **var)
+    gf.load_links(U)
+    gf.set_field(lgf.FIELD_W, w)
+    g2 = gf.get_field(lgf.FIELD_G, alpha=ALPHA)
+    assert np.abs(g2 - g).max() < 1e-14
+    gf.stage(lgf.STAGE_UPDATE, alpha=ALPHA)
+    U1 = oracle.update_links(N, U.copy(), g)
+    assert np.abs(gf.get_links() - U1).max() < 1e-13
+
+
+@pytest.mark.parametrize("lat", LATTICES, ids=ids)
+@pytest.mark.parametrize("var", VARIANTS, ids=ids)
+def test_one_iteration_matches_oracle(lgf, lat, var):
+    N, sigma, seed = lat
+    U = gen.gen_links(N, sigma, seed)
+    Uo = U.copy()
+    hist = oracle.iterate(N, Uo, ALPHA, 1)
+    gf = fixer(lgf, N, **var)
+    gf.load_links(U)
+    r = gf.iterate(ALPHA, 1)
+    assert r.iterations == 1
+    assert np.abs(gf.get_links() - Uo).max() < 1e-12
+    assert abs(r.F - hist[1, 0]) <= 1e-10 * abs(hist[1, 0])
+    assert abs(r.theta - hist[1, 1]) <= 1e-10 * hist[1, 1]
+    h = gf.history()
+    assert h.shape == (2, 2)
+    assert np.allclose(h, hist, rtol=1e-10, atol=0)
+
+
+@pytest.mark.parametrize("n,sigma,seed", [(8, 0.3, gen.BASE_SEED + 8), (8, 0.3, gen.BASE_SEED + 1008),
+                                          (8, 0.3, gen.BASE_SEED + 2008), (16, 0.5, gen.BASE_SEED + 16),
+                                          (16, 0.5, gen.BASE_SEED + 1016)])
+@pytest.mark.parametrize("var", [VARIANTS[0], VARIANTS[1], VARIANTS[2]], ids=ids)
+def test_convergence_matches_oracle_golden(lgf, n, sigma, seed, var):
+    it, F, th, hist = read_golden(golden_path(n, seed))
+    U = gen.gen_links(n, sigma, seed)
+    gf = fixer(lgf, n, **var)
+    gf.load_links(U)
+    r = gf.fix(ALPHA, 1e-15)
+    assert r.converged == 1 and r.theta <= 1e-15
+    assert abs(r.iterations - it) <= 0.02 * it
+    assert abs(r.F - F) <= 1e-10
+    h = gf.history()
+    assert h.shape[0] == r.iterations + 1
+    k = min(h.shape[0], hist.shape[0]) - 3                  # the tail sits at the rounding floor
+    assert np.allclose(h[:k, 0], hist[:k, 0], rtol=0, atol=1e-10)
+    assert np.allclose(h[:k, 1], hist[:k, 1], rtol=1e-6, atol=1e-25)
+    assert np.all(np.diff(h[:, 0]) >= -1e-15)              # F never decreases (pin P12)
+    # the fixed links are unitary with det 1 and the plaquette is that of the input (pin P11)
+    Ufix = gf.get_links()
+    I = np.eye(3)
+    assert np.abs(Ufix @ np.conj(np.swapaxes(Ufix, -1, -2)) - I).max() < 1e-12
+    assert np.abs(np.linalg.det(Ufix) - 1).max() < 1e-12
+    if n == 8:
+        assert abs(oracle.plaquette(n, Ufix) - oracle.plaquette(n, U)) < 1e-12
+    # calling fix again on converged links does nothing
+    r2 = gf.fix(ALPHA, 1e-15)
+    assert r2.iterations == 0 and r2.converged == 1 and r2.F == r.F
+
+
+def test_iterate_equals_fix_prefix_and_is_deterministic(lgf):
+    n, seed = 8, gen.BASE_SEED + 8
+    U = gen.gen_links(n, 0.3, seed)
+    a = fixer(lgf, n)
+    a.load_links(U)
+    ra = a.iterate(ALPHA, 12)
+    b = fixer(lgf, n, check_interval=1)
+    b.load_links(U)
+    rb = b.iterate(ALPHA, 5)
+    rb = b.iterate(ALPHA, 7)
+    assert ra.iterations == 12 and rb.iterations == 7
+    assert ra.F == rb.F and ra.theta == rb.theta            # bitwise: fixed-order reductions
+    assert np.array_equal(a.get_links(), b.get_links())
+    assert a.launch_count() > 12 * 3
+
+
+def test_edge_cases(lgf):
+    from helpers import unit_links
+    n = (4, 4, 4, 4)
+    gf = fixer(lgf, n, max_iter=3)
+    # unit field: Delta = theta = 0, F = 1 exactly (pin P1): zero iterations
+    gf.load_links(unit_links(n))
+    r = gf.fix(ALPHA, 1e-15)
+    assert (r.iterations, r.F, r.theta, r.converged) == (0, 1.0, 0.0, 1)
+    # iteration cap: LGF_ERR_NOT_CONVERGED with the result still filled
+    U = gen.gen_links(n, 0.5, 3)
+    gf.load_links(U)
+    with pytest.raises(lgf.LgfError) as e:
+        gf.fix(ALPHA, 1e-15)
+    assert e.value.code == lgf.ERR_NOT_CONVERGED
+    r = gf.fix(ALPHA, 1e-15, allow_not_converged=True)
+    assert r.iterations == 3 and r.converged == 0 and r.theta > 1e-15
+    # stage order is checked
+    with pytest.raises(lgf.LgfError):
+        gf.stage(lgf.STAGE_UPDATE)
+    # a NaN link is reported, not iterated on
+    U[5, 2, 1, 1] = np.nan
+    gf.load_links(U)
+    with pytest.raises(lgf.LgfError) as e:
+        gf.fix(ALPHA, 1e-15)
+    assert e.value.code == lgf.ERR_NUMERIC
+    # pure gauge field: F -> 1 (pin P13)
+    gf2 = fixer(lgf, n)
+    gf2.load_links(gen.gen_links(n, 0.0, 11))
+    r = gf2.fix(ALPHA, 1e-15)
+    assert r.converged and abs(r.F - 1) < 1e-12
+
+
+@pytest.mark.parametrize("lat", [LATTICES[0], LATTICES[1], LATTICES[3]], ids=ids)
+@pytest.mark.parametrize("var", [VARIANTS[0], VARIANTS[1]], ids=ids)
+def test_fp32_variant(lgf, lat, var):
+    N, sigma, seed = lat
+    U = gen.gen_links(N, sigma, seed)
+    Uo = U.copy()
+    hist = oracle.iterate(N, Uo, ALPHA, 1)
+    gf = fixer(lgf, N, precision="fp32", **var)
+    gf.load_links(U.astype(np.complex64))
+    r = gf.iterate(ALPHA, 1)
+    assert np.abs(gf.get_links().astype(np.complex128) - Uo).max() < 1e-5
+    assert abs(r.F - hist[1, 0]) < 1e-5 and abs(r.theta - hist[1, 1]) < 1e-4 * hist[1, 1]
+    gf.load_links(U.astype(np.complex64))
+    r = gf.fix(ALPHA, 1e-12)
+    assert r.converged == 1 and r.theta <= 1e-12
+    it_ref = oracle.fix(N, U.copy(), ALPHA, 1e-12)[0]
+    assert abs(r.iterations - it_ref) <= max(1, 0.02 * it_ref)
+
+
+def test_headline_32_12real_one_iteration_and_golden(lgf):
+    """BASELINE config 3 in the configuration bench.py times: 32^4, FP64, 12-real links."""
+    n, seed = 32, gen.BASE_SEED + 32
+    U = gen.gen_links(n, 0.5, seed)
+    gf = fixer(lgf, n, recon=12)
+    gf.load_links(U)
+    r1 = gf.iterate(ALPHA, 1)
+    U1 = gf.get_links()
+    Uo = U.copy()
+    hist = oracle.iterate(n, Uo, ALPHA, 1)
+    assert np.abs(U1 - Uo).max() < 1e-12
+    assert abs(r1.F - hist[1, 0]) <= 1e-10 * abs(hist[1, 0])
+    assert abs(r1.theta - hist[1, 1]) <= 1e-10 * hist[1, 1]
+    path = golden_path(n, seed)
+    if os.path.exists(path):
+        it, F, th, ghist = read_golden(path)
+        gf.load_links(U)
+        r = gf.fix(ALPHA, 1e-15)
+        assert r.converged == 1 and abs(r.iterations - it) <= 0.02 * it and abs(r.F - F) <= 1e-10
