@@ -36,6 +36,7 @@ LATTICES = [
     ((4, 6, 8, 12), 0.5, 77),
     ((16, 8, 4, 6), 0.5, 78),
     ((16, 16, 16, 16), 0.5, gen.BASE_SEED + 16),
+    ((12, 12, 12, 12), 0.5, 79),        # radix-3 lines of the tiled FFT
 ]
 VARIANTS = [dict(recon=18, fft_batch=4), dict(recon=12, fft_batch=4), dict(recon=18, fft_batch=9),
             dict(recon=12, fft_batch=9), dict(recon=18, fft_batch=4, fft_path=1)]
@@ -228,6 +229,26 @@ def test_fp32_variant(lgf, lat, var):
     assert r.converged == 1 and r.theta <= 1e-12
     it_ref = oracle.fix(N, U.copy(), ALPHA, 1e-12)[0]
     assert abs(r.iterations - it_ref) <= max(1, 0.02 * it_ref)
+
+
+def test_tiled_fft_is_taken_where_expected(lgf):
+    for n, want in [(8, True), (12, True), (16, True), (24, True), (32, True), ((8, 8, 8, 16), False), (4, False), (48, False)]:
+        gf = fixer(lgf, n)
+        assert gf.uses_tiled_fft() == want, n
+    assert not fixer(lgf, 16, fft_path=1).uses_tiled_fft()
+
+
+def test_24_one_iteration(lgf):
+    n = 24
+    U = gen.gen_links(n, 0.5, 80)
+    Uo = U.copy()
+    hist = oracle.iterate(n, Uo, ALPHA, 1)
+    for prec, tol in (("fp64", 1e-12), ("fp32", 1e-5)):
+        gf = fixer(lgf, n, precision=prec, recon=12)
+        gf.load_links(U if prec == "fp64" else U.astype(np.complex64))
+        r = gf.iterate(ALPHA, 1)
+        assert np.abs(gf.get_links().astype(np.complex128) - Uo).max() < tol
+        assert abs(r.theta - hist[1, 1]) <= (1e-10 if prec == "fp64" else 1e-4) * hist[1, 1]
 
 
 def test_headline_32_12real_one_iteration_and_golden(lgf):
