@@ -68,8 +68,14 @@ enum {
                                    kernels launched after convergence exit at once. */
     LGF_OPT_FFT_PATH = 5,       /* 0 (default): tiled register FFT when the extents allow it,
                                    1: always the generic per-axis transform */
-    LGF_OPT_PROFILE = 6         /* 1: bracket every kernel launch with CUDA events on the bound
+    LGF_OPT_PROFILE = 6,        /* 1: bracket every kernel launch with CUDA events on the bound
                                    stream so that lgf_kernel_time works; default 0 */
+    LGF_OPT_FUSION = 7          /* 1 (default): lgf_iterate / lgf_fix run the link update and the
+                                   measure of the next iteration as ONE kernel over double-buffered
+                                   links (each link read once, written once per iteration), with g
+                                   built in the last FFT pass where the tile fits;
+                                   0: the three separate kernels of lgf_stage (measure, Fourier,
+                                   update in place), as in the paper's kernel list */
 };
 
 /* lgf_get_field / lgf_set_field selectors */
@@ -95,7 +101,9 @@ enum {
     LGF_KERNEL_UPDATE = 4,
     LGF_KERNEL_FFT_GENERIC = 5,
     LGF_KERNEL_LAYOUT = 6,
-    LGF_KERNEL_KINDS = 7
+    LGF_KERNEL_FFT_XY_INV_G = 7,   /* last FFT pass with the g build as its epilogue */
+    LGF_KERNEL_UPDATE_MEASURE = 8, /* fused link update + measure */
+    LGF_KERNEL_KINDS = 9
 };
 
 /* Create a context for an Nx*Ny*Nz*Nt lattice.  host call; allocates host memory only.

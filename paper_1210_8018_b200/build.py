@@ -15,7 +15,7 @@ CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "liblgf.so")
 INCLUDE = os.path.join(os.path.dirname(HERE), "include")
-SOURCES = ["lgf_api.cu", "kernels_site.cu", "fft_generic.cu", "fft_tiled.cu"]
+SOURCES = ["lgf_api.cu", "kernels_site.cu", "kernels_fused.cu", "fft_generic.cu", "fft_tiled.cu"]
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
     "-Xcompiler", "-fPIC", "-Wno-deprecated-gpu-targets", "-I", INCLUDE,

@@ -19,16 +19,63 @@ __device__ __forceinline__ double2 operator+(double2 a, double2 b) { return make
 __device__ __forceinline__ double2 operator-(double2 a, double2 b) { return make_double2(a.x - b.x, a.y - b.y); }
 __device__ __forceinline__ float2 operator+(float2 a, float2 b) { return make_float2(a.x + b.x, a.y + b.y); }
 __device__ __forceinline__ float2 operator-(float2 a, float2 b) { return make_float2(a.x - b.x, a.y - b.y); }
+// Complex products written as explicit fused multiply-adds: `acc.x += a.x*b.x - a.y*b.y` as plain
+// C++ costs DMUL + DFMA + DADD per component (the compiler may not reassociate), the forms
+// below cost two FMAs.  The FP64 pipe is the second roofline of this path.
+__device__ __forceinline__ double fma_t(double a, double b, double c) { return ::fma(a, b, c); }
+__device__ __forceinline__ float fma_t(float a, float b, float c) { return ::fmaf(a, b, c); }
 // a*b
-template <typename V> __device__ __forceinline__ V cmul(V a, V b) { V r; r.x = a.x * b.x - a.y * b.y; r.y = a.x * b.y + a.y * b.x; return r; }
+template <typename V> __device__ __forceinline__ V cmul(V a, V b)
+{
+    V r;
+    r.x = fma_t(-a.y, b.y, a.x * b.x);
+    r.y = fma_t(a.y, b.x, a.x * b.y);
+    return r;
+}
 // a*conj(b)
-template <typename V> __device__ __forceinline__ V cmulc(V a, V b) { V r; r.x = a.x * b.x + a.y * b.y; r.y = a.y * b.x - a.x * b.y; return r; }
+template <typename V> __device__ __forceinline__ V cmulc(V a, V b)
+{
+    V r;
+    r.x = fma_t(a.y, b.y, a.x * b.x);
+    r.y = fma_t(-a.x, b.y, a.y * b.x);
+    return r;
+}
 // conj(a)*b
-template <typename V> __device__ __forceinline__ V cconjmul(V a, V b) { V r; r.x = a.x * b.x + a.y * b.y; r.y = a.x * b.y - a.y * b.x; return r; }
+template <typename V> __device__ __forceinline__ V cconjmul(V a, V b)
+{
+    V r;
+    r.x = fma_t(a.y, b.y, a.x * b.x);
+    r.y = fma_t(-a.y, b.x, a.x * b.y);
+    return r;
+}
 // acc + a*b
-template <typename V> __device__ __forceinline__ V cfma(V a, V b, V acc) { acc.x += a.x * b.x - a.y * b.y; acc.y += a.x * b.y + a.y * b.x; return acc; }
+template <typename V> __device__ __forceinline__ V cfma(V a, V b, V acc)
+{
+    acc.x = fma_t(-a.y, b.y, fma_t(a.x, b.x, acc.x));
+    acc.y = fma_t(a.y, b.x, fma_t(a.x, b.y, acc.y));
+    return acc;
+}
+// acc - a*b
+template <typename V> __device__ __forceinline__ V cfms(V a, V b, V acc)
+{
+    acc.x = fma_t(a.y, b.y, fma_t(-a.x, b.x, acc.x));
+    acc.y = fma_t(-a.y, b.x, fma_t(-a.x, b.y, acc.y));
+    return acc;
+}
 // acc + a*conj(b)
-template <typename V> __device__ __forceinline__ V cfmac(V a, V b, V acc) { acc.x += a.x * b.x + a.y * b.y; acc.y += a.y * b.x - a.x * b.y; return acc; }
+template <typename V> __device__ __forceinline__ V cfmac(V a, V b, V acc)
+{
+    acc.x = fma_t(a.y, b.y, fma_t(a.x, b.x, acc.x));
+    acc.y = fma_t(-a.x, b.y, fma_t(a.y, b.x, acc.y));
+    return acc;
+}
+// acc + conj(a)*b
+template <typename V> __device__ __forceinline__ V cfmaconj(V a, V b, V acc)
+{
+    acc.x = fma_t(a.y, b.y, fma_t(a.x, b.x, acc.x));
+    acc.y = fma_t(-a.y, b.x, fma_t(a.x, b.y, acc.y));
+    return acc;
+}
 template <typename V> __device__ __forceinline__ V cconj(V a) { a.y = -a.y; return a; }
 template <typename V> __device__ __forceinline__ auto cnorm2(V a) -> decltype(a.x) { return a.x * a.x + a.y * a.y; }
 template <typename V, typename T> __device__ __forceinline__ V cscale(V a, T s) { a.x *= s; a.y *= s; return a; }
@@ -42,10 +89,11 @@ struct Geom {
 
 __device__ __forceinline__ void site_coords(const Geom &g, int64_t s, int c[4])
 {
-    c[0] = (int)(s % g.N[0]); s /= g.N[0];
-    c[1] = (int)(s % g.N[1]); s /= g.N[1];
-    c[2] = (int)(s % g.N[2]); s /= g.N[2];
-    c[3] = (int)s;
+    unsigned u = (unsigned)s;               // V <= 64^4 < 2^32: 32-bit divisions
+    c[0] = (int)(u % (unsigned)g.N[0]); u /= (unsigned)g.N[0];
+    c[1] = (int)(u % (unsigned)g.N[1]); u /= (unsigned)g.N[1];
+    c[2] = (int)(u % (unsigned)g.N[2]); u /= (unsigned)g.N[2];
+    c[3] = (int)u;
 }
 
 // ---------------------------------------------------------------- device control block

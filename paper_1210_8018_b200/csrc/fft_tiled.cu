@@ -18,6 +18,7 @@
 // loaded straight from global memory into registers and the last one stored straight back.
 #include "launch.h"
 #include "twiddles.cuh"
+#include "su3.cuh"
 
 namespace lgf {
 
@@ -210,6 +211,66 @@ k_fft_xy(cx<T> *__restrict__ w, int64_t nplanes, const Ctrl *ctrl)
     }
 }
 
+// ---------------------------------------------------------------- pass 2 with the g build fused
+// (x,y) inverse of all four packed fields of one (z,t) plane in one CTA, then
+// g(x) = reunit(1 + (alpha/2) w(x)) (Alg. 1 lines 9-11) straight from shared
+// memory: w never goes back to HBM, rows 0, 1 of g (12 reals) do.  The fused link kernel
+// (kernels_fused.cu) then reads g at x and its 8 neighbours instead of rebuilding it 9 times.
+template <typename T, int NA, int NB>
+__global__ void __launch_bounds__(CTA_THREADS)
+k_fft_xy_inv_g(const cx<T> *__restrict__ w, cx<T> *__restrict__ gbuf, int64_t V, int64_t nplanes, T a, const Ctrl *ctrl)
+{
+    if (*(volatile const int *)&ctrl->done) return;
+    typedef Tile<NA, NB, 1> TL;
+    constexpr int TP = TL::THREADS;               // threads of one field of one plane
+    constexpr int TG = 4 * TP;                    // threads of one plane
+    constexpr int G = CTA_THREADS / TG;           // planes per CTA
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int grp = threadIdx.x / TG, t = threadIdx.x % TG;
+    const int fld = t / TP, l = t % TP;
+    cx<T> *smp = (cx<T> *)smem_raw + (size_t)grp * 4 * TL::ELEMS;   // the 4 fields of this plane
+    cx<T> *sm = smp + (size_t)fld * TL::ELEMS;
+    const int64_t plane = (int64_t)blockIdx.x * G + grp;
+    const bool ok = plane < nplanes && grp < G;
+    const int64_t base = plane * (int64_t)(NA * NB);
+
+    if (ok && l < NA) {
+        const cx<T> *f = w + (int64_t)fld * V + base;
+#pragma unroll
+        for (int j = 0; j < NB; j++) sm[j * TL::RS + l] = f[j * NA + l];
+    }
+    __syncthreads();
+    if (ok && l < NB) {
+        cx<T> v[NA];
+#pragma unroll
+        for (int j = 0; j < NA; j++) v[j] = sm[l * TL::RS + j];
+        Dif<T, NA, NA, +1>::run(v);
+#pragma unroll
+        for (int s = 0; s < NA; s++) sm[l * TL::RS + slot_freq<NA>(s)] = v[s];
+    }
+    __syncthreads();
+    if (ok && l < NA) {
+        cx<T> v[NB];
+#pragma unroll
+        for (int j = 0; j < NB; j++) v[j] = sm[j * TL::RS + l];
+        Dif<T, NB, NB, +1>::run(v);
+#pragma unroll
+        for (int s = 0; s < NB; s++) sm[slot_freq<NB>(s) * TL::RS + l] = v[s];
+    }
+    __syncthreads();
+    if (ok) {
+        for (int i = t; i < NA * NB; i += TG) {
+            const int o = (i / NA) * TL::RS + (i % NA);
+            cx<T> g[9];
+            m_from_packed<T>(smp[o], smp[TL::ELEMS + o], smp[2 * TL::ELEMS + o], smp[3 * TL::ELEMS + o], a, g);
+            reunit01<T>(g);
+            cx<T> *dst = gbuf + base + i;
+#pragma unroll
+            for (int k = 0; k < 6; k++) dst[(int64_t)k * V] = g[k];
+        }
+    }
+}
+
 // ---------------------------------------------------------------- pass 1: (z,t) tiles
 // Tile = C consecutive x at fixed (field, y): element (c, z, t) at global x0 + c + sz*z + st*t.
 // z-lines straight from global (thread = (c, t)), Dif(-) along z -> shared; t-lines from
@@ -287,6 +348,11 @@ template <typename T, int NA, int NB> struct XYCfg {
     static constexpr int G = CTA_THREADS / TL::THREADS;
     static constexpr size_t SMEM = (size_t)G * TL::ELEMS * sizeof(cx<T>);
 };
+template <typename T, int NA, int NB> struct XYGCfg {
+    typedef Tile<NA, NB, 1> TL;
+    static constexpr int G = CTA_THREADS / (4 * TL::THREADS);
+    static constexpr size_t SMEM = (size_t)G * 4 * TL::ELEMS * sizeof(cx<T>);
+};
 template <typename T, int NA, int NB, int C> struct ZTCfg {
     typedef Tile<NA, NB, C> TL;
     static constexpr int G = CTA_THREADS / TL::THREADS;
@@ -301,6 +367,8 @@ template <typename T, int N> static int setup_n()
     e = cudaFuncSetAttribute(k_fft_xy<T, N, N, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)XYCfg<T, N, N>::SMEM);
     if (e != cudaSuccess) return 1;
     e = cudaFuncSetAttribute(k_fft_xy<T, N, N, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)XYCfg<T, N, N>::SMEM);
+    if (e != cudaSuccess) return 1;
+    e = cudaFuncSetAttribute(k_fft_xy_inv_g<T, N, N>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)XYGCfg<T, N, N>::SMEM);
     if (e != cudaSuccess) return 1;
     e = cudaFuncSetAttribute(k_fft_zt<T, N, N, ZT_C>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ZTCfg<T, N, N, ZT_C>::SMEM);
     if (e != cudaSuccess) return 1;
@@ -321,6 +389,14 @@ template <typename T, int N> static void launch_n(const FftArgs &a, int which, c
         if (which == 0) k_fft_xy<T, N, N, 0><<<grid, CTA_THREADS, X::SMEM, st>>>((cx<T> *)a.w, nplanes, a.ctrl);
         else k_fft_xy<T, N, N, 1><<<grid, CTA_THREADS, X::SMEM, st>>>((cx<T> *)a.w, nplanes, a.ctrl);
     }
+}
+
+template <typename T, int N> static void launch_inv_g_n(const FftArgs &a, void *gbuf, double alpha, cudaStream_t st)
+{
+    typedef XYGCfg<T, N, N> X;
+    const int64_t nplanes = (int64_t)a.geo.N[2] * a.geo.N[3];
+    const unsigned grid = (unsigned)((nplanes + X::G - 1) / X::G);
+    k_fft_xy_inv_g<T, N, N><<<grid, CTA_THREADS, X::SMEM, st>>>((const cx<T> *)a.w, (cx<T> *)gbuf, a.geo.V, nplanes, (T)(alpha / 2.0), a.ctrl);
 }
 
 // Hypercubic N^4 lattices whose lines fit in registers: N = 8, 16, 32 in both precisions,
@@ -353,6 +429,13 @@ void launch_fft_tiled(const FftArgs &a, int which, cudaStream_t st)
 {
     const int n = a.geo.N[0], prec = a.prec;
     LGF_FFT_SWITCH(launch_n, a, which, st)
+}
+
+// pass 2 fused with the g build: needs the 4 packed fields (nfields == 4)
+void launch_fft_tiled_inv_g(const FftArgs &a, void *gbuf, double alpha, cudaStream_t st)
+{
+    const int n = a.geo.N[0], prec = a.prec;
+    LGF_FFT_SWITCH(launch_inv_g_n, a, gbuf, alpha, st)
 }
 
 } // namespace lgf

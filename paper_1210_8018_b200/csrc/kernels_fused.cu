@@ -1,0 +1,142 @@
+// kernels_fused.cu -- kernel (c) and kernel (a) of the NEXT iteration in one pass over the links
+// (arXiv 1210.8018, Alg. 1 lines 12-17):
+//     U'_mu(x) = g(x) U_mu(x) g^dagger(x+mu)                       (stored, each link read once, written once)
+//     Delta'(x) from  A'(x) = sum_nu [U'_nu(x-nu) - U'_nu(x)]      (eq. 1.5)
+//     F', theta'                                                   (eq. 1.1, 1.4)
+// The paper runs these as two kernels (k6, then k2 of the next iteration: Table 1,
+// PAPER.md:146-150), so every link crosses the memory bus three times per iteration; here it
+// crosses twice.  The thread of site x also needs the four NEW backward links
+// U'_nu(x-nu) = g(x-nu) U_nu(x-nu) g^dagger(x); it recomputes them from the OLD links (served
+// by L2, they were or will be streamed by the thread of x-nu) instead of waiting for a grid-wide
+// barrier.  That is why the links are double-buffered: `lin` is read-only, `lout` write-only.
+// g comes from the g buffer written by the last FFT pass (GBUF) or is rebuilt from w.
+#include "launch.h"
+#include "su3.cuh"
+#include "reduce.cuh"
+
+namespace lgf {
+
+static const int FUSED_THREADS = 128;
+#ifndef LGF_FUSED_MINB
+#define LGF_FUSED_MINB 4
+#endif
+
+// links are streamed: read (twice, the second time from L2) and written once per iteration
+template <typename V> __device__ __forceinline__ V ld_link(const V *p) { return __ldg(p); }
+template <typename V> __device__ __forceinline__ void st_link(V *p, V v) { *p = v; }
+
+template <typename T, int NE>
+__device__ __forceinline__ void load_link_in(const cx<T> *__restrict__ links, int64_t V, int mu, int64_t s, cx<T> (&u)[9])
+{
+    const cx<T> *p = links + (int64_t)mu * NE * V + s;
+#pragma unroll
+    for (int k = 0; k < NE; k++) u[k] = ld_link(p + (int64_t)k * V);
+    if (NE == 6) su3_row2(u);
+}
+
+// anti-Hermitian part of a link, accumulated with sign sg:  di += sg Im M_ii,
+// Eij += sg (M_ij - conj(M_ji)).  (D = A - A^dagger is linear in A; reading R3.)
+template <typename T>
+__device__ __forceinline__ void acc_ah(const cx<T> (&m)[9], T sg, T (&di)[3], cx<T> (&E)[3])
+{
+    di[0] += sg * m[0].y; di[1] += sg * m[4].y; di[2] += sg * m[8].y;
+    E[0].x += sg * (m[1].x - m[3].x); E[0].y += sg * (m[1].y + m[3].y);
+    E[1].x += sg * (m[2].x - m[6].x); E[1].y += sg * (m[2].y + m[6].y);
+    E[2].x += sg * (m[5].x - m[7].x); E[2].y += sg * (m[5].y + m[7].y);
+}
+
+template <typename T, int NE, int PACK, bool GBUF>
+__global__ void __launch_bounds__(FUSED_THREADS, LGF_FUSED_MINB)
+k_update_measure(const cx<T> *__restrict__ lin, cx<T> *__restrict__ lout, const cx<T> *__restrict__ gsrc,
+                 cx<T> *__restrict__ wout, Geom geo, T a, Ctrl *ctrl, double *partials, double2 *hist, double eps)
+{
+    if (*(volatile int *)&ctrl->done) return;
+    const int64_t V = geo.V;
+    const int64_t s = (int64_t)blockIdx.x * FUSED_THREADS + threadIdx.x;
+    constexpr int R = (NE == 6) ? 2 : 3;
+    double trF = 0, th = 0;
+    if (s < V) {
+        int c[4];
+        site_coords(geo, s, c);
+        cx<T> g0[9];
+        load_g01<T, PACK, GBUF>(gsrc, V, s, a, g0);
+        su3_row2(g0);
+        T di[3] = {0, 0, 0};
+        cx<T> E[3] = {mk<T>(0, 0), mk<T>(0, 0), mk<T>(0, 0)};
+        T tr = 0;
+#pragma unroll
+        for (int mu = 0; mu < 4; mu++) {
+            const int64_t sp = s + (c[mu] == geo.N[mu] - 1 ? -(int64_t)(geo.N[mu] - 1) : (int64_t)1) * geo.st[mu];
+            const int64_t sb = s + (c[mu] == 0 ? (int64_t)(geo.N[mu] - 1) : (int64_t)-1) * geo.st[mu];
+            {   // U'_mu(x) = g(x) U_mu(x) g^dagger(x+mu): stored
+                cx<T> g1[9], u[9], t[9], r[9];
+                load_g01<T, PACK, GBUF>(gsrc, V, sp, a, g1);
+                su3_row2(g1);
+                load_link_in<T, NE>(lin, V, mu, s, u);
+                mul_rows<R>(g0, u, t);
+                mul_rows_dag<R>(t, g1, r);
+                cx<T> *p = lout + (int64_t)mu * NE * V + s;
+#pragma unroll
+                for (int k = 0; k < NE; k++) st_link(p + (int64_t)k * V, r[k]);
+                if (NE == 6) su3_row2(r);          // what a later load of the stored rows rebuilds (R15)
+                tr += r[0].x + r[4].x + r[8].x;
+                acc_ah<T>(r, (T)-1, di, E);
+            }
+            {   // U'_mu(x-mu) = g(x-mu) U_mu(x-mu) g^dagger(x): only its contribution to A'(x)
+                cx<T> gb[9], u[9], t[9], r[9];
+                load_g01<T, PACK, GBUF>(gsrc, V, sb, a, gb);
+                if (NE == 9) su3_row2(gb);
+                load_link_in<T, NE>(lin, V, mu, sb, u);
+                mul_rows<R>(gb, u, t);
+                mul_rows_dag<R>(t, g0, r);
+                if (NE == 6) su3_row2(r);
+                acc_ah<T>(r, (T)1, di, E);
+            }
+        }
+        trF = (double)tr;
+        T d0 = 2 * di[0], d1 = 2 * di[1], d2 = 2 * di[2];
+        const T m = (d0 + d1 + d2) * (T)(1.0 / 3.0);
+        d0 -= m; d1 -= m; d2 -= m;
+        th = (double)(d0 * d0 + d1 * d1 + d2 * d2) + 2.0 * (double)(cnorm2(E[0]) + cnorm2(E[1]) + cnorm2(E[2]));
+        if (PACK == 4) {
+            wout[s] = mk<T>(d0, d1);
+            wout[V + s] = E[0];
+            wout[2 * V + s] = E[1];
+            wout[3 * V + s] = E[2];
+        } else {
+            wout[s] = mk<T>(0, d0);
+            wout[V + s] = E[0];
+            wout[2 * V + s] = E[1];
+            wout[3 * V + s] = mk<T>(-E[0].x, E[0].y);
+            wout[4 * V + s] = mk<T>(0, d1);
+            wout[5 * V + s] = E[2];
+            wout[6 * V + s] = mk<T>(-E[1].x, E[1].y);
+            wout[7 * V + s] = mk<T>(-E[2].x, E[2].y);
+            wout[8 * V + s] = mk<T>(0, d2);
+        }
+    }
+    finish_measure<FUSED_THREADS>(trF, th, V, ctrl, partials, hist, eps, 1);
+}
+
+int fused_blocks(int64_t V) { return (int)((V + FUSED_THREADS - 1) / FUSED_THREADS); }
+
+void launch_update_measure(const SiteArgs &a, const void *lin, void *lout, const void *gsrc, int gbuf, void *wout,
+                           double alpha, double eps, cudaStream_t st)
+{
+    const int nb = fused_blocks(a.geo.V);
+#define CALL(T, NE, PACK, GB) \
+    k_update_measure<T, NE, PACK, GB><<<nb, FUSED_THREADS, 0, st>>>((const cx<T> *)lin, (cx<T> *)lout, (const cx<T> *)gsrc, \
+        (cx<T> *)wout, a.geo, (T)(alpha / 2.0), a.ctrl, a.partials, a.hist, eps)
+#define CALL_NE(T, NE)                                           \
+    do {                                                         \
+        if (gbuf) { CALL(T, NE, 4, true); }                      \
+        else if (a.pack == 4) { CALL(T, NE, 4, false); }         \
+        else { CALL(T, NE, 9, false); }                          \
+    } while (0)
+    if (a.prec == 0) { if (a.recon == 12) CALL_NE(double, 6); else CALL_NE(double, 9); }
+    else             { if (a.recon == 12) CALL_NE(float, 6); else CALL_NE(float, 9); }
+#undef CALL_NE
+#undef CALL
+}
+
+} // namespace lgf

@@ -7,36 +7,11 @@
 // contiguous run of 16-byte (FP64) or 8-byte (FP32) complex numbers.
 #include "launch.h"
 #include "su3.cuh"
+#include "reduce.cuh"
 
 namespace lgf {
 
 static const int SITE_THREADS = 128;
-
-// ------------------------------------------------------------------ block reduction (fixed order)
-__device__ __forceinline__ double warp_sum(double v)
-{
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
-    return v;
-}
-
-// Sum of (a, b) over the block; result valid in thread 0.  Order is fixed by the code, so
-// the sums are bitwise reproducible run to run.
-template <int THREADS> __device__ __forceinline__ void block_sum2(double &a, double &b)
-{
-    __shared__ double sa[THREADS / 32], sb[THREADS / 32];
-    a = warp_sum(a); b = warp_sum(b);
-    int w = threadIdx.x >> 5, l = threadIdx.x & 31;
-    if (l == 0) { sa[w] = a; sb[w] = b; }
-    __syncthreads();
-    if (threadIdx.x == 0) {
-        double ta = 0, tb = 0;
-#pragma unroll
-        for (int i = 0; i < THREADS / 32; i++) { ta += sa[i]; tb += sb[i]; }
-        a = ta; b = tb;
-    }
-    __syncthreads();
-}
 
 // ------------------------------------------------------------------ kernel (a)
 // A = sum_nu [U_nu(x-nu) - U_nu(x)];  Delta = (A - A^dagger) - (1/3) Tr(A - A^dagger) 1  (reading R3).
@@ -93,32 +68,7 @@ k_measure(const cx<T> *__restrict__ links, cx<T> *__restrict__ w, Geom geo, Ctrl
             w[8 * V + s] = mk<T>(0, d2);
         }
     }
-    block_sum2<SITE_THREADS>(trF, th);
-    __shared__ bool last;
-    if (threadIdx.x == 0) {
-        partials[2 * (int64_t)blockIdx.x] = trF;
-        partials[2 * (int64_t)blockIdx.x + 1] = th;
-        __threadfence();
-        const unsigned tk = atomicInc(&ctrl->ticket, gridDim.x - 1); // wraps back to 0 for the next launch
-        last = (tk == gridDim.x - 1);
-    }
-    __syncthreads();
-    if (!last) return;
-    __threadfence();
-    double f = 0, t = 0;
-    for (unsigned i = threadIdx.x; i < gridDim.x; i += SITE_THREADS) {
-        f += __ldcg(partials + 2 * (int64_t)i);
-        t += __ldcg(partials + 2 * (int64_t)i + 1);
-    }
-    block_sum2<SITE_THREADS>(f, t);
-    if (threadIdx.x == 0) {
-        const double F = f / (12.0 * (double)V), theta = t / (3.0 * (double)V);
-        long long it = ctrl->iter + (count_iter ? 1 : 0);
-        ctrl->F = F; ctrl->theta = theta; ctrl->iter = it;
-        if (it < LGF_HIST_CAP) hist[it] = make_double2(F, theta);
-        if (!(theta == theta) || theta > 1.0e300) ctrl->done = 2;
-        else if (theta <= eps) ctrl->done = 1;
-    }
+    finish_measure<SITE_THREADS>(trF, th, V, ctrl, partials, hist, eps, count_iter);
 }
 
 __global__ void k_ctrl_reset(Ctrl *ctrl, double2 *hist, double eps)

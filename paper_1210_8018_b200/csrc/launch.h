@@ -21,6 +21,11 @@ void launch_measure(const SiteArgs &a, double eps, int count_iter, cudaStream_t 
 int measure_blocks(int64_t V);
 // kernel (c): g(x) = reunit(1 + (alpha/2) w), U_mu(x) <- g(x) U_mu(x) g^dagger(x+mu)
 void launch_update(const SiteArgs &a, double alpha, cudaStream_t st);
+// kernels (c) + (a) fused: lin -> lout (distinct buffers), Delta of the new links -> wout, F, theta.
+// gsrc: the g buffer (gbuf = 1: 6 complex arrays over sites) or w (gbuf = 0: a.pack fields; then wout != gsrc).
+void launch_update_measure(const SiteArgs &a, const void *lin, void *lout, const void *gsrc, int gbuf, void *wout,
+                           double alpha, double eps, cudaStream_t st);
+int fused_blocks(int64_t V);
 // iter = 0, hist[0] = (F, theta), done = (theta <= eps)
 void launch_ctrl_reset(const SiteArgs &a, double eps, cudaStream_t st);
 
@@ -47,6 +52,8 @@ int launch_fft_generic(const FftArgs &a, cudaStream_t st);
 // tiled register FFT: three passes.  which = 0 (x,y) forward, 1 (z,t) forward*mask*inverse, 2 (x,y) inverse
 bool fft_tiled_supported(const int N[4], int prec);
 void launch_fft_tiled(const FftArgs &a, int which, cudaStream_t st);
+// pass 2 of all 4 packed fields with g(x) = reunit(1 + (alpha/2) w(x)) as its epilogue: rows 0, 1 of g -> gbuf
+void launch_fft_tiled_inv_g(const FftArgs &a, void *gbuf, double alpha, cudaStream_t st);
 int fft_tiled_setup(const int N[4], int prec); // sets kernel attributes (smem opt-in); 0 on success
 
 } // namespace lgf

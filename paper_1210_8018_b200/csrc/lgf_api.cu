@@ -2,6 +2,7 @@
 // Owns no device memory: carves the caller's workspace, launches the kernels of
 // kernels_site.cu / fft_tiled.cu / fft_generic.cu on the caller's stream, and keeps the
 // loop of Algorithm 1 on the device between polls of the `done` flag.
+#include <algorithm>
 #include <cmath>
 #include <cstdio>
 #include <cstring>
@@ -24,7 +25,7 @@ struct EvPair { cudaEvent_t a, b; int kind; };
 size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 
 struct Layout {
-    size_t links, w, partials, ctrl, hist, ptab, tw, staging, total;
+    size_t links[2], w[2], gbuf, partials, ctrl, hist, ptab, tw, staging, total;
     int64_t staging_sites;
 };
 
@@ -34,7 +35,10 @@ struct lgf_ctx {
     int N[4];
     int64_t V;
     int prec;
-    int recon = 18, pack = 4, check_interval = 8, fft_path = 0, profile = 0;
+    int recon = 18, pack = 4, check_interval = 8, fft_path = 0, profile = 0, fusion = 1;
+    int cur = 0, wcur = 0;   // which of the two link / field buffers is current
+    bool use_gbuf = false;   // last FFT pass writes g (fusion, tiled FFT, 4 packed fields)
+    void *links_buf[2] = {nullptr, nullptr}, *w_buf[2] = {nullptr, nullptr}, *gbuf = nullptr;
     int64_t max_iter = 100000;
     bool bound = false, loaded = false;
     int wstate = 0; // 0 invalid, 1 holds Delta of the current links, 2 holds w
@@ -65,9 +69,17 @@ Layout make_layout(const lgf_ctx *c)
     const size_t e = elem_bytes(c);
     const int ne = c->recon == 12 ? 6 : 9;
     size_t off = 0;
-    L.links = off; off = align_up(off + (size_t)4 * ne * c->V * e, 256);
-    L.w = off; off = align_up(off + (size_t)c->pack * c->V * e, 256);
-    L.partials = off; off = align_up(off + (size_t)2 * measure_blocks(c->V) * sizeof(double), 256);
+    // fusion: links are double-buffered (the fused kernel reads old neighbours while new links
+    // are written); the fields are double-buffered when g is rebuilt from w inside that kernel,
+    // else the last FFT pass writes rows 0, 1 of g (6 complex per site) to gbuf
+    const int nl = c->fusion ? 2 : 1;
+    const bool gb = c->fusion && c->pack == 4 && c->fft_path == 0 && fft_tiled_supported(c->N, c->prec);
+    const int nw = (c->fusion && !gb) ? 2 : 1;
+    for (int i = 0; i < 2; i++) { L.links[i] = off; if (i < nl) off = align_up(off + (size_t)4 * ne * c->V * e, 256); }
+    for (int i = 0; i < 2; i++) { L.w[i] = off; if (i < nw) off = align_up(off + (size_t)c->pack * c->V * e, 256); }
+    L.gbuf = off; if (gb) off = align_up(off + (size_t)6 * c->V * e, 256);
+    const int nblk = std::max(measure_blocks(c->V), fused_blocks(c->V));
+    L.partials = off; off = align_up(off + (size_t)2 * nblk * sizeof(double), 256);
     L.ctrl = off; off = align_up(off + sizeof(Ctrl), 256);
     L.hist = off; off = align_up(off + (size_t)LGF_HIST_CAP * sizeof(double2), 256);
     L.ptab = off; off = align_up(off + (size_t)sum_n(c) * sizeof(double), 256);
@@ -136,6 +148,13 @@ void flush_events(lgf_ctx *c)
     c->ev_used = 0;
 }
 
+void sync_ptrs(lgf_ctx *c)
+{
+    c->sa.links = c->links_buf[c->cur];
+    c->sa.w = c->w_buf[c->wcur];
+    c->fa.w = c->sa.w;
+}
+
 void do_measure(lgf_ctx *c, double eps, int count_iter)
 {
     run_kernel(c, LGF_KERNEL_MEASURE, 1, [&] { launch_measure(c->sa, eps, count_iter, c->st); });
@@ -163,9 +182,40 @@ void do_update(lgf_ctx *c, double alpha)
 // one execution of the loop body of Algorithm 1 (lines 3-17) on the device
 void do_iteration(lgf_ctx *c, double alpha, double eps)
 {
-    do_fourier(c);
-    do_update(c, alpha);
-    do_measure(c, eps, 1);
+    if (!c->fusion) {
+        do_fourier(c);
+        do_update(c, alpha);
+        do_measure(c, eps, 1);
+        return;
+    }
+    // w_buf[wcur] holds Delta of links_buf[cur]
+    void *lin = c->links_buf[c->cur], *lout = c->links_buf[c->cur ^ 1];
+    if (c->use_gbuf) {
+        run_kernel(c, LGF_KERNEL_FFT_XY_FWD, 1, [&] { launch_fft_tiled(c->fa, 0, c->st); });
+        run_kernel(c, LGF_KERNEL_FFT_ZT, 1, [&] { launch_fft_tiled(c->fa, 1, c->st); });
+        run_kernel(c, LGF_KERNEL_FFT_XY_INV_G, 1, [&] { launch_fft_tiled_inv_g(c->fa, c->gbuf, alpha, c->st); });
+        run_kernel(c, LGF_KERNEL_UPDATE_MEASURE, 1,
+                   [&] { launch_update_measure(c->sa, lin, lout, c->gbuf, 1, c->w_buf[c->wcur], alpha, eps, c->st); });
+    } else {
+        do_fourier(c);
+        void *win = c->w_buf[c->wcur], *wout = c->w_buf[c->wcur ^ 1];
+        run_kernel(c, LGF_KERNEL_UPDATE_MEASURE, 1,
+                   [&] { launch_update_measure(c->sa, lin, lout, win, 0, wout, alpha, eps, c->st); });
+        c->wcur ^= 1;
+    }
+    c->cur ^= 1;
+    sync_ptrs(c);
+    c->wstate = 1;
+}
+
+// Kernels launched after the device raised `done` exit without writing, so after a poll the
+// current buffers are those of the `executed`-th iteration since `cur0` / `wcur0`.
+void settle_buffers(lgf_ctx *c, int cur0, int wcur0, long long executed)
+{
+    if (!c->fusion) return;
+    c->cur = cur0 ^ (int)(executed & 1);
+    if (!c->use_gbuf) c->wcur = wcur0 ^ (int)(executed & 1);
+    sync_ptrs(c);
 }
 
 int read_ctrl(lgf_ctx *ctx, Ctrl *h)
@@ -229,7 +279,7 @@ int lgf_create(int Nx, int Ny, int Nz, int Nt, int precision, lgf_ctx **out)
 int lgf_set_option(lgf_ctx *ctx, int key, int64_t value)
 {
     if (!ctx) return LGF_ERR_INVALID_ARG;
-    const bool layout_key = (key == LGF_OPT_RECON || key == LGF_OPT_FFT_BATCH || key == LGF_OPT_FFT_PATH);
+    const bool layout_key = (key == LGF_OPT_RECON || key == LGF_OPT_FFT_BATCH || key == LGF_OPT_FFT_PATH || key == LGF_OPT_FUSION);
     if (layout_key && ctx->bound) return fail(ctx, LGF_ERR_INVALID_ARG, "this option must be set before lgf_bind");
     switch (key) {
     case LGF_OPT_RECON:
@@ -247,6 +297,9 @@ int lgf_set_option(lgf_ctx *ctx, int key, int64_t value)
     case LGF_OPT_FFT_PATH:
         if (value != 0 && value != 1) return fail(ctx, LGF_ERR_INVALID_ARG, "FFT_PATH must be 0 or 1");
         ctx->fft_path = (int)value; break;
+    case LGF_OPT_FUSION:
+        if (value != 0 && value != 1) return fail(ctx, LGF_ERR_INVALID_ARG, "FUSION must be 0 or 1");
+        ctx->fusion = (int)value; break;
     case LGF_OPT_PROFILE:
         if (ctx->bound) flush_events(ctx);
         ctx->profile = value ? 1 : 0; break;
@@ -278,14 +331,16 @@ int lgf_bind(lgf_ctx *ctx, void *dev_workspace, size_t bytes, void *cuda_stream)
     g.st[0] = 1; g.st[1] = g.N[0]; g.st[2] = (int64_t)g.N[0] * g.N[1]; g.st[3] = (int64_t)g.N[0] * g.N[1] * g.N[2];
     SiteArgs &s = ctx->sa;
     s.geo = g;
-    s.links = ctx->base + L.links;
-    s.w = ctx->base + L.w;
+    for (int i = 0; i < 2; i++) { ctx->links_buf[i] = ctx->base + L.links[i]; ctx->w_buf[i] = ctx->base + L.w[i]; }
+    ctx->gbuf = ctx->base + L.gbuf;
+    ctx->cur = 0; ctx->wcur = 0;
     s.partials = (double *)(ctx->base + L.partials);
     s.ctrl = (Ctrl *)(ctx->base + L.ctrl);
     s.hist = (double2 *)(ctx->base + L.hist);
     s.prec = ctx->prec; s.recon = ctx->recon; s.pack = ctx->pack;
     FftArgs &f = ctx->fa;
-    f.geo = g; f.w = s.w; f.nfields = ctx->pack; f.prec = ctx->prec;
+    f.geo = g; f.nfields = ctx->pack; f.prec = ctx->prec;
+    sync_ptrs(ctx);
     f.ptab = (const double *)(ctx->base + L.ptab);
     f.pmax2 = ctx->pmax2;
     f.tw = ctx->base + L.tw;
@@ -312,6 +367,7 @@ int lgf_bind(lgf_ctx *ctx, void *dev_workspace, size_t bytes, void *cuda_stream)
         cudaError_t e = cudaGetLastError();
         return cuda_fail(ctx, e, "fft_tiled_setup");
     }
+    ctx->use_gbuf = ctx->fusion && ctx->tiled && ctx->pack == 4;
     ctx->bound = true;
     ctx->loaded = false;
     ctx->wstate = 0;
@@ -389,11 +445,13 @@ int lgf_iterate(lgf_ctx *ctx, double alpha, int64_t n, lgf_result *out)
         do_measure(ctx, -1.0, 0);
     }
     run_kernel(ctx, LGF_KERNEL_LAYOUT, 1, [&] { launch_ctrl_reset(ctx->sa, -1.0, ctx->st); });
+    const int cur0 = ctx->cur, wcur0 = ctx->wcur;
     for (int64_t i = 0; i < n; i++) do_iteration(ctx, alpha, -1.0);
     CK(cudaGetLastError());
     if (out) {
         Ctrl h;
         if ((rc = read_ctrl(ctx, &h))) return rc;
+        settle_buffers(ctx, cur0, wcur0, h.iter);
         out->iterations = h.iter; out->F = h.F; out->theta = h.theta; out->converged = 0;
         if (h.done == 2) return fail(ctx, LGF_ERR_NUMERIC, "theta is NaN or Inf");
     }
@@ -413,6 +471,7 @@ int lgf_fix(lgf_ctx *ctx, double alpha, double eps, lgf_result *out)
     Ctrl h;
     if ((rc = read_ctrl(ctx, &h))) return rc;
     int64_t launched = 0;
+    const int cur0 = ctx->cur, wcur0 = ctx->wcur;
     while (!h.done && launched < ctx->max_iter) {
         const int64_t n = std::min<int64_t>(ctx->check_interval, ctx->max_iter - launched);
         for (int64_t i = 0; i < n; i++) do_iteration(ctx, alpha, eps);
@@ -420,6 +479,7 @@ int lgf_fix(lgf_ctx *ctx, double alpha, double eps, lgf_result *out)
         CK(cudaGetLastError());
         if ((rc = read_ctrl(ctx, &h))) return rc;
     }
+    settle_buffers(ctx, cur0, wcur0, h.iter);
     ctx->wstate = 1; // kernels after `done` exited at once: w still holds Delta of the final links
     if (out) { out->iterations = h.iter; out->F = h.F; out->theta = h.theta; out->converged = (h.done == 1); }
     if (h.done == 2) return fail(ctx, LGF_ERR_NUMERIC, "theta is NaN or Inf");

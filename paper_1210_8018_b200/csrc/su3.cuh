@@ -8,9 +8,9 @@ namespace lgf {
 // (12-real compression; reading R15).  m[0..5] given, m[6..8] written.
 template <typename V> __device__ __forceinline__ void su3_row2(V (&m)[9])
 {
-    m[6] = cconj(cmul(m[1], m[5]) - cmul(m[2], m[4]));
-    m[7] = cconj(cmul(m[2], m[3]) - cmul(m[0], m[5]));
-    m[8] = cconj(cmul(m[0], m[4]) - cmul(m[1], m[3]));
+    m[6] = cconj(cfms(m[2], m[4], cmul(m[1], m[5])));
+    m[7] = cconj(cfms(m[0], m[5], cmul(m[2], m[3])));
+    m[8] = cconj(cfms(m[1], m[3], cmul(m[0], m[4])));
 }
 
 // Load U_mu(s) from the SoA link arrays: element k = 3*row + col of direction mu lives at
@@ -28,23 +28,42 @@ template <typename T> __device__ __forceinline__ T rsqrt_t(T x);
 template <> __device__ __forceinline__ double rsqrt_t<double>(double x) { return rsqrt(x); }
 template <> __device__ __forceinline__ float rsqrt_t<float>(float x) { return rsqrtf(x); }
 
-// g = reunit(m): Gram-Schmidt on rows 0, 1 of m, row 2 = conj(row0 x row1)
-// ("followed by a reunitarization"; readings R12, R13).
-// m[0..5] = rows 0, 1 on entry; g[0..8] on exit.
-template <typename T> __device__ __forceinline__ void reunit(cx<T> (&g)[9])
+// Gram-Schmidt on rows 0, 1 of m in place ("followed by a reunitarization";
+// DESIGN.md readings R12, R13).  Row 2 is not touched.
+template <typename T> __device__ __forceinline__ void reunit01(cx<T> (&g)[9])
 {
     T n0 = rsqrt_t<T>(cnorm2(g[0]) + cnorm2(g[1]) + cnorm2(g[2]));
     g[0] = cscale(g[0], n0); g[1] = cscale(g[1], n0); g[2] = cscale(g[2], n0);
     // <u, m1> = sum_j conj(u_j) m_1j
     cx<T> ip = cconjmul(g[0], g[3]);
-    ip = ip + cconjmul(g[1], g[4]);
-    ip = ip + cconjmul(g[2], g[5]);
-    g[3] = g[3] - cmul(ip, g[0]);
-    g[4] = g[4] - cmul(ip, g[1]);
-    g[5] = g[5] - cmul(ip, g[2]);
+    ip = cfmaconj(g[1], g[4], ip);
+    ip = cfmaconj(g[2], g[5], ip);
+    g[3] = cfms(ip, g[0], g[3]);
+    g[4] = cfms(ip, g[1], g[4]);
+    g[5] = cfms(ip, g[2], g[5]);
     T n1 = rsqrt_t<T>(cnorm2(g[3]) + cnorm2(g[4]) + cnorm2(g[5]));
     g[3] = cscale(g[3], n1); g[4] = cscale(g[4], n1); g[5] = cscale(g[5], n1);
+}
+
+// g = reunit(m): Gram-Schmidt on rows 0, 1 of m, row 2 = conj(row0 x row1).
+// m[0..5] = rows 0, 1 on entry; g[0..8] on exit.
+template <typename T> __device__ __forceinline__ void reunit(cx<T> (&g)[9])
+{
+    reunit01<T>(g);
     su3_row2(g);
+}
+
+// Rows 0, 1 of m = 1 + a w from the 4 packed fields f0 = Im w00 + i Im w11, f1 = w01, f2 = w02,
+// f3 = w12 (w anti-Hermitian traceless, so w10 = -conj(w01)); a = alpha/2 (eq. 1.2).
+template <typename T>
+__device__ __forceinline__ void m_from_packed(cx<T> f0, cx<T> f1, cx<T> f2, cx<T> f3, T a, cx<T> (&g)[9])
+{
+    g[0] = mk<T>((T)1, a * f0.x);
+    g[1] = cscale(f1, a);
+    g[2] = cscale(f2, a);
+    g[3] = mk<T>(-a * f1.x, a * f1.y);
+    g[4] = mk<T>((T)1, a * f0.y);
+    g[5] = cscale(f3, a);
 }
 
 // Rows 0, 1 of w(x) from the field buffer, then g(x) = reunit(1 + (alpha/2) w(x)), a = alpha/2
@@ -62,14 +81,31 @@ __device__ __forceinline__ void build_g(const cx<T> *__restrict__ w, int64_t V, 
         g[0].x += (T)1; g[4].x += (T)1;
     } else {
         cx<T> f0 = __ldg(w + s), f1 = __ldg(w + V + s), f2 = __ldg(w + 2 * V + s), f3 = __ldg(w + 3 * V + s);
-        g[0] = mk<T>((T)1, a * f0.x);
-        g[1] = cscale(f1, a);
-        g[2] = cscale(f2, a);
-        g[3] = mk<T>(-a * f1.x, a * f1.y);
-        g[4] = mk<T>((T)1, a * f0.y);
-        g[5] = cscale(f3, a);
+        m_from_packed<T>(f0, f1, f2, f3, a, g);
     }
     reunit<T>(g);
+}
+
+// Rows 0, 1 of g(s) (g[0..5]) for the fused kernel: read from the g buffer written by the last
+// FFT pass (GBUF: 6 complex SoA arrays over sites) or built from w as above.  Row 2 is left
+// to the caller (su3_row2) because not every use needs it.
+template <typename T, int PACK, bool GBUF>
+__device__ __forceinline__ void load_g01(const cx<T> *__restrict__ src, int64_t V, int64_t s, T a, cx<T> (&g)[9])
+{
+    if (GBUF) {
+#pragma unroll
+        for (int k = 0; k < 6; k++) g[k] = __ldg(src + (int64_t)k * V + s);
+    } else {
+        if (PACK == 9) {
+#pragma unroll
+            for (int k = 0; k < 6; k++) g[k] = cscale(__ldg(src + (int64_t)k * V + s), a);
+            g[0].x += (T)1; g[4].x += (T)1;
+        } else {
+            cx<T> f0 = __ldg(src + s), f1 = __ldg(src + V + s), f2 = __ldg(src + 2 * V + s), f3 = __ldg(src + 3 * V + s);
+            m_from_packed<T>(f0, f1, f2, f3, a, g);
+        }
+        reunit01<T>(g);
+    }
 }
 
 // rows [0, R) of c = a b

@@ -55,7 +55,11 @@ def test_options_and_workspace_size(L):
     ctx = ctypes.c_void_p()
     assert L.lgf_create(32, 32, 32, 32, lgf.PREC_FP64, ctypes.byref(ctx)) == lgf.OK
     V = 32 ** 4
+    bfused = L.lgf_workspace_bytes(ctx)
+    assert L.lgf_set_option(ctx, lgf.OPT_FUSION, 2) == lgf.ERR_INVALID_ARG
+    assert L.lgf_set_option(ctx, lgf.OPT_FUSION, 0) == lgf.OK
     b18 = L.lgf_workspace_bytes(ctx)
+    assert bfused - b18 == (4 * 9 + 6) * V * 16          # fusion: second link buffer + rows 0, 1 of g
     assert L.lgf_set_option(ctx, lgf.OPT_RECON, 12) == lgf.OK
     b12 = L.lgf_workspace_bytes(ctx)
     assert b18 - b12 == 4 * 3 * V * 16                   # row 2 of every link is not stored

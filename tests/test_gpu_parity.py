@@ -39,7 +39,9 @@ LATTICES = [
     ((12, 12, 12, 12), 0.5, 79),        # radix-3 lines of the tiled FFT
 ]
 VARIANTS = [dict(recon=18, fft_batch=4), dict(recon=12, fft_batch=4), dict(recon=18, fft_batch=9),
-            dict(recon=12, fft_batch=9), dict(recon=18, fft_batch=4, fft_path=1)]
+            dict(recon=12, fft_batch=9), dict(recon=18, fft_batch=4, fft_path=1),
+            # the three separate kernels of the paper's kernel list instead of the fused default
+            dict(recon=12, fft_batch=4, fusion=0), dict(recon=18, fft_batch=9, fusion=0)]
 
 
 def ids(v):
@@ -136,7 +138,7 @@ def test_one_iteration_matches_oracle(lgf, lat, var):
 @pytest.mark.parametrize("n,sigma,seed", [(8, 0.3, gen.BASE_SEED + 8), (8, 0.3, gen.BASE_SEED + 1008),
                                           (8, 0.3, gen.BASE_SEED + 2008), (16, 0.5, gen.BASE_SEED + 16),
                                           (16, 0.5, gen.BASE_SEED + 1016)])
-@pytest.mark.parametrize("var", [VARIANTS[0], VARIANTS[1], VARIANTS[2]], ids=ids)
+@pytest.mark.parametrize("var", [VARIANTS[0], VARIANTS[1], VARIANTS[2], VARIANTS[4], VARIANTS[5]], ids=ids)
 def test_convergence_matches_oracle_golden(lgf, n, sigma, seed, var):
     it, F, th, hist = read_golden(golden_path(n, seed))
     U = gen.gen_links(n, sigma, seed)
