@@ -192,7 +192,9 @@ def run_ours(args):
     if args.recon:
         recon = args.recon
     V = N[0] * N[1] * N[2] * N[3]
-    seed = gen.BASE_SEED + soff + 7919 * rank           # every rank its own lattice (replicas)
+    from paper_1210_8018_b200 import replicas
+
+    seed = replicas.replica_seed(gen.BASE_SEED + soff, rank)   # every rank its own lattice (replicas)
     U = gen.gen_links(N, sigma, seed)
     cdt = np.complex128 if prec == "fp64" else np.complex64
     tdt = torch.complex128 if prec == "fp64" else torch.complex64
@@ -257,10 +259,7 @@ def run_ours(args):
     e2e_s = time.perf_counter() - te
     clocks = sampler.stop(t0, t1) if sampler else None
 
-    tmax = torch.tensor([ms, e2e_s], dtype=torch.float64, device=f"cuda:{local}")
-    if world > 1:
-        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
-    ms_all, e2e_all = float(tmax[0]), float(tmax[1])
+    (ms_all, e2e_all), _ = replicas.reduce_timing([ms, e2e_s], V * K, device=f"cuda:{local}")
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
