@@ -8,7 +8,9 @@
 // (four passes per direction change); here the reorder is tile
 // addressing and the mask and 1/V ride on the middle pass.
 //
-// Every 1D transform is done by ONE thread on a whole line held in registers: a fully
+// Every 1D transform is done on a whole line held in registers -- by ONE thread for lengths up
+// to 32, by TWO threads (lanes l and l^16, half a line each, one shuffle exchange) for 48 and
+// 64, where a line would not fit the register file -- as a fully
 // unrolled decimation-in-frequency network (natural order in, digit-reversed slots out)
 // with compile-time twiddles; the inverse right after the mask is the transposed
 // (decimation-in-time) network, which takes digit-reversed slots and returns natural order,
@@ -130,30 +132,121 @@ template <int N> __host__ __device__ constexpr int slot_freq(int s)
     return k;
 }
 
+// ---------------------------------------------------------------- a line held by S threads
+// S = 1: one thread holds the whole line.  S = 2: the line is shared by the lanes l and l^16 of
+// a warp (half h = 0, 1).  The first radix-2 stage of the decimation-in-frequency network,
+//     y[j] = x[j] + x[j+N/2],   z[j] = (x[j] - x[j+N/2]) exp(SIGN 2 pi i j/N),   j < N/2,
+// is done on the pairs each thread holds (j in [h N/4, (h+1) N/4)); then the two threads swap
+// half of their results by warp shuffle so that h = 0 owns all of y (even frequencies) and
+// h = 1 all of z (odd frequencies), and each runs the N/2-point network on its own.
+// The transposed (decimation-in-time) network runs the same steps backwards.
+// nat(i, h): line position held in local element i on the natural-order side;
+// slot(s, h): frequency (or position, for an inverse written as Dif) held in local slot s on the other side.
+template <typename T, int N, int S> struct Line;
+
+template <typename T, int N> struct Line<T, N, 1> {
+    static constexpr int NL = N;
+    static __device__ __forceinline__ int nat(int i, int) { return i; }
+    static __device__ __forceinline__ int slot(int s, int) { return slot_freq<N>(s); }
+    template <int SIGN> static __device__ __forceinline__ void dif(cx<T> (&v)[NL], int, unsigned) { Dif<T, N, N, SIGN>::run(v); }
+    template <int SIGN> static __device__ __forceinline__ void dit(cx<T> (&v)[NL], int, unsigned) { Dit<T, N, N, SIGN>::run(v); }
+};
+
+template <typename V> __device__ __forceinline__ V shfl16(unsigned mask, V v)
+{
+    v.x = __shfl_xor_sync(mask, v.x, 16);
+    v.y = __shfl_xor_sync(mask, v.y, 16);
+    return v;
+}
+// x * (SIGN i)
+template <int SIGN, typename V> __device__ __forceinline__ V rot90(V x)
+{
+    V r;
+    if (SIGN > 0) { r.x = -x.y; r.y = x.x; } else { r.x = x.y; r.y = -x.x; }
+    return r;
+}
+
+template <typename T, int N> struct Line<T, N, 2> {
+    static_assert(N % 4 == 0, "split lines need N divisible by 4");
+    static constexpr int NL = N / 2, Q = N / 4;
+    static __device__ __forceinline__ int nat(int i, int h) { return h * Q + i + (i >= Q ? Q : 0); }
+    static __device__ __forceinline__ int slot(int s, int h) { return 2 * slot_freq<NL>(s) + h; }
+    template <int SIGN> static __device__ __forceinline__ void dif(cx<T> (&v)[NL], int h, unsigned mask)
+    {
+#pragma unroll
+        for (int i = 0; i < Q; i++) {
+            const cx<T> a = v[i], b = v[Q + i];
+            const cx<T> y = a + b;
+            cx<T> z = mul_tw<T, N, SIGN>(a - b, i);
+            if (h) z = rot90<SIGN>(z);                       // exp(SIGN 2 pi i (N/4)/N) = SIGN i
+            const cx<T> got = shfl16(mask, h ? y : z);       // h = 0 gives z away, h = 1 gives y away
+            v[i] = h ? got : y;
+            v[Q + i] = h ? z : got;
+        }
+        Dif<T, NL, NL, SIGN>::run(v);
+    }
+    template <int SIGN> static __device__ __forceinline__ void dit(cx<T> (&v)[NL], int h, unsigned mask)
+    {
+        Dit<T, NL, NL, SIGN>::run(v);
+#pragma unroll
+        for (int i = 0; i < Q; i++) {
+            const cx<T> got = shfl16(mask, h ? v[i] : v[Q + i]);
+            const cx<T> y = h ? got : v[i];
+            cx<T> z = h ? v[Q + i] : got;
+            z = mul_tw<T, N, SIGN>(z, i);
+            if (h) z = rot90<SIGN>(z);
+            v[i] = y + z;
+            v[Q + i] = y - z;
+        }
+    }
+};
+
+// thread t of a group -> (line, half).  S = 2 keeps the two halves of a line 16 lanes apart, so
+// that the 8 lanes of a shared-memory wavefront still belong to 8 consecutive lines.
+template <int S> __device__ __forceinline__ void line_of_thread(int t, int &line, int &h)
+{
+    if (S == 1) { line = t; h = 0; }
+    else { h = (t >> 4) & 1; line = (t & 15) | ((t >> 5) << 4); }
+}
+constexpr int split_of(int n) { return n >= 48 ? 2 : 1; }
+
 // ---------------------------------------------------------------- tile geometry
 // Shared tile of a group: element (c, a, b) at (b*RS + a*C + c), RS = NA*C + C (one padding
 // column block per row keeps 16-byte accesses of 8 consecutive threads on distinct banks).
+// Lines along a: C*NB of them, SA threads each; lines along b: C*NA, SB threads each.
+constexpr int imax(int a, int b) { return a > b ? a : b; }
 template <int NA, int NB, int C> struct Tile {
+    static constexpr int SA = split_of(NA), SB = split_of(NB);
     static constexpr int RS = NA * C + C;
     static constexpr int ELEMS = RS * NB;
-    static constexpr int THREADS = C * (NA > NB ? NA : NB);
+    static constexpr int THREADS = C * imax(SA * NB, SB * NA);
 };
-
-static const int CTA_THREADS = 128;
+// CTA size: at least 128 threads, whole groups
+constexpr int cta_threads(int group) { return group >= 128 ? group : (128 / group) * group; }
 
 // ---------------------------------------------------------------- pass 0 / pass 2: (x,y) planes
 // INVERSE = 0: load columns (lines along y) straight from global, Dif along y, through shared
 //              memory, Dif along x, back through shared memory, coalesced store.
 // INVERSE = 1: coalesced load into shared memory, Dif(+) along x, shared, Dif(+) along y,
 //              store straight from registers.  Natural order in global memory in both cases.
+template <typename T, int NA, int NB> struct XYCfg {
+    typedef Tile<NA, NB, 1> TL;
+    static constexpr int TP = TL::THREADS;             // threads of one plane
+    static constexpr int CTA = cta_threads(TP);
+    static constexpr int G = CTA / TP;                 // planes per CTA
+    static constexpr size_t SMEM = (size_t)G * TL::ELEMS * sizeof(cx<T>);
+};
+
 template <typename T, int NA, int NB, int INVERSE>
-__global__ void __launch_bounds__(CTA_THREADS)
+__global__ void __launch_bounds__((XYCfg<T, NA, NB>::CTA))
 k_fft_xy(cx<T> *__restrict__ w, int64_t nplanes, const Ctrl *ctrl)
 {
     if (*(volatile const int *)&ctrl->done) return;
-    typedef Tile<NA, NB, 1> TL;
-    constexpr int TP = TL::THREADS;               // threads of one plane
-    constexpr int G = CTA_THREADS / TP;           // planes per CTA
+    typedef XYCfg<T, NA, NB> CF;
+    typedef typename CF::TL TL;
+    typedef Line<T, NA, TL::SA> LA;
+    typedef Line<T, NB, TL::SB> LB;
+    constexpr int TP = CF::TP, G = CF::G;
     constexpr int SIGN = INVERSE ? +1 : -1;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int grp = threadIdx.x / TP, t = threadIdx.x % TP;
@@ -161,52 +254,57 @@ k_fft_xy(cx<T> *__restrict__ w, int64_t nplanes, const Ctrl *ctrl)
     const int64_t plane = (int64_t)blockIdx.x * G + grp;
     const bool ok = plane < nplanes && grp < G;
     cx<T> *f = w + plane * (int64_t)(NA * NB);
+    int xa, ha, yb, hb;                                   // thread as (x, half) of a y-line / (ky, half) of an x-line
+    line_of_thread<TL::SB>(t, xa, ha);
+    line_of_thread<TL::SA>(t, yb, hb);
+    const bool on_y = ok && xa < NA && t < TL::SB * NA, on_x = ok && yb < NB && t < TL::SA * NB;
+    const unsigned my = __ballot_sync(0xffffffffu, on_y), mx = __ballot_sync(0xffffffffu, on_x);
 
     if (!INVERSE) {
-        if (ok && t < NA) {                       // thread = x, line along y
-            cx<T> v[NB];
+        if (on_y) {                                       // line along y at x = xa
+            cx<T> v[LB::NL];
 #pragma unroll
-            for (int j = 0; j < NB; j++) v[j] = f[j * NA + t];
-            Dif<T, NB, NB, SIGN>::run(v);
+            for (int i = 0; i < LB::NL; i++) v[i] = f[LB::nat(i, ha) * NA + xa];
+            LB::template dif<SIGN>(v, ha, my);
 #pragma unroll
-            for (int s = 0; s < NB; s++) sm[slot_freq<NB>(s) * TL::RS + t] = v[s];
+            for (int q = 0; q < LB::NL; q++) sm[LB::slot(q, ha) * TL::RS + xa] = v[q];
         }
         __syncthreads();
-        if (ok && t < NB) {                       // thread = ky, line along x
-            cx<T> v[NA];
+        if (on_x) {                                       // line along x at ky = yb
+            cx<T> v[LA::NL];
 #pragma unroll
-            for (int j = 0; j < NA; j++) v[j] = sm[t * TL::RS + j];
-            Dif<T, NA, NA, SIGN>::run(v);
+            for (int i = 0; i < LA::NL; i++) v[i] = sm[yb * TL::RS + LA::nat(i, hb)];
+            LA::template dif<SIGN>(v, hb, mx);
 #pragma unroll
-            for (int s = 0; s < NA; s++) sm[t * TL::RS + slot_freq<NA>(s)] = v[s];
+            for (int q = 0; q < LA::NL; q++) sm[yb * TL::RS + LA::slot(q, hb)] = v[q];
         }
         __syncthreads();
-        if (ok && t < NA) {
-#pragma unroll
-            for (int j = 0; j < NB; j++) f[j * NA + t] = sm[j * TL::RS + t];
+        if (ok) {
+#pragma unroll 4
+            for (int e = t; e < NA * NB; e += TP) f[e] = sm[(e / NA) * TL::RS + (e % NA)];
         }
     } else {
-        if (ok && t < NA) {
-#pragma unroll
-            for (int j = 0; j < NB; j++) sm[j * TL::RS + t] = f[j * NA + t];
+        if (ok) {
+#pragma unroll 4
+            for (int e = t; e < NA * NB; e += TP) sm[(e / NA) * TL::RS + (e % NA)] = f[e];
         }
         __syncthreads();
-        if (ok && t < NB) {
-            cx<T> v[NA];
+        if (on_x) {
+            cx<T> v[LA::NL];
 #pragma unroll
-            for (int j = 0; j < NA; j++) v[j] = sm[t * TL::RS + j];
-            Dif<T, NA, NA, SIGN>::run(v);
+            for (int i = 0; i < LA::NL; i++) v[i] = sm[yb * TL::RS + LA::nat(i, hb)];
+            LA::template dif<SIGN>(v, hb, mx);
 #pragma unroll
-            for (int s = 0; s < NA; s++) sm[t * TL::RS + slot_freq<NA>(s)] = v[s];
+            for (int q = 0; q < LA::NL; q++) sm[yb * TL::RS + LA::slot(q, hb)] = v[q];
         }
         __syncthreads();
-        if (ok && t < NA) {
-            cx<T> v[NB];
+        if (on_y) {
+            cx<T> v[LB::NL];
 #pragma unroll
-            for (int j = 0; j < NB; j++) v[j] = sm[j * TL::RS + t];
-            Dif<T, NB, NB, SIGN>::run(v);
+            for (int i = 0; i < LB::NL; i++) v[i] = sm[LB::nat(i, ha) * TL::RS + xa];
+            LB::template dif<SIGN>(v, ha, my);
 #pragma unroll
-            for (int s = 0; s < NB; s++) f[slot_freq<NB>(s) * NA + t] = v[s];
+            for (int q = 0; q < LB::NL; q++) f[LB::slot(q, ha) * NA + xa] = v[q];
         }
     }
 }
@@ -216,15 +314,27 @@ k_fft_xy(cx<T> *__restrict__ w, int64_t nplanes, const Ctrl *ctrl)
 // g(x) = reunit(1 + (alpha/2) w(x)) (Alg. 1 lines 9-11) straight from shared
 // memory: w never goes back to HBM, rows 0, 1 of g (12 reals) do.  The fused link kernel
 // (kernels_fused.cu) then reads g at x and its 8 neighbours instead of rebuilding it 9 times.
+template <typename T, int NA, int NB> struct XYGCfg {
+    typedef Tile<NA, NB, 1> TL;
+    // threads of one field of one plane; whole warps when lines are split (the halves shuffle)
+    static constexpr int TP = (TL::SA > 1 || TL::SB > 1) ? (TL::THREADS + 31) / 32 * 32 : TL::THREADS;
+    static constexpr int TG = 4 * TP;                         // threads of one plane
+    static constexpr int CTA = cta_threads(TG);
+    static constexpr int G = CTA / TG;
+    static constexpr size_t SMEM = (size_t)G * 4 * TL::ELEMS * sizeof(cx<T>);
+    static constexpr bool FITS = SMEM <= 227 * 1024 && CTA <= 1024;
+};
+
 template <typename T, int NA, int NB>
-__global__ void __launch_bounds__(CTA_THREADS)
+__global__ void __launch_bounds__((XYGCfg<T, NA, NB>::CTA))
 k_fft_xy_inv_g(const cx<T> *__restrict__ w, cx<T> *__restrict__ gbuf, int64_t V, int64_t nplanes, T a, const Ctrl *ctrl)
 {
     if (*(volatile const int *)&ctrl->done) return;
-    typedef Tile<NA, NB, 1> TL;
-    constexpr int TP = TL::THREADS;               // threads of one field of one plane
-    constexpr int TG = 4 * TP;                    // threads of one plane
-    constexpr int G = CTA_THREADS / TG;           // planes per CTA
+    typedef XYGCfg<T, NA, NB> CF;
+    typedef typename CF::TL TL;
+    typedef Line<T, NA, TL::SA> LA;
+    typedef Line<T, NB, TL::SB> LB;
+    constexpr int TP = CF::TP, TG = CF::TG, G = CF::G;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int grp = threadIdx.x / TG, t = threadIdx.x % TG;
     const int fld = t / TP, l = t % TP;
@@ -233,29 +343,34 @@ k_fft_xy_inv_g(const cx<T> *__restrict__ w, cx<T> *__restrict__ gbuf, int64_t V,
     const int64_t plane = (int64_t)blockIdx.x * G + grp;
     const bool ok = plane < nplanes && grp < G;
     const int64_t base = plane * (int64_t)(NA * NB);
+    int xa, ha, yb, hb;
+    line_of_thread<TL::SB>(l, xa, ha);
+    line_of_thread<TL::SA>(l, yb, hb);
+    const bool on_y = ok && xa < NA && l < TL::SB * NA, on_x = ok && yb < NB && l < TL::SA * NB;
+    const unsigned my = __ballot_sync(0xffffffffu, on_y), mx = __ballot_sync(0xffffffffu, on_x);
 
-    if (ok && l < NA) {
+    if (ok) {
         const cx<T> *f = w + (int64_t)fld * V + base;
-#pragma unroll
-        for (int j = 0; j < NB; j++) sm[j * TL::RS + l] = f[j * NA + l];
+#pragma unroll 4
+        for (int e = l; e < NA * NB; e += TP) sm[(e / NA) * TL::RS + (e % NA)] = f[e];
     }
     __syncthreads();
-    if (ok && l < NB) {
-        cx<T> v[NA];
+    if (on_x) {
+        cx<T> v[LA::NL];
 #pragma unroll
-        for (int j = 0; j < NA; j++) v[j] = sm[l * TL::RS + j];
-        Dif<T, NA, NA, +1>::run(v);
+        for (int i = 0; i < LA::NL; i++) v[i] = sm[yb * TL::RS + LA::nat(i, hb)];
+        LA::template dif<+1>(v, hb, mx);
 #pragma unroll
-        for (int s = 0; s < NA; s++) sm[l * TL::RS + slot_freq<NA>(s)] = v[s];
+        for (int q = 0; q < LA::NL; q++) sm[yb * TL::RS + LA::slot(q, hb)] = v[q];
     }
     __syncthreads();
-    if (ok && l < NA) {
-        cx<T> v[NB];
+    if (on_y) {
+        cx<T> v[LB::NL];
 #pragma unroll
-        for (int j = 0; j < NB; j++) v[j] = sm[j * TL::RS + l];
-        Dif<T, NB, NB, +1>::run(v);
+        for (int i = 0; i < LB::NL; i++) v[i] = sm[LB::nat(i, ha) * TL::RS + xa];
+        LB::template dif<+1>(v, ha, my);
 #pragma unroll
-        for (int s = 0; s < NB; s++) sm[slot_freq<NB>(s) * TL::RS + l] = v[s];
+        for (int q = 0; q < LB::NL; q++) sm[LB::slot(q, ha) * TL::RS + xa] = v[q];
     }
     __syncthreads();
     if (ok) {
@@ -277,17 +392,28 @@ k_fft_xy_inv_g(const cx<T> *__restrict__ w, cx<T> *__restrict__ gbuf, int64_t V,
 // shared (thread = (c, kz)): Dif(-), mask, Dit(+) -> shared; z-lines from shared: Dif(+),
 // stored straight to global.  p^2 = sum_mu 4 sin^2(pi k_mu/N_mu) (reading R5) from the
 // per-axis tables; the factor p_max^2/(p^2 V) is one FP64 division per mode.
+template <typename T, int NA, int NB, int C> struct ZTCfg {
+    typedef Tile<NA, NB, C> TL;
+    static constexpr int TT = TL::THREADS;
+    static constexpr int CTA = cta_threads(TT);
+    static constexpr int G = CTA / TT;
+    static constexpr size_t PT = ((NB * sizeof(double) + 15) / 16) * 16;
+    static constexpr size_t SMEM = PT + (size_t)G * TL::ELEMS * sizeof(cx<T>);
+};
+
 template <typename T, int NA, int NB, int C>
-__global__ void __launch_bounds__(CTA_THREADS)
+__global__ void __launch_bounds__((ZTCfg<T, NA, NB, C>::CTA))
 k_fft_zt(cx<T> *__restrict__ w, Geom geo, const double *__restrict__ ptab, double pmax2_over_V, int64_t ntiles, const Ctrl *ctrl)
 {
     if (*(volatile const int *)&ctrl->done) return;
-    typedef Tile<NA, NB, C> TL;
-    constexpr int TT = TL::THREADS;
-    constexpr int G = CTA_THREADS / TT;
+    typedef ZTCfg<T, NA, NB, C> CF;
+    typedef typename CF::TL TL;
+    typedef Line<T, NA, TL::SA> LA;
+    typedef Line<T, NB, TL::SB> LB;
+    constexpr int TT = CF::TT, G = CF::G;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     double *pt = (double *)smem_raw;                                  // 4 sin^2(pi kt/Nt), NB entries
-    cx<T> *sm0 = (cx<T> *)(smem_raw + ((NB * sizeof(double) + 15) / 16) * 16);
+    cx<T> *sm0 = (cx<T> *)(smem_raw + CF::PT);
     const int grp = threadIdx.x / TT, t = threadIdx.x % TT;
     cx<T> *sm = sm0 + (size_t)grp * TL::ELEMS;
     const int64_t tile = (int64_t)blockIdx.x * G + grp;
@@ -301,111 +427,116 @@ k_fft_zt(cx<T> *__restrict__ w, Geom geo, const double *__restrict__ ptab, doubl
     const int x0 = xc * C;
     cx<T> *f = w + fld * geo.V + x0 + (int64_t)Nx * y;
     const int64_t sz = geo.st[2], st = geo.st[3];
-    if (threadIdx.x < NB) pt[threadIdx.x] = ptab[Nx + Ny + NA + threadIdx.x];
-    const int c = t % C, l = t / C;                                    // l = t-index or z-index of the line
+    for (int i = threadIdx.x; i < NB; i += CF::CTA) pt[i] = ptab[Nx + Ny + NA + i];
+    int la, ha, lb, hb;                                                // z-line (c, t) / t-line (c, kz) of this thread
+    line_of_thread<TL::SA>(t, la, ha);
+    line_of_thread<TL::SB>(t, lb, hb);
+    const int ca = la % C, ta = la / C, cb = lb % C, zb = lb / C;
+    const bool on_z = ok && ta < NB && t < TL::SA * C * NB, on_t = ok && zb < NA && t < TL::SB * C * NA;
+    const unsigned mz = __ballot_sync(0xffffffffu, on_z), mt = __ballot_sync(0xffffffffu, on_t);
 
-    if (ok && l < NB) {                                                // z-lines, thread = (c, t = l)
-        cx<T> v[NA];
-        const cx<T> *g = f + c + st * l;
+    if (on_z) {                                                        // z-line at (c, t) = (ca, ta)
+        cx<T> v[LA::NL];
+        const cx<T> *g = f + ca + st * ta;
 #pragma unroll
-        for (int j = 0; j < NA; j++) v[j] = g[sz * j];
-        Dif<T, NA, NA, -1>::run(v);
+        for (int i = 0; i < LA::NL; i++) v[i] = g[sz * LA::nat(i, ha)];
+        LA::template dif<-1>(v, ha, mz);
 #pragma unroll
-        for (int s = 0; s < NA; s++) sm[l * TL::RS + slot_freq<NA>(s) * C + c] = v[s];
+        for (int q = 0; q < LA::NL; q++) sm[ta * TL::RS + LA::slot(q, ha) * C + ca] = v[q];
     }
     __syncthreads();
-    if (ok && l < NA) {                                                // t-lines, thread = (c, kz = l)
-        cx<T> v[NB];
+    if (on_t) {                                                        // t-line at (c, kz) = (cb, zb)
+        cx<T> v[LB::NL];
 #pragma unroll
-        for (int j = 0; j < NB; j++) v[j] = sm[j * TL::RS + l * C + c];
-        Dif<T, NB, NB, -1>::run(v);
-        const double pxyz = ptab[x0 + c] + ptab[Nx + y] + ptab[Nx + Ny + l];
+        for (int i = 0; i < LB::NL; i++) v[i] = sm[LB::nat(i, hb) * TL::RS + zb * C + cb];
+        LB::template dif<-1>(v, hb, mt);
+        const double pxyz = ptab[x0 + cb] + ptab[Nx + y] + ptab[Nx + Ny + zb];
 #pragma unroll
-        for (int s = 0; s < NB; s++) {
-            const double p2 = pxyz + pt[slot_freq<NB>(s)];
+        for (int q = 0; q < LB::NL; q++) {
+            const double p2 = pxyz + pt[LB::slot(q, hb)];
             const T fac = (p2 > 0.0) ? (T)(pmax2_over_V / p2) : (T)0;  // zero mode -> 0 (reading R7)
-            v[s] = cscale(v[s], fac);
+            v[q] = cscale(v[q], fac);
         }
-        Dit<T, NB, NB, +1>::run(v);
+        LB::template dit<+1>(v, hb, mt);
 #pragma unroll
-        for (int j = 0; j < NB; j++) sm[j * TL::RS + l * C + c] = v[j];
+        for (int i = 0; i < LB::NL; i++) sm[LB::nat(i, hb) * TL::RS + zb * C + cb] = v[i];
     }
     __syncthreads();
-    if (ok && l < NB) {
-        cx<T> v[NA];
+    if (on_z) {
+        cx<T> v[LA::NL];
 #pragma unroll
-        for (int j = 0; j < NA; j++) v[j] = sm[l * TL::RS + j * C + c];
-        Dif<T, NA, NA, +1>::run(v);
-        cx<T> *g = f + c + st * l;
+        for (int i = 0; i < LA::NL; i++) v[i] = sm[ta * TL::RS + LA::nat(i, ha) * C + ca];
+        LA::template dif<+1>(v, ha, mz);
+        cx<T> *g = f + ca + st * ta;
 #pragma unroll
-        for (int s = 0; s < NA; s++) g[sz * slot_freq<NA>(s)] = v[s];
+        for (int q = 0; q < LA::NL; q++) g[sz * LA::slot(q, ha)] = v[q];
     }
 }
 
 // ---------------------------------------------------------------- dispatch
-template <typename T, int NA, int NB> struct XYCfg {
-    typedef Tile<NA, NB, 1> TL;
-    static constexpr int G = CTA_THREADS / TL::THREADS;
-    static constexpr size_t SMEM = (size_t)G * TL::ELEMS * sizeof(cx<T>);
-};
-template <typename T, int NA, int NB> struct XYGCfg {
-    typedef Tile<NA, NB, 1> TL;
-    static constexpr int G = CTA_THREADS / (4 * TL::THREADS);
-    static constexpr size_t SMEM = (size_t)G * 4 * TL::ELEMS * sizeof(cx<T>);
-};
-template <typename T, int NA, int NB, int C> struct ZTCfg {
-    typedef Tile<NA, NB, C> TL;
-    static constexpr int G = CTA_THREADS / TL::THREADS;
-    static constexpr size_t SMEM = ((NB * sizeof(double) + 15) / 16) * 16 + (size_t)G * TL::ELEMS * sizeof(cx<T>);
-};
+// x-columns per (z,t) tile: 64-byte runs in global memory (FP64), unless the tile would not fit
+template <typename T, int N> struct ZTC { static constexpr int C = (sizeof(cx<T>) == 16 && N == 64) ? 2 : 4; };
 
-static const int ZT_C = 4; // x-columns per (z,t) tile: 64-byte (FP64) runs in global memory
-
-template <typename T, int N> static int setup_n()
+template <typename T, int N> static int setup_xy_n()
 {
     cudaError_t e;
     e = cudaFuncSetAttribute(k_fft_xy<T, N, N, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)XYCfg<T, N, N>::SMEM);
     if (e != cudaSuccess) return 1;
     e = cudaFuncSetAttribute(k_fft_xy<T, N, N, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)XYCfg<T, N, N>::SMEM);
     if (e != cudaSuccess) return 1;
-    e = cudaFuncSetAttribute(k_fft_xy_inv_g<T, N, N>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)XYGCfg<T, N, N>::SMEM);
-    if (e != cudaSuccess) return 1;
-    e = cudaFuncSetAttribute(k_fft_zt<T, N, N, ZT_C>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ZTCfg<T, N, N, ZT_C>::SMEM);
-    if (e != cudaSuccess) return 1;
+    if (XYGCfg<T, N, N>::FITS) {
+        e = cudaFuncSetAttribute(k_fft_xy_inv_g<T, N, N>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)XYGCfg<T, N, N>::SMEM);
+        if (e != cudaSuccess) return 1;
+    }
     return 0;
 }
 
-template <typename T, int N> static void launch_n(const FftArgs &a, int which, cudaStream_t st)
+template <typename T, int N> static int setup_zt_n()
 {
-    if (which == 1) {
-        typedef ZTCfg<T, N, N, ZT_C> Z;
-        const int64_t ntiles = (int64_t)a.nfields * a.geo.N[1] * (a.geo.N[0] / ZT_C);
-        const unsigned grid = (unsigned)((ntiles + Z::G - 1) / Z::G);
-        k_fft_zt<T, N, N, ZT_C><<<grid, CTA_THREADS, Z::SMEM, st>>>((cx<T> *)a.w, a.geo, a.ptab, a.pmax2 / (double)a.geo.V, ntiles, a.ctrl);
-    } else {
-        typedef XYCfg<T, N, N> X;
-        const int64_t nplanes = (int64_t)a.nfields * a.geo.N[2] * a.geo.N[3];
-        const unsigned grid = (unsigned)((nplanes + X::G - 1) / X::G);
-        if (which == 0) k_fft_xy<T, N, N, 0><<<grid, CTA_THREADS, X::SMEM, st>>>((cx<T> *)a.w, nplanes, a.ctrl);
-        else k_fft_xy<T, N, N, 1><<<grid, CTA_THREADS, X::SMEM, st>>>((cx<T> *)a.w, nplanes, a.ctrl);
-    }
+    typedef ZTCfg<T, N, N, ZTC<T, N>::C> Z;
+    cudaError_t e = cudaFuncSetAttribute(k_fft_zt<T, N, N, ZTC<T, N>::C>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Z::SMEM);
+    return e == cudaSuccess ? 0 : 1;
 }
 
-template <typename T, int N> static void launch_inv_g_n(const FftArgs &a, void *gbuf, double alpha, cudaStream_t st)
+template <typename T, int N> static int launch_zt_n(const FftArgs &a, cudaStream_t st)
+{
+    constexpr int C = ZTC<T, N>::C;
+    typedef ZTCfg<T, N, N, C> Z;
+    const int64_t ntiles = (int64_t)a.nfields * a.geo.N[1] * (a.geo.N[0] / C);
+    const unsigned grid = (unsigned)((ntiles + Z::G - 1) / Z::G);
+    k_fft_zt<T, N, N, C><<<grid, Z::CTA, Z::SMEM, st>>>((cx<T> *)a.w, a.geo, a.ptab, a.pmax2 / (double)a.geo.V, ntiles, a.ctrl);
+    return 0;
+}
+
+template <typename T, int N> static int launch_xy_n(const FftArgs &a, int which, cudaStream_t st)
+{
+    typedef XYCfg<T, N, N> X;
+    const int64_t nplanes = (int64_t)a.nfields * a.geo.N[2] * a.geo.N[3];
+    const unsigned grid = (unsigned)((nplanes + X::G - 1) / X::G);
+    if (which == 0) k_fft_xy<T, N, N, 0><<<grid, X::CTA, X::SMEM, st>>>((cx<T> *)a.w, nplanes, a.ctrl);
+    else k_fft_xy<T, N, N, 1><<<grid, X::CTA, X::SMEM, st>>>((cx<T> *)a.w, nplanes, a.ctrl);
+    return 0;
+}
+
+template <typename T, int N> static int launch_inv_g_n(const FftArgs &a, void *gbuf, double alpha, cudaStream_t st)
 {
     typedef XYGCfg<T, N, N> X;
     const int64_t nplanes = (int64_t)a.geo.N[2] * a.geo.N[3];
     const unsigned grid = (unsigned)((nplanes + X::G - 1) / X::G);
-    k_fft_xy_inv_g<T, N, N><<<grid, CTA_THREADS, X::SMEM, st>>>((const cx<T> *)a.w, (cx<T> *)gbuf, a.geo.V, nplanes, (T)(alpha / 2.0), a.ctrl);
+    k_fft_xy_inv_g<T, N, N><<<grid, X::CTA, X::SMEM, st>>>((const cx<T> *)a.w, (cx<T> *)gbuf, a.geo.V, nplanes, (T)(alpha / 2.0), a.ctrl);
+    return 0;
 }
 
-// Hypercubic N^4 lattices whose lines fit in registers: N = 8, 16, 32 in both precisions,
-// N = 12, 24 (radix 3 x 2^a).  Everything else takes the generic path.
+template <typename T, int N> static int gbuf_fits_n() { return XYGCfg<T, N, N>::FITS ? 1 : 0; }
+
+// Lattices Nx = Ny, Nz = Nt with both extents in {8, 12, 16, 24, 32, 48, 64}: the (x,y) passes
+// are instantiated per Nx and the (z,t) pass per Nz (x-columns per tile must divide Nx: 2 or 4).
+// Everything else takes the generic path.
+static bool tiled_extent(int n) { return n == 8 || n == 16 || n == 32 || n == 64 || n == 12 || n == 24 || n == 48; }
 bool fft_tiled_supported(const int N[4], int prec)
 {
     (void)prec;
-    if (!(N[0] == N[1] && N[1] == N[2] && N[2] == N[3])) return false;
-    return N[0] == 8 || N[0] == 16 || N[0] == 32 || N[0] == 12 || N[0] == 24;
+    return N[0] == N[1] && N[2] == N[3] && tiled_extent(N[0]) && tiled_extent(N[2]);
 }
 
 #define LGF_FFT_SWITCH(FN, ...)                                         \
@@ -415,27 +546,56 @@ bool fft_tiled_supported(const int N[4], int prec)
     case 16: return prec == 0 ? FN<double, 16>(__VA_ARGS__) : FN<float, 16>(__VA_ARGS__); \
     case 24: return prec == 0 ? FN<double, 24>(__VA_ARGS__) : FN<float, 24>(__VA_ARGS__); \
     case 32: return prec == 0 ? FN<double, 32>(__VA_ARGS__) : FN<float, 32>(__VA_ARGS__); \
+    case 48: return prec == 0 ? FN<double, 48>(__VA_ARGS__) : FN<float, 48>(__VA_ARGS__); \
+    case 64: return prec == 0 ? FN<double, 64>(__VA_ARGS__) : FN<float, 64>(__VA_ARGS__); \
     default: break;                                                     \
     }
 
-int fft_tiled_setup(const int N[4], int prec)
+static int setup_xy(int n, int prec)
 {
-    const int n = N[0];
-    LGF_FFT_SWITCH(setup_n)
+    LGF_FFT_SWITCH(setup_xy_n)
     return 1;
 }
+static int setup_zt(int n, int prec)
+{
+    LGF_FFT_SWITCH(setup_zt_n)
+    return 1;
+}
+int fft_tiled_setup(const int N[4], int prec) { return setup_xy(N[0], prec) | setup_zt(N[2], prec); }
 
-void launch_fft_tiled(const FftArgs &a, int which, cudaStream_t st)
+// does the plane of 4 packed fields fit in shared memory (pass 2 with the g build fused)?
+bool fft_tiled_gbuf_supported(const int N[4], int prec)
+{
+    if (!fft_tiled_supported(N, prec)) return false;
+    const int n = N[0];
+    LGF_FFT_SWITCH(gbuf_fits_n)
+    return false;
+}
+
+static int run_xy(const FftArgs &a, int which, cudaStream_t st)
 {
     const int n = a.geo.N[0], prec = a.prec;
-    LGF_FFT_SWITCH(launch_n, a, which, st)
+    LGF_FFT_SWITCH(launch_xy_n, a, which, st)
+    return 1;
+}
+static int run_zt(const FftArgs &a, cudaStream_t st)
+{
+    const int n = a.geo.N[2], prec = a.prec;
+    LGF_FFT_SWITCH(launch_zt_n, a, st)
+    return 1;
+}
+void launch_fft_tiled(const FftArgs &a, int which, cudaStream_t st)
+{
+    if (which == 1) run_zt(a, st); else run_xy(a, which, st);
 }
 
 // pass 2 fused with the g build: needs the 4 packed fields (nfields == 4)
-void launch_fft_tiled_inv_g(const FftArgs &a, void *gbuf, double alpha, cudaStream_t st)
+static int run_inv_g(const FftArgs &a, void *gbuf, double alpha, cudaStream_t st)
 {
     const int n = a.geo.N[0], prec = a.prec;
     LGF_FFT_SWITCH(launch_inv_g_n, a, gbuf, alpha, st)
+    return 1;
 }
+void launch_fft_tiled_inv_g(const FftArgs &a, void *gbuf, double alpha, cudaStream_t st) { run_inv_g(a, gbuf, alpha, st); }
 
 } // namespace lgf

@@ -51,6 +51,7 @@ struct FftArgs {
 int launch_fft_generic(const FftArgs &a, cudaStream_t st);
 // tiled register FFT: three passes.  which = 0 (x,y) forward, 1 (z,t) forward*mask*inverse, 2 (x,y) inverse
 bool fft_tiled_supported(const int N[4], int prec);
+bool fft_tiled_gbuf_supported(const int N[4], int prec); // pass 2 with the g build fits in shared memory
 void launch_fft_tiled(const FftArgs &a, int which, cudaStream_t st);
 // pass 2 of all 4 packed fields with g(x) = reunit(1 + (alpha/2) w(x)) as its epilogue: rows 0, 1 of g -> gbuf
 void launch_fft_tiled_inv_g(const FftArgs &a, void *gbuf, double alpha, cudaStream_t st);

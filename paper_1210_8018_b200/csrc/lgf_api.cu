@@ -73,7 +73,7 @@ Layout make_layout(const lgf_ctx *c)
     // are written); the fields are double-buffered when g is rebuilt from w inside that kernel,
     // else the last FFT pass writes rows 0, 1 of g (6 complex per site) to gbuf
     const int nl = c->fusion ? 2 : 1;
-    const bool gb = c->fusion && c->pack == 4 && c->fft_path == 0 && fft_tiled_supported(c->N, c->prec);
+    const bool gb = c->fusion && c->pack == 4 && c->fft_path == 0 && fft_tiled_gbuf_supported(c->N, c->prec);
     const int nw = (c->fusion && !gb) ? 2 : 1;
     for (int i = 0; i < 2; i++) { L.links[i] = off; if (i < nl) off = align_up(off + (size_t)4 * ne * c->V * e, 256); }
     for (int i = 0; i < 2; i++) { L.w[i] = off; if (i < nw) off = align_up(off + (size_t)c->pack * c->V * e, 256); }
@@ -367,7 +367,7 @@ int lgf_bind(lgf_ctx *ctx, void *dev_workspace, size_t bytes, void *cuda_stream)
         cudaError_t e = cudaGetLastError();
         return cuda_fail(ctx, e, "fft_tiled_setup");
     }
-    ctx->use_gbuf = ctx->fusion && ctx->tiled && ctx->pack == 4;
+    ctx->use_gbuf = ctx->fusion && ctx->tiled && ctx->pack == 4 && fft_tiled_gbuf_supported(ctx->N, ctx->prec);
     ctx->bound = true;
     ctx->loaded = false;
     ctx->wstate = 0;

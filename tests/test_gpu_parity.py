@@ -234,10 +234,56 @@ def test_fp32_variant(lgf, lat, var):
 
 
 def test_tiled_fft_is_taken_where_expected(lgf):
-    for n, want in [(8, True), (12, True), (16, True), (24, True), (32, True), ((8, 8, 8, 16), False), (4, False), (48, False)]:
+    for n, want in [(8, True), (12, True), (16, True), (24, True), (32, True), (48, True), (64, True), ((16, 16, 8, 8), True),
+                    ((8, 8, 8, 16), False), ((8, 16, 8, 8), False), (4, False), (36, False)]:
         gf = fixer(lgf, n)
         assert gf.uses_tiled_fft() == want, n
     assert not fixer(lgf, 16, fft_path=1).uses_tiled_fft()
+
+
+# Lines of 48 and 64 are shared by two threads (fft_tiled.cu, Line<T, N, 2>); lattices with
+# Nx = Ny != Nz = Nt put them in the (x,y) passes or in the (z,t) pass at a size the oracle
+# finishes in about a second.
+SPLIT_LATTICES = [((64, 64, 8, 8), 81), ((8, 8, 64, 64), 82), ((48, 48, 12, 12), 83), ((16, 16, 48, 48), 84)]
+
+
+@pytest.mark.parametrize("lat", SPLIT_LATTICES, ids=lambda v: "x".join(map(str, v[0])))
+@pytest.mark.parametrize("fft_batch", [4, 9])
+def test_split_line_fourier_matches_oracle(lgf, lat, fft_batch):
+    N, seed = lat
+    U = gen.gen_links(N, 0.5, seed)
+    D, _, _ = oracle.measure(N, U)
+    w = oracle.fourier_accelerate(N, D)
+    for prec, tol in (("fp64", 2e-13), ("fp32", 2e-5)):
+        gf = fixer(lgf, N, precision=prec, fft_batch=fft_batch)
+        assert gf.uses_tiled_fft()
+        gf.load_links(U if prec == "fp64" else U.astype(np.complex64))
+        gf.set_field(lgf.FIELD_DELTA, D if prec == "fp64" else D.astype(np.complex64))
+        gf.stage(lgf.STAGE_FOURIER)
+        w2 = gf.get_field(lgf.FIELD_W).astype(np.complex128)
+        assert np.abs(w2 - w).max() < tol * np.abs(w).max()
+
+
+@pytest.mark.parametrize("lat", SPLIT_LATTICES, ids=lambda v: "x".join(map(str, v[0])))
+def test_split_line_one_iteration(lgf, lat):
+    N, seed = lat
+    U = gen.gen_links(N, 0.5, seed)
+    Uo = U.copy()
+    hist = oracle.iterate(N, Uo, ALPHA, 1)
+    for prec, recon, tol in (("fp64", 12, 1e-12), ("fp64", 18, 1e-12), ("fp32", 18, 1e-5)):
+        gf = fixer(lgf, N, precision=prec, recon=recon)
+        gf.load_links(U if prec == "fp64" else U.astype(np.complex64))
+        r = gf.iterate(ALPHA, 1)
+        assert np.abs(gf.get_links().astype(np.complex128) - Uo).max() < tol
+        assert abs(r.theta - hist[1, 1]) <= (1e-10 if prec == "fp64" else 1e-4) * hist[1, 1]
+        r = gf.iterate(ALPHA, 2)                       # three fused iterations stay on the oracle's trajectory
+    Uo3 = U.copy()
+    hist3 = oracle.iterate(N, Uo3, ALPHA, 3)
+    gf = fixer(lgf, N, recon=12)
+    gf.load_links(U)
+    r = gf.iterate(ALPHA, 3)
+    assert np.abs(gf.get_links() - Uo3).max() < 1e-12
+    assert abs(r.F - hist3[3, 0]) <= 1e-10 * abs(hist3[3, 0]) and abs(r.theta - hist3[3, 1]) <= 1e-10 * hist3[3, 1]
 
 
 def test_24_one_iteration(lgf):
