@@ -38,13 +38,12 @@ WORKLOADS = {
 }
 
 
-def algorithmic_bytes(recon, nfields, real_bytes, tiled, fusion):
+def algorithmic_bytes(recon, nfields, real_bytes, tiled, fusion, gbuf):
     """Bytes per site each kernel must move once:
     L = link bytes per site, W = field bytes per site, Gb = bytes of rows 0, 1 of g per site."""
     L = 4 * recon * real_bytes
     W = nfields * 2 * real_bytes
     Gb = 12 * real_bytes
-    gbuf = fusion and tiled and nfields == 4
     per = {}
     if fusion:
         per["update_measure"] = (Gb if gbuf else W) + 2 * L + W
@@ -267,7 +266,7 @@ def run_ours(args):
 
     real_bytes = 8 if prec == "fp64" else 4
     tiled = gf.uses_tiled_fft()
-    per = algorithmic_bytes(recon, args.fft_batch, real_bytes, tiled, args.fusion)
+    per = algorithmic_bytes(recon, args.fft_batch, real_bytes, tiled, args.fusion, gf.uses_gbuf())
     peak, peak_src = peaks()
     kern = {k: {"ms_total": v[0], "launches": v[1], "us_per_launch": 1e3 * v[0] / v[1]}
             for k, v in ktimes.items() if v[1] and k in per}

@@ -169,6 +169,10 @@ int lgf_reset_counters(lgf_ctx *ctx);
 
 /* 1 if this context takes the tiled register-FFT path, 0 if the generic one. */
 int lgf_uses_tiled_fft(const lgf_ctx *ctx);
+/* 1 if the last FFT pass builds g(x) in its epilogue (fused path, 4 packed fields, plane fits in
+ * shared memory of one SM or of a 2-CTA cluster), 0 if g is rebuilt from w by the link kernel.
+ * Valid after lgf_bind. */
+int lgf_uses_gbuf(const lgf_ctx *ctx);
 
 /* Text of the last error of this context (or of lgf_create when ctx == NULL). Never NULL. */
 const char *lgf_last_error(const lgf_ctx *ctx);

@@ -21,6 +21,7 @@
 #include "launch.h"
 #include "twiddles.cuh"
 #include "su3.cuh"
+#include <cooperative_groups.h>
 
 namespace lgf {
 
@@ -386,6 +387,81 @@ k_fft_xy_inv_g(const cx<T> *__restrict__ w, cx<T> *__restrict__ gbuf, int64_t V,
     }
 }
 
+// The same pass for planes whose four fields do not fit one SM's shared memory (64^2 in FP64:
+// 266 KB): a thread-block CLUSTER of two CTAs holds the plane, two fields each; after the
+// transforms each CTA builds g for half of the sites, reading its own two fields locally and
+// the other two from the peer's shared memory (DSMEM).
+template <typename T, int NA, int NB> struct XYG2Cfg {
+    typedef Tile<NA, NB, 1> TL;
+    static constexpr int TP = (TL::SA > 1 || TL::SB > 1) ? (TL::THREADS + 31) / 32 * 32 : TL::THREADS;
+    static constexpr int CTA = 2 * TP;                        // two fields per CTA
+    static constexpr size_t SMEM = (size_t)2 * TL::ELEMS * sizeof(cx<T>);
+    static constexpr bool FITS = SMEM <= 227 * 1024 && CTA <= 1024 && CTA >= 64;
+};
+
+template <typename T, int NA, int NB>
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__((XYG2Cfg<T, NA, NB>::CTA))
+k_fft_xy_inv_g2(const cx<T> *__restrict__ w, cx<T> *__restrict__ gbuf, int64_t V, T a, const Ctrl *ctrl)
+{
+    namespace cg = cooperative_groups;
+    if (*(volatile const int *)&ctrl->done) return;          // uniform over the grid: both CTAs of a cluster leave
+    typedef XYG2Cfg<T, NA, NB> CF;
+    typedef typename CF::TL TL;
+    typedef Line<T, NA, TL::SA> LA;
+    typedef Line<T, NB, TL::SB> LB;
+    constexpr int TP = CF::TP;
+    cg::cluster_group cluster = cg::this_cluster();
+    const int rank = (int)cluster.block_rank();              // 0: fields 0, 1;  1: fields 2, 3
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    cx<T> *smp = (cx<T> *)smem_raw;
+    const int t = threadIdx.x, lf = t / TP, l = t % TP;
+    cx<T> *sm = smp + (size_t)lf * TL::ELEMS;
+    const int64_t plane = blockIdx.x >> 1;
+    const int64_t base = plane * (int64_t)(NA * NB);
+    int xa, ha, yb, hb;
+    line_of_thread<TL::SB>(l, xa, ha);
+    line_of_thread<TL::SA>(l, yb, hb);
+    const bool on_y = xa < NA && l < TL::SB * NA, on_x = yb < NB && l < TL::SA * NB;
+    const unsigned my = __ballot_sync(0xffffffffu, on_y), mx = __ballot_sync(0xffffffffu, on_x);
+    {
+        const cx<T> *f = w + (int64_t)(2 * rank + lf) * V + base;
+#pragma unroll 4
+        for (int e = l; e < NA * NB; e += TP) sm[(e / NA) * TL::RS + (e % NA)] = f[e];
+    }
+    __syncthreads();
+    if (on_x) {
+        cx<T> v[LA::NL];
+#pragma unroll
+        for (int i = 0; i < LA::NL; i++) v[i] = sm[yb * TL::RS + LA::nat(i, hb)];
+        LA::template dif<+1>(v, hb, mx);
+#pragma unroll
+        for (int q = 0; q < LA::NL; q++) sm[yb * TL::RS + LA::slot(q, hb)] = v[q];
+    }
+    __syncthreads();
+    if (on_y) {
+        cx<T> v[LB::NL];
+#pragma unroll
+        for (int i = 0; i < LB::NL; i++) v[i] = sm[LB::nat(i, ha) * TL::RS + xa];
+        LB::template dif<+1>(v, ha, my);
+#pragma unroll
+        for (int q = 0; q < LB::NL; q++) sm[LB::slot(q, ha) * TL::RS + xa] = v[q];
+    }
+    cluster.sync();                                          // all four fields of the plane are in place
+    const cx<T> *peer = cluster.map_shared_rank(smp, rank ^ 1);
+    const cx<T> *f01 = rank == 0 ? smp : peer, *f23 = rank == 0 ? peer : smp;
+    constexpr int HALF = NA * NB / 2;
+    for (int i = rank * HALF + t; i < (rank + 1) * HALF; i += CF::CTA) {
+        const int o = (i / NA) * TL::RS + (i % NA);
+        cx<T> g[9];
+        m_from_packed<T>(f01[o], f01[TL::ELEMS + o], f23[o], f23[TL::ELEMS + o], a, g);
+        reunit01<T>(g);
+        cx<T> *dst = gbuf + base + i;
+#pragma unroll
+        for (int k = 0; k < 6; k++) dst[(int64_t)k * V] = g[k];
+    }
+    cluster.sync();                                          // the peer may still be reading this CTA's fields
+}
+
 // ---------------------------------------------------------------- pass 1: (z,t) tiles
 // Tile = C consecutive x at fixed (field, y): element (c, z, t) at global x0 + c + sz*z + st*t.
 // z-lines straight from global (thread = (c, t)), Dif(-) along z -> shared; t-lines from
@@ -487,6 +563,9 @@ template <typename T, int N> static int setup_xy_n()
     if (XYGCfg<T, N, N>::FITS) {
         e = cudaFuncSetAttribute(k_fft_xy_inv_g<T, N, N>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)XYGCfg<T, N, N>::SMEM);
         if (e != cudaSuccess) return 1;
+    } else if (XYG2Cfg<T, N, N>::FITS) {
+        e = cudaFuncSetAttribute(k_fft_xy_inv_g2<T, N, N>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)XYG2Cfg<T, N, N>::SMEM);
+        if (e != cudaSuccess) return 1;
     }
     return 0;
 }
@@ -520,14 +599,19 @@ template <typename T, int N> static int launch_xy_n(const FftArgs &a, int which,
 
 template <typename T, int N> static int launch_inv_g_n(const FftArgs &a, void *gbuf, double alpha, cudaStream_t st)
 {
-    typedef XYGCfg<T, N, N> X;
     const int64_t nplanes = (int64_t)a.geo.N[2] * a.geo.N[3];
-    const unsigned grid = (unsigned)((nplanes + X::G - 1) / X::G);
-    k_fft_xy_inv_g<T, N, N><<<grid, X::CTA, X::SMEM, st>>>((const cx<T> *)a.w, (cx<T> *)gbuf, a.geo.V, nplanes, (T)(alpha / 2.0), a.ctrl);
+    if (XYGCfg<T, N, N>::FITS) {
+        typedef XYGCfg<T, N, N> X;
+        const unsigned grid = (unsigned)((nplanes + X::G - 1) / X::G);
+        k_fft_xy_inv_g<T, N, N><<<grid, X::CTA, X::SMEM, st>>>((const cx<T> *)a.w, (cx<T> *)gbuf, a.geo.V, nplanes, (T)(alpha / 2.0), a.ctrl);
+    } else {
+        typedef XYG2Cfg<T, N, N> X;                           // one cluster of two CTAs per plane
+        k_fft_xy_inv_g2<T, N, N><<<(unsigned)(2 * nplanes), X::CTA, X::SMEM, st>>>((const cx<T> *)a.w, (cx<T> *)gbuf, a.geo.V, (T)(alpha / 2.0), a.ctrl);
+    }
     return 0;
 }
 
-template <typename T, int N> static int gbuf_fits_n() { return XYGCfg<T, N, N>::FITS ? 1 : 0; }
+template <typename T, int N> static int gbuf_fits_n() { return (XYGCfg<T, N, N>::FITS || XYG2Cfg<T, N, N>::FITS) ? 1 : 0; }
 
 // Lattices Nx = Ny, Nz = Nt with both extents in {8, 12, 16, 24, 32, 48, 64}: the (x,y) passes
 // are instantiated per Nx and the (z,t) pass per Nz (x-columns per tile must divide Nx: 2 or 4).

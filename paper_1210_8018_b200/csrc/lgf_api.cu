@@ -599,6 +599,7 @@ int lgf_reset_counters(lgf_ctx *ctx)
 }
 
 int lgf_uses_tiled_fft(const lgf_ctx *ctx) { return ctx && ctx->tiled ? 1 : 0; }
+int lgf_uses_gbuf(const lgf_ctx *ctx) { return ctx && ctx->bound && ctx->use_gbuf ? 1 : 0; }
 
 const char *lgf_last_error(const lgf_ctx *ctx) { return ctx ? ctx->err.c_str() : g_create_err.c_str(); }
 

@@ -28,7 +28,7 @@ KERNEL_NAMES = ["measure", "fft_xy_fwd", "fft_zt", "fft_xy_inv", "update", "fft_
 SYMBOLS = [
     "lgf_create", "lgf_set_option", "lgf_workspace_bytes", "lgf_bind", "lgf_load_links", "lgf_get_links",
     "lgf_measure", "lgf_iterate", "lgf_fix", "lgf_stage", "lgf_get_field", "lgf_set_field", "lgf_history",
-    "lgf_kernel_time", "lgf_launch_count", "lgf_reset_counters", "lgf_uses_tiled_fft", "lgf_last_error",
+    "lgf_kernel_time", "lgf_launch_count", "lgf_reset_counters", "lgf_uses_tiled_fft", "lgf_uses_gbuf", "lgf_last_error",
     "lgf_destroy",
 ]
 
@@ -78,6 +78,7 @@ def lib():
     L.lgf_launch_count.restype = i64
     L.lgf_reset_counters.argtypes = [vp]
     L.lgf_uses_tiled_fft.argtypes = [vp]
+    L.lgf_uses_gbuf.argtypes = [vp]
     L.lgf_last_error.argtypes = [vp]
     L.lgf_last_error.restype = ctypes.c_char_p
     L.lgf_destroy.argtypes = [vp]
@@ -244,6 +245,9 @@ class GaugeFixer:
 
     def uses_tiled_fft(self):
         return bool(self.L.lgf_uses_tiled_fft(self.ctx))
+
+    def uses_gbuf(self):
+        return bool(self.L.lgf_uses_gbuf(self.ctx))
 
     def synchronize(self):
         self.stream.synchronize()
