@@ -6,9 +6,10 @@
 // The paper runs these as two kernels (k6, then k2 of the next iteration: Table 1,
 // PAPER.md:146-150), so every link crosses the memory bus three times per iteration; here it
 // crosses twice.  The thread of site x also needs the four NEW backward links
-// U'_nu(x-nu) = g(x-nu) U_nu(x-nu) g^dagger(x); it recomputes them from the OLD links (served
-// by L2, they were or will be streamed by the thread of x-nu) instead of waiting for a grid-wide
-// barrier.  That is why the links are double-buffered: `lin` is read-only, `lout` write-only.
+// U'_nu(x-nu) = g(x-nu) U_nu(x-nu) g^dagger(x); it recomputes what it needs of them from the OLD
+// links (served by L2, they were or will be streamed by the thread of x-nu) instead of waiting
+// for a grid-wide barrier.  That is why the links are double-buffered: `lin` is read-only,
+// `lout` write-only.
 // g comes from the g buffer written by the last FFT pass (GBUF) or is rebuilt from w.
 #include "launch.h"
 #include "su3.cuh"
@@ -53,45 +54,56 @@ k_update_measure(const cx<T> *__restrict__ lin, cx<T> *__restrict__ lout, const 
     if (*(volatile int *)&ctrl->done) return;
     const int64_t V = geo.V;
     const int64_t s = (int64_t)blockIdx.x * FUSED_THREADS + threadIdx.x;
-    constexpr int R = (NE == 6) ? 2 : 3;
     double trF = 0, th = 0;
     if (s < V) {
         int c[4];
         site_coords(geo, s, c);
+        // Backward links first: only their sum enters A'(x),
+        //     sum_nu U'_nu(x-nu) = [sum_nu H_nu(x-nu)] g^dagger(x),   H_nu(y) = g(y) U_nu(y),
+        // so rows 0, 1 of each H are one product, row 2 is conj(row0 x row1) (H is special
+        // unitary) and g^dagger(x) is applied once to the sum.
+        cx<T> X[9];
+#pragma unroll
+        for (int k = 0; k < 9; k++) X[k] = mk<T>(0, 0);
+#pragma unroll
+        for (int nu = 0; nu < 4; nu++) {
+            const int64_t sb = s + (c[nu] == 0 ? (int64_t)(geo.N[nu] - 1) : (int64_t)-1) * geo.st[nu];
+            cx<T> gb[9], u[9], h[9];
+            load_g01<T, PACK, GBUF>(gsrc, V, sb, a, gb);
+            load_link_in<T, NE>(lin, V, nu, sb, u);
+            mul_rows<2>(gb, u, h);
+            su3_row2(h);
+#pragma unroll
+            for (int k = 0; k < 9; k++) X[k] = X[k] + h[k];
+        }
         cx<T> g0[9];
         load_g01<T, PACK, GBUF>(gsrc, V, s, a, g0);
         su3_row2(g0);
         T di[3] = {0, 0, 0};
         cx<T> E[3] = {mk<T>(0, 0), mk<T>(0, 0), mk<T>(0, 0)};
+        {
+            cx<T> B[9];
+            mul_rows_dag<3>(X, g0, B);
+            acc_ah<T>(B, (T)1, di, E);
+        }
+        // Forward links U'_mu(x) = g(x) U_mu(x) g^dagger(x+mu): rows 0, 1 computed and stored; row 2 is
+        // conj(row0 x row1), which is also what a later load of 12-real storage rebuilds (R15).
         T tr = 0;
 #pragma unroll
         for (int mu = 0; mu < 4; mu++) {
             const int64_t sp = s + (c[mu] == geo.N[mu] - 1 ? -(int64_t)(geo.N[mu] - 1) : (int64_t)1) * geo.st[mu];
-            const int64_t sb = s + (c[mu] == 0 ? (int64_t)(geo.N[mu] - 1) : (int64_t)-1) * geo.st[mu];
-            {   // U'_mu(x) = g(x) U_mu(x) g^dagger(x+mu): stored
-                cx<T> g1[9], u[9], t[9], r[9];
-                load_g01<T, PACK, GBUF>(gsrc, V, sp, a, g1);
-                su3_row2(g1);
-                load_link_in<T, NE>(lin, V, mu, s, u);
-                mul_rows<R>(g0, u, t);
-                mul_rows_dag<R>(t, g1, r);
-                cx<T> *p = lout + (int64_t)mu * NE * V + s;
+            cx<T> g1[9], u[9], t[9], r[9];
+            load_g01<T, PACK, GBUF>(gsrc, V, sp, a, g1);
+            su3_row2(g1);
+            load_link_in<T, NE>(lin, V, mu, s, u);
+            mul_rows<2>(g0, u, t);
+            mul_rows_dag<2>(t, g1, r);
+            su3_row2(r);
+            cx<T> *p = lout + (int64_t)mu * NE * V + s;
 #pragma unroll
-                for (int k = 0; k < NE; k++) st_link(p + (int64_t)k * V, r[k]);
-                if (NE == 6) su3_row2(r);          // what a later load of the stored rows rebuilds (R15)
-                tr += r[0].x + r[4].x + r[8].x;
-                acc_ah<T>(r, (T)-1, di, E);
-            }
-            {   // U'_mu(x-mu) = g(x-mu) U_mu(x-mu) g^dagger(x): only its contribution to A'(x)
-                cx<T> gb[9], u[9], t[9], r[9];
-                load_g01<T, PACK, GBUF>(gsrc, V, sb, a, gb);
-                if (NE == 9) su3_row2(gb);
-                load_link_in<T, NE>(lin, V, mu, sb, u);
-                mul_rows<R>(gb, u, t);
-                mul_rows_dag<R>(t, g0, r);
-                if (NE == 6) su3_row2(r);
-                acc_ah<T>(r, (T)1, di, E);
-            }
+            for (int k = 0; k < NE; k++) st_link(p + (int64_t)k * V, r[k]);
+            tr += r[0].x + r[4].x + r[8].x;
+            acc_ah<T>(r, (T)-1, di, E);
         }
         trF = (double)tr;
         T d0 = 2 * di[0], d1 = 2 * di[1], d2 = 2 * di[2];
