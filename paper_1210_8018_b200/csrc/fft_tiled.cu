@@ -209,7 +209,10 @@ template <int S> __device__ __forceinline__ void line_of_thread(int t, int &line
     if (S == 1) { line = t; h = 0; }
     else { h = (t >> 4) & 1; line = (t & 15) | ((t >> 5) << 4); }
 }
-constexpr int split_of(int n) { return n >= 48 ? 2 : 1; }
+#ifndef LGF_SPLIT_MIN
+#define LGF_SPLIT_MIN 48
+#endif
+constexpr int split_of(int n) { return n >= LGF_SPLIT_MIN ? 2 : 1; }
 
 // ---------------------------------------------------------------- tile geometry
 // Shared tile of a group: element (c, a, b) at (b*RS + a*C + c), RS = NA*C + C (one padding
@@ -551,7 +554,14 @@ k_fft_zt(cx<T> *__restrict__ w, Geom geo, const double *__restrict__ ptab, doubl
 
 // ---------------------------------------------------------------- dispatch
 // x-columns per (z,t) tile: 64-byte runs in global memory (FP64), unless the tile would not fit
-template <typename T, int N> struct ZTC { static constexpr int C = (sizeof(cx<T>) == 16 && N == 64) ? 2 : 4; };
+#ifndef LGF_ZT_BYTES
+#define LGF_ZT_BYTES 64
+#endif
+template <typename T, int N> struct ZTC {
+    static constexpr int WANT = LGF_ZT_BYTES / (int)sizeof(cx<T>);
+    static constexpr size_t tile_bytes(int c) { return (size_t)(N * c + c) * N * sizeof(cx<T>); }
+    static constexpr int C = tile_bytes(WANT) <= 200 * 1024 && N % WANT == 0 ? WANT : (tile_bytes(WANT / 2) <= 200 * 1024 && N % (WANT / 2) == 0 ? WANT / 2 : WANT / 4);
+};
 
 template <typename T, int N> static int setup_xy_n()
 {
