@@ -284,13 +284,19 @@ k_fft_xy(cx<T> *__restrict__ w, int64_t nplanes, const Ctrl *ctrl)
         }
         __syncthreads();
         if (ok) {
-#pragma unroll 4
-            for (int e = t; e < NA * NB; e += TP) f[e] = sm[(e / NA) * TL::RS + (e % NA)];
+#pragma unroll
+            for (int k = 0; k < (NA * NB + TP - 1) / TP; k++) {
+                const int e = t + k * TP;
+                if (e < NA * NB) f[e] = sm[(e / NA) * TL::RS + (e % NA)];
+            }
         }
     } else {
         if (ok) {
-#pragma unroll 4
-            for (int e = t; e < NA * NB; e += TP) sm[(e / NA) * TL::RS + (e % NA)] = f[e];
+#pragma unroll
+            for (int k = 0; k < (NA * NB + TP - 1) / TP; k++) {
+                const int e = t + k * TP;
+                if (e < NA * NB) sm[(e / NA) * TL::RS + (e % NA)] = f[e];
+            }
         }
         __syncthreads();
         if (on_x) {
@@ -355,8 +361,11 @@ k_fft_xy_inv_g(const cx<T> *__restrict__ w, cx<T> *__restrict__ gbuf, int64_t V,
 
     if (ok) {
         const cx<T> *f = w + (int64_t)fld * V + base;
-#pragma unroll 4
-        for (int e = l; e < NA * NB; e += TP) sm[(e / NA) * TL::RS + (e % NA)] = f[e];
+#pragma unroll
+        for (int k = 0; k < (NA * NB + TP - 1) / TP; k++) {
+            const int e = l + k * TP;
+            if (e < NA * NB) sm[(e / NA) * TL::RS + (e % NA)] = f[e];
+        }
     }
     __syncthreads();
     if (on_x) {
@@ -428,8 +437,11 @@ k_fft_xy_inv_g2(const cx<T> *__restrict__ w, cx<T> *__restrict__ gbuf, int64_t V
     const unsigned my = __ballot_sync(0xffffffffu, on_y), mx = __ballot_sync(0xffffffffu, on_x);
     {
         const cx<T> *f = w + (int64_t)(2 * rank + lf) * V + base;
-#pragma unroll 4
-        for (int e = l; e < NA * NB; e += TP) sm[(e / NA) * TL::RS + (e % NA)] = f[e];
+#pragma unroll
+        for (int k = 0; k < (NA * NB + TP - 1) / TP; k++) {
+            const int e = l + k * TP;
+            if (e < NA * NB) sm[(e / NA) * TL::RS + (e % NA)] = f[e];
+        }
     }
     __syncthreads();
     if (on_x) {
@@ -557,10 +569,10 @@ k_fft_zt(cx<T> *__restrict__ w, Geom geo, const double *__restrict__ ptab, doubl
 #ifndef LGF_ZT_BYTES
 #define LGF_ZT_BYTES 64
 #endif
-template <typename T, int N> struct ZTC {
+template <typename T, int NA, int NB> struct ZTC {
     static constexpr int WANT = LGF_ZT_BYTES / (int)sizeof(cx<T>);
-    static constexpr size_t tile_bytes(int c) { return (size_t)(N * c + c) * N * sizeof(cx<T>); }
-    static constexpr int C = tile_bytes(WANT) <= 200 * 1024 && N % WANT == 0 ? WANT : (tile_bytes(WANT / 2) <= 200 * 1024 && N % (WANT / 2) == 0 ? WANT / 2 : WANT / 4);
+    static constexpr size_t tile_bytes(int c) { return (size_t)(NA * c + c) * NB * sizeof(cx<T>); }
+    static constexpr int C = tile_bytes(WANT) <= 200 * 1024 && NA % WANT == 0 ? WANT : (tile_bytes(WANT / 2) <= 200 * 1024 && NA % (WANT / 2) == 0 ? WANT / 2 : WANT / 4);
 };
 
 template <typename T, int N> static int setup_xy_n()
@@ -580,20 +592,21 @@ template <typename T, int N> static int setup_xy_n()
     return 0;
 }
 
-template <typename T, int N> static int setup_zt_n()
+template <typename T, int NA, int NB> static int setup_zt_n()
 {
-    typedef ZTCfg<T, N, N, ZTC<T, N>::C> Z;
-    cudaError_t e = cudaFuncSetAttribute(k_fft_zt<T, N, N, ZTC<T, N>::C>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Z::SMEM);
+    constexpr int C = ZTC<T, NA, NB>::C;
+    typedef ZTCfg<T, NA, NB, C> Z;
+    cudaError_t e = cudaFuncSetAttribute(k_fft_zt<T, NA, NB, C>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Z::SMEM);
     return e == cudaSuccess ? 0 : 1;
 }
 
-template <typename T, int N> static int launch_zt_n(const FftArgs &a, cudaStream_t st)
+template <typename T, int NA, int NB> static int launch_zt_n(const FftArgs &a, cudaStream_t st)
 {
-    constexpr int C = ZTC<T, N>::C;
-    typedef ZTCfg<T, N, N, C> Z;
+    constexpr int C = ZTC<T, NA, NB>::C;
+    typedef ZTCfg<T, NA, NB, C> Z;
     const int64_t ntiles = (int64_t)a.nfields * a.geo.N[1] * (a.geo.N[0] / C);
     const unsigned grid = (unsigned)((ntiles + Z::G - 1) / Z::G);
-    k_fft_zt<T, N, N, C><<<grid, Z::CTA, Z::SMEM, st>>>((cx<T> *)a.w, a.geo, a.ptab, a.pmax2 / (double)a.geo.V, ntiles, a.ctrl);
+    k_fft_zt<T, NA, NB, C><<<grid, Z::CTA, Z::SMEM, st>>>((cx<T> *)a.w, a.geo, a.ptab, a.pmax2 / (double)a.geo.V, ntiles, a.ctrl);
     return 0;
 }
 
@@ -623,14 +636,20 @@ template <typename T, int N> static int launch_inv_g_n(const FftArgs &a, void *g
 
 template <typename T, int N> static int gbuf_fits_n() { return (XYGCfg<T, N, N>::FITS || XYG2Cfg<T, N, N>::FITS) ? 1 : 0; }
 
-// Lattices Nx = Ny, Nz = Nt with both extents in {8, 12, 16, 24, 32, 48, 64}: the (x,y) passes
-// are instantiated per Nx and the (z,t) pass per Nz (x-columns per tile must divide Nx: 2 or 4).
-// Everything else takes the generic path.
+// Lattices with Nx = Ny in {8, 12, 16, 24, 32, 48, 64} and (Nz, Nt) either equal and in the same
+// set or (32, n), n in {8, 16, 48, 64} (the paper's 32^3 x n lattices): the (x,y)
+// passes are instantiated per Nx and the (z,t) pass per (Nz, Nt).  The x-columns of a (z,t) tile
+// must divide Nx (2 or 4).  Everything else takes the generic path.
 static bool tiled_extent(int n) { return n == 8 || n == 16 || n == 32 || n == 64 || n == 12 || n == 24 || n == 48; }
+static bool tiled_zt(int nz, int nt)
+{
+    if (nz == nt) return tiled_extent(nz);
+    return nz == 32 && (nt == 8 || nt == 16 || nt == 48 || nt == 64);
+}
 bool fft_tiled_supported(const int N[4], int prec)
 {
     (void)prec;
-    return N[0] == N[1] && N[2] == N[3] && tiled_extent(N[0]) && tiled_extent(N[2]);
+    return N[0] == N[1] && tiled_extent(N[0]) && tiled_zt(N[2], N[3]);
 }
 
 #define LGF_FFT_SWITCH(FN, ...)                                         \
@@ -650,12 +669,21 @@ static int setup_xy(int n, int prec)
     LGF_FFT_SWITCH(setup_xy_n)
     return 1;
 }
-static int setup_zt(int n, int prec)
+// (z,t) pass: FN<T, Nz, Nt> for the supported pairs
+#define LGF_ZT_CASE(FN, A, B, ...) \
+    if (nz == A && nt == B) return prec == 0 ? FN<double, A, B>(__VA_ARGS__) : FN<float, A, B>(__VA_ARGS__);
+#define LGF_ZT_SWITCH(FN, ...)                                                                              \
+    LGF_ZT_CASE(FN, 8, 8, __VA_ARGS__) LGF_ZT_CASE(FN, 12, 12, __VA_ARGS__) LGF_ZT_CASE(FN, 16, 16, __VA_ARGS__) \
+    LGF_ZT_CASE(FN, 24, 24, __VA_ARGS__) LGF_ZT_CASE(FN, 32, 32, __VA_ARGS__) LGF_ZT_CASE(FN, 48, 48, __VA_ARGS__) \
+    LGF_ZT_CASE(FN, 64, 64, __VA_ARGS__) LGF_ZT_CASE(FN, 32, 8, __VA_ARGS__) LGF_ZT_CASE(FN, 32, 16, __VA_ARGS__) \
+    LGF_ZT_CASE(FN, 32, 48, __VA_ARGS__) LGF_ZT_CASE(FN, 32, 64, __VA_ARGS__)
+
+static int setup_zt(int nz, int nt, int prec)
 {
-    LGF_FFT_SWITCH(setup_zt_n)
+    LGF_ZT_SWITCH(setup_zt_n)
     return 1;
 }
-int fft_tiled_setup(const int N[4], int prec) { return setup_xy(N[0], prec) | setup_zt(N[2], prec); }
+int fft_tiled_setup(const int N[4], int prec) { return setup_xy(N[0], prec) | setup_zt(N[2], N[3], prec); }
 
 // does the plane of 4 packed fields fit in shared memory (pass 2 with the g build fused)?
 bool fft_tiled_gbuf_supported(const int N[4], int prec)
@@ -674,8 +702,8 @@ static int run_xy(const FftArgs &a, int which, cudaStream_t st)
 }
 static int run_zt(const FftArgs &a, cudaStream_t st)
 {
-    const int n = a.geo.N[2], prec = a.prec;
-    LGF_FFT_SWITCH(launch_zt_n, a, st)
+    const int nz = a.geo.N[2], nt = a.geo.N[3], prec = a.prec;
+    LGF_ZT_SWITCH(launch_zt_n, a, st)
     return 1;
 }
 void launch_fft_tiled(const FftArgs &a, int which, cudaStream_t st)

@@ -234,7 +234,8 @@ def test_fp32_variant(lgf, lat, var):
 
 
 def test_tiled_fft_is_taken_where_expected(lgf):
-    for n, want in [(8, True), (12, True), (16, True), (24, True), (32, True), (48, True), (64, True), ((16, 16, 8, 8), True),
+    for n, want in [(8, True), (12, True), (16, True), (24, True), (32, True), (48, True), (64, True), ((16, 16, 8, 8), True), ((32, 32, 32, 16), True), ((8, 8, 32, 64), True),
+                    ((8, 8, 16, 32), False),
                     ((8, 8, 8, 16), False), ((8, 16, 8, 8), False), (4, False), (36, False)]:
         gf = fixer(lgf, n)
         assert gf.uses_tiled_fft() == want, n
@@ -244,7 +245,9 @@ def test_tiled_fft_is_taken_where_expected(lgf):
 # Lines of 48 and 64 are shared by two threads (fft_tiled.cu, Line<T, N, 2>); lattices with
 # Nx = Ny != Nz = Nt put them in the (x,y) passes or in the (z,t) pass at a size the oracle
 # finishes in about a second.
-SPLIT_LATTICES = [((64, 64, 8, 8), 81), ((8, 8, 64, 64), 82), ((48, 48, 12, 12), 83), ((16, 16, 48, 48), 84)]
+SPLIT_LATTICES = [((64, 64, 8, 8), 81), ((8, 8, 64, 64), 82), ((48, 48, 12, 12), 83), ((16, 16, 48, 48), 84),
+                  # (z,t) tiles with Nz = 32 != Nt: the paper's 32^3 x n lattices
+                  ((32, 32, 32, 8), 85), ((8, 8, 32, 16), 86), ((8, 8, 32, 48), 87), ((8, 8, 32, 64), 88)]
 
 
 @pytest.mark.parametrize("lat", SPLIT_LATTICES, ids=lambda v: "x".join(map(str, v[0])))
@@ -318,3 +321,93 @@ def test_headline_32_12real_one_iteration_and_golden(lgf):
         gf.load_links(U)
         r = gf.fix(ALPHA, 1e-15)
         assert r.converged == 1 and abs(r.iterations - it) <= 0.02 * it and abs(r.F - F) <= 1e-10
+
+
+def _mem_available_gb():
+    try:
+        with open("/proc/meminfo") as f:
+            for line in f:
+                if line.startswith("MemAvailable:"):
+                    return int(line.split()[1]) / 1e6
+    except OSError:
+        pass
+    return 0.0
+
+
+def _unitarity_defect(U):
+    I = np.eye(3)
+    worst = 0.0
+    for lo in range(0, U.shape[0], 1 << 20):                 # chunked: the full product would double the memory
+        u = U[lo:lo + (1 << 20)].astype(np.complex128)
+        worst = max(worst, float(np.abs(u @ np.conj(np.swapaxes(u, -1, -2)) - I).max()),
+                    float(np.abs(np.linalg.det(u) - 1).max()))
+    return worst
+
+
+@pytest.mark.slow
+def test_full_size_48_fp32(lgf):
+    """BASELINE config 4 in the configuration bench.py times: 48^4, FP32 storage and FFT, FP64 sums,
+    18-real links.  One iteration against the oracle element by element (north_star: 1e-5), then
+    Algorithm 1 to theta <= 1e-12 with the invariants that hold at any size."""
+    n, seed = 48, gen.BASE_SEED + 48
+    U = gen.gen_links(n, 0.5, seed)
+    gf = fixer(lgf, n, precision="fp32", recon=18)
+    assert gf.uses_tiled_fft() and gf.uses_gbuf()
+    U32 = U.astype(np.complex64)
+    gf.load_links(U32)
+    _, F0, th0 = oracle.measure(n, U, want_delta=False)
+    Fg, thg = gf.measure()
+    assert abs(Fg - F0) < 1e-6 and abs(thg - th0) <= 1e-5 * th0
+    r1 = gf.iterate(ALPHA, 1)
+    U1 = gf.get_links().astype(np.complex128)
+    Uo = U.copy()
+    hist = oracle.iterate(n, Uo, ALPHA, 1)
+    assert np.abs(U1 - Uo).max() < 1e-5
+    assert abs(r1.F - hist[1, 0]) < 1e-5 and abs(r1.theta - hist[1, 1]) <= 1e-4 * hist[1, 1]
+    del Uo, U1
+    gf.load_links(U32)
+    r = gf.fix(ALPHA, 1e-12)
+    assert r.converged == 1 and r.theta <= 1e-12 and 35 <= r.iterations <= 70
+    h = gf.history()
+    assert np.all(np.diff(h[:, 0]) >= -1e-6)                 # F never decreases (pin P12), FP32 rounding
+    Ufix = gf.get_links()
+    assert _unitarity_defect(Ufix) < 5e-5                     # no reunitarisation of links (reading R18)
+    assert abs(oracle.plaquette(n, Ufix.astype(np.complex128)) - oracle.plaquette(n, U)) < 1e-5
+
+
+@pytest.mark.slow
+def test_full_size_64_fp64(lgf):
+    """BASELINE config 5 in the configuration bench.py times: 64^4, FP64, 18-real links (9.7 GB of
+    links).  Measure and one iteration against the oracle (element by element when the host has the
+    memory for it), then Algorithm 1 to theta <= 1e-15 with the invariants that hold at any size."""
+    if _mem_available_gb() < 48:
+        pytest.skip("needs about 45 GB of host memory")
+    n, seed = 64, gen.BASE_SEED + 64
+    U = gen.gen_links(n, 0.6, seed)
+    gf = fixer(lgf, n, recon=18)
+    assert gf.uses_tiled_fft() and gf.uses_gbuf()             # 64^2 planes: 2-CTA cluster variant of the last pass
+    gf.load_links(U)
+    D, F0, th0 = oracle.measure(n, U)
+    Fg, thg = gf.measure()
+    assert abs(Fg - F0) <= 1e-12 * max(abs(F0), 1e-3) + 1e-15 and abs(thg - th0) <= 1e-12 * th0
+    assert np.abs(gf.get_field(lgf.FIELD_DELTA) - D).max() < 1e-13
+    del D
+    p0 = oracle.plaquette(n, U)
+    r1 = gf.iterate(ALPHA, 1)
+    U1 = gf.get_links()
+    # the fused kernel's F, theta are those of the links it stored
+    _, F1, th1 = oracle.measure(n, U1, want_delta=False)
+    assert abs(r1.F - F1) <= 1e-10 * abs(F1) and abs(r1.theta - th1) <= 1e-10 * th1
+    assert r1.F > F0 and abs(oracle.plaquette(n, U1) - p0) < 1e-12     # a gauge transformation (pin P11)
+    if _mem_available_gb() >= 40:
+        hist = oracle.iterate(n, U, ALPHA, 1)                 # in place: U becomes the oracle's U after one iteration
+        assert np.abs(U1 - U).max() < 1e-12
+        assert abs(r1.F - hist[1, 0]) <= 1e-10 * abs(hist[1, 0]) and abs(r1.theta - hist[1, 1]) <= 1e-10 * hist[1, 1]
+    del U1
+    r = gf.fix(ALPHA, 1e-15)                                  # continues from the links after one iteration
+    assert r.converged == 1 and r.theta <= 1e-15 and 35 <= r.iterations <= 70
+    h = gf.history()
+    assert np.all(np.diff(h[:, 0]) >= -1e-15)
+    Ufix = gf.get_links()
+    assert _unitarity_defect(Ufix) < 1e-12
+    assert abs(oracle.plaquette(n, Ufix) - p0) < 1e-12
