@@ -204,7 +204,7 @@ def run_ours(args):
     torch.cuda.synchronize()
 
     gf = lgf.GaugeFixer(N, precision=prec, recon=recon, fft_batch=args.fft_batch, fft_path=args.fft_path,
-                        fusion=args.fusion, device=f"cuda:{local}")
+                        fusion=args.fusion, l2_persist=args.l2_persist, device=f"cuda:{local}")
     K, W = args.steps, args.warmup
     stream = gf.stream
 
@@ -336,6 +336,7 @@ def main():
     ap.add_argument("--fft-batch", type=int, default=4, choices=[4, 9])
     ap.add_argument("--fft-path", type=int, default=0, choices=[0, 1])
     ap.add_argument("--fusion", type=int, default=1, choices=[0, 1])
+    ap.add_argument("--l2-persist", type=int, default=0, choices=[0, 1])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup

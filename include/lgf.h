@@ -70,12 +70,19 @@ enum {
                                    1: always the generic per-axis transform */
     LGF_OPT_PROFILE = 6,        /* 1: bracket every kernel launch with CUDA events on the bound
                                    stream so that lgf_kernel_time works; default 0 */
-    LGF_OPT_FUSION = 7          /* 1 (default): lgf_iterate / lgf_fix run the link update and the
+    LGF_OPT_FUSION = 7,         /* 1 (default): lgf_iterate / lgf_fix run the link update and the
                                    measure of the next iteration as ONE kernel over double-buffered
                                    links (each link read once, written once per iteration), with g
                                    built in the last FFT pass where the tile fits;
                                    0: the three separate kernels of lgf_stage (measure, Fourier,
                                    update in place), as in the paper's kernel list */
+    LGF_OPT_L2_PERSIST = 8      /* 1: when the field buffer (Delta / w) fits in the persisting part of the
+                                   L2 cache, lgf_bind sets an access-policy window on the bound stream so
+                                   that the passes over the field between the link kernels are served by
+                                   L2 instead of HBM (sets the device limit cudaLimitPersistingL2CacheSize;
+                                   undone by lgf_destroy).  0 (default): off -- measured slower at 32^4,
+                                   the set-aside takes L2 away from the link kernel's neighbour re-reads
+                                   (DESIGN.md section 6). */
 };
 
 /* lgf_get_field / lgf_set_field selectors */

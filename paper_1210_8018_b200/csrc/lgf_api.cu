@@ -35,7 +35,8 @@ struct lgf_ctx {
     int N[4];
     int64_t V;
     int prec;
-    int recon = 18, pack = 4, check_interval = 8, fft_path = 0, profile = 0, fusion = 1;
+    int recon = 18, pack = 4, check_interval = 8, fft_path = 0, profile = 0, fusion = 1, l2_persist = 0;
+    bool l2_window = false;  // an access-policy window is set on the bound stream
     int cur = 0, wcur = 0;   // which of the two link / field buffers is current
     bool use_gbuf = false;   // last FFT pass writes g (fusion, tiled FFT, 4 packed fields)
     void *links_buf[2] = {nullptr, nullptr}, *w_buf[2] = {nullptr, nullptr}, *gbuf = nullptr;
@@ -232,6 +233,42 @@ int clear_done(lgf_ctx *ctx)
     return LGF_OK;
 }
 
+// L2 residency of the field buffer: Delta is written by the link kernel, then read and written by
+// the three FFT passes; it is far smaller than the links (64 of 1344 bytes per site), so keeping it
+// in the persisting part of L2 removes its HBM round trips.  Best effort: silently skipped when
+// the device has no persisting L2 or the buffer does not fit.
+void l2_window_set(lgf_ctx *c)
+{
+    c->l2_window = false;
+    if (!c->l2_persist) return;
+    int dev = 0, max_persist = 0, max_window = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) return;
+    cudaDeviceGetAttribute(&max_persist, cudaDevAttrMaxPersistingL2CacheSize, dev);
+    cudaDeviceGetAttribute(&max_window, cudaDevAttrMaxAccessPolicyWindowSize, dev);
+    const size_t bytes = (size_t)c->pack * c->V * elem_bytes(c);
+    if (max_persist <= 0 || bytes > (size_t)max_persist || bytes > (size_t)max_window) { cudaGetLastError(); return; }
+    if (cudaDeviceSetLimit(cudaLimitPersistingL2CacheSize, bytes) != cudaSuccess) { cudaGetLastError(); return; }
+    cudaStreamAttrValue v{};
+    v.accessPolicyWindow.base_ptr = c->w_buf[0];
+    v.accessPolicyWindow.num_bytes = bytes;
+    v.accessPolicyWindow.hitRatio = 1.0f;
+    v.accessPolicyWindow.hitProp = cudaAccessPropertyPersisting;
+    v.accessPolicyWindow.missProp = cudaAccessPropertyStreaming;
+    if (cudaStreamSetAttribute(c->st, cudaStreamAttributeAccessPolicyWindow, &v) != cudaSuccess) { cudaGetLastError(); return; }
+    c->l2_window = true;
+}
+
+void l2_window_clear(lgf_ctx *c)
+{
+    if (!c->l2_window) return;
+    cudaStreamAttrValue v{};
+    v.accessPolicyWindow.num_bytes = 0;
+    cudaStreamSetAttribute(c->st, cudaStreamAttributeAccessPolicyWindow, &v);
+    cudaCtxResetPersistingL2Cache();
+    cudaGetLastError();
+    c->l2_window = false;
+}
+
 int need_loaded(lgf_ctx *ctx)
 {
     if (!ctx) return LGF_ERR_INVALID_ARG;
@@ -279,7 +316,8 @@ int lgf_create(int Nx, int Ny, int Nz, int Nt, int precision, lgf_ctx **out)
 int lgf_set_option(lgf_ctx *ctx, int key, int64_t value)
 {
     if (!ctx) return LGF_ERR_INVALID_ARG;
-    const bool layout_key = (key == LGF_OPT_RECON || key == LGF_OPT_FFT_BATCH || key == LGF_OPT_FFT_PATH || key == LGF_OPT_FUSION);
+    const bool layout_key = (key == LGF_OPT_RECON || key == LGF_OPT_FFT_BATCH || key == LGF_OPT_FFT_PATH || key == LGF_OPT_FUSION ||
+                             key == LGF_OPT_L2_PERSIST);
     if (layout_key && ctx->bound) return fail(ctx, LGF_ERR_INVALID_ARG, "this option must be set before lgf_bind");
     switch (key) {
     case LGF_OPT_RECON:
@@ -300,6 +338,9 @@ int lgf_set_option(lgf_ctx *ctx, int key, int64_t value)
     case LGF_OPT_FUSION:
         if (value != 0 && value != 1) return fail(ctx, LGF_ERR_INVALID_ARG, "FUSION must be 0 or 1");
         ctx->fusion = (int)value; break;
+    case LGF_OPT_L2_PERSIST:
+        if (value != 0 && value != 1) return fail(ctx, LGF_ERR_INVALID_ARG, "L2_PERSIST must be 0 or 1");
+        ctx->l2_persist = (int)value; break;
     case LGF_OPT_PROFILE:
         if (ctx->bound) flush_events(ctx);
         ctx->profile = value ? 1 : 0; break;
@@ -368,6 +409,8 @@ int lgf_bind(lgf_ctx *ctx, void *dev_workspace, size_t bytes, void *cuda_stream)
         return cuda_fail(ctx, e, "fft_tiled_setup");
     }
     ctx->use_gbuf = ctx->fusion && ctx->tiled && ctx->pack == 4 && fft_tiled_gbuf_supported(ctx->N, ctx->prec);
+    l2_window_clear(ctx);
+    if (ctx->use_gbuf) l2_window_set(ctx);   // one field buffer, used in place by every pass
     ctx->bound = true;
     ctx->loaded = false;
     ctx->wstate = 0;
@@ -606,6 +649,7 @@ const char *lgf_last_error(const lgf_ctx *ctx) { return ctx ? ctx->err.c_str() :
 int lgf_destroy(lgf_ctx *ctx)
 {
     if (!ctx) return LGF_OK;
+    l2_window_clear(ctx);
     for (auto &p : ctx->evs) { cudaEventDestroy(p.a); cudaEventDestroy(p.b); }
     delete ctx;
     return LGF_OK;

@@ -18,7 +18,7 @@ ERR_INVALID_ARG, ERR_UNSUPPORTED_SIZE, ERR_NOT_BOUND, ERR_NOT_LOADED = -1, -2, -
 ERR_WORKSPACE_TOO_SMALL, ERR_CUDA, ERR_NOT_CONVERGED, ERR_NUMERIC = -5, -6, -7, -8
 PREC_FP64, PREC_FP32 = 0, 1
 LAYOUT_AOS = 0
-OPT_RECON, OPT_FFT_BATCH, OPT_MAX_ITER, OPT_CHECK_INTERVAL, OPT_FFT_PATH, OPT_PROFILE, OPT_FUSION = 1, 2, 3, 4, 5, 6, 7
+OPT_RECON, OPT_FFT_BATCH, OPT_MAX_ITER, OPT_CHECK_INTERVAL, OPT_FFT_PATH, OPT_PROFILE, OPT_FUSION, OPT_L2_PERSIST = 1, 2, 3, 4, 5, 6, 7, 8
 FIELD_DELTA, FIELD_W, FIELD_G = 0, 1, 2
 STAGE_MEASURE, STAGE_FOURIER, STAGE_UPDATE = 0, 1, 2
 KERNEL_NAMES = ["measure", "fft_xy_fwd", "fft_zt", "fft_xy_inv", "update", "fft_generic", "layout", "fft_xy_inv_g",
@@ -99,7 +99,7 @@ class GaugeFixer:
     torch complex tensors of the same shapes."""
 
     def __init__(self, N, precision="fp64", recon=18, fft_batch=4, fft_path=0, device="cuda:0",
-                 stream=None, max_iter=None, check_interval=None, profile=False, fusion=None):
+                 stream=None, max_iter=None, check_interval=None, profile=False, fusion=None, l2_persist=None):
         import torch
 
         self.torch = torch
@@ -118,6 +118,8 @@ class GaugeFixer:
         self.set_option(OPT_FFT_PATH, fft_path)
         if fusion is not None:
             self.set_option(OPT_FUSION, fusion)
+        if l2_persist is not None:
+            self.set_option(OPT_L2_PERSIST, l2_persist)
         if max_iter is not None:
             self.set_option(OPT_MAX_ITER, max_iter)
         if check_interval is not None:
