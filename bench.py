@@ -114,6 +114,20 @@ def peaks():
     return 6650.0, "fallback (B200_PROFILING.md)"
 
 
+def ncu_traffic(workload_key, kernel):
+    """DRAM bytes per launch of `kernel` from the committed ncu summary (profiles/*_traffic.csv), or None."""
+    import csv
+    import glob
+
+    best = None
+    for path in sorted(glob.glob(os.path.join(ROOT, "profiles", "*_traffic.csv"))):
+        with open(path) as f:
+            for row in csv.DictReader(f):
+                if row["workload"] == workload_key and row["kernel"] == kernel:
+                    best = int(row["dram_read_bytes"]) + int(row["dram_write_bytes"])
+    return best
+
+
 def time_oracle(N, sigma, seed, iters):
     """The oracle as it stands, single thread: site-iterations/s over `iters` iterations."""
     import gen
@@ -312,7 +326,9 @@ def run_ours(args):
                 "what": "lgf_load_links(pinned host) + lgf_iterate(1) + result readback, every step"},
         "gpu_launches": int(launches),
         "roofline": {"bound": "hbm", "kernel": dom, "achieved": kern[dom]["GBps"], "peak": peak, "unit": "GB/s",
-                     "frac": kern[dom]["GBps"] / peak, "traffic": None, "peak_source": peak_src,
+                     "frac": kern[dom]["GBps"] / peak,
+                     "traffic": ncu_traffic(f"{args.workload}-{prec}-recon{recon}-fields{args.fft_batch}", dom),
+                     "algorithmic_bytes": per[dom] * V, "peak_source": peak_src,
                      "bytes_per_site": per[dom],
                      "iteration": {"bytes_per_site": iter_bytes, "bytes_per_site_this_build": moved_bytes, "GBps": iter_bytes * V * K / (ms_all * 1e-3) / 1e9,
                                    "frac": iter_bytes * V * K / (ms_all * 1e-3) / 1e9 / peak,
