@@ -1,0 +1,80 @@
+"""Variant sweep on 32^3 x n lattices: the shape of Fig. 1 of arXiv 1210.8018 (PAPER.md:140,
+165-169, 183) on one B200.
+
+    python -m paper_1210_8018_b200.sweep [--nt 8 16 32 48 64] [--steps 20] [--out sweep.md]
+
+Variants: single / double precision x 18 / 12 reals per link (the paper's sp/dp and 18/12-real
+axes; its texture and ECC axes are Fermi board settings).  For every variant
+and lattice it times `steps` iterations of Algorithm 1 with lgf_iterate (CUDA events on the
+library's stream, 5 warm-up iterations) and prints a markdown table: ms per iteration,
+site-iterations/s, and the GFlops the PAPER'S flop model would credit for that rate
+(Table 1, plus V 5 (log2(nx ny) + log2(nz nt)) per 4D FFT, 9 forward and
+9 inverse) -- the unit of the paper's 186 / 71 GFlops on a Tesla C2070
+(PAPER.md:185).  This build executes fewer operations than that model counts (4 packed FFT fields,
+rows-only link products), so the figure is a rate in the paper's currency, not an operation count.
+Inputs are the seeded synthetic generator of DESIGN.md section 4 (sigma = 0.5).
+"""
+import argparse
+import math
+import os
+import sys
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+
+def paper_flops_per_site(N, recon):
+    """Flop count per site and iteration in the paper's model (Table 1 + FFT model)."""
+    k2, k5, k6 = (841, 153, 1962) if recon == 12 else (505, 153, 1584)
+    k4 = 2 * 9
+    fft = 18 * 5 * (math.log2(N[0] * N[1]) + math.log2(N[2] * N[3]))
+    return k2 + k4 + k5 + k6 + fft
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--nt", type=int, nargs="+", default=[8, 16, 32, 48, 64])
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--out", default=None)
+    args = ap.parse_args()
+    import numpy as np
+    import torch
+
+    import gen
+    from paper_1210_8018_b200 import lgf
+
+    lines = ["| lattice | precision | reals/link | FFT path | ms/iteration | site-iterations/s | paper-model GFlops |",
+             "|---|---|---|---|---|---|---|"]
+    for nt in args.nt:
+        N = (32, 32, 32, nt)
+        V = 32 * 32 * 32 * nt
+        U = gen.gen_links(N, 0.5, gen.BASE_SEED + 3200 + nt)
+        for prec in ("fp32", "fp64"):
+            Ud = torch.from_numpy(U.astype(np.complex64 if prec == "fp32" else np.complex128)).cuda()
+            for recon in (18, 12):
+                gf = lgf.GaugeFixer(N, precision=prec, recon=recon)
+                gf.load_links(Ud)
+                gf.iterate(0.08, 5)
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                torch.cuda.synchronize()
+                with torch.cuda.stream(gf.stream):
+                    e0.record(gf.stream)
+                    gf.iterate(0.08, args.steps, sync=False)
+                    e1.record(gf.stream)
+                torch.cuda.synchronize()
+                ms = e0.elapsed_time(e1) / args.steps
+                rate = V / (ms * 1e-3)
+                lines.append(f"| 32^3 x {nt} | {prec} | {recon} | {'tiled' if gf.uses_tiled_fft() else 'generic'} | {ms:.4f} | "
+                             f"{rate:.3e} | {rate * paper_flops_per_site(N, recon) / 1e9:.0f} |")
+                gf.close()
+            del Ud
+    text = "\n".join(lines)
+    print(text)
+    if args.out:
+        with open(args.out, "w") as f:
+            f.write(text + "\n")
+
+
+if __name__ == "__main__":
+    main()
