@@ -299,6 +299,29 @@ def run_ours(args):
     e2e_val = world * V * e2e_steps / e2e_all
     h2d = V * 36 * 2 * real_bytes
 
+    # ---- side-by-side reference only (never on the product path): cuFFT through torch.fft on the same
+    # number of fields, forward + inverse 4D transforms, against the three hand-written passes
+    fft_ref = None
+    if tiled and args.cufft_reference:
+        try:
+            del dev
+            f = torch.randn((args.fft_batch, N[3], N[2], N[1], N[0]), dtype=tdt, device=f"cuda:{local}")
+            for _ in range(3):
+                f = torch.fft.ifftn(torch.fft.fftn(f, dim=(1, 2, 3, 4)), dim=(1, 2, 3, 4))
+            c0, c1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            torch.cuda.synchronize()
+            c0.record()
+            for _ in range(10):
+                f = torch.fft.ifftn(torch.fft.fftn(f, dim=(1, 2, 3, 4)), dim=(1, 2, 3, 4))
+            c1.record()
+            torch.cuda.synchronize()
+            ours = sum(kern[k]["us_per_launch"] for k in kern if k.startswith("fft_")) * 1e-3
+            fft_ref = {"cufft_fwd_inv_ms": c0.elapsed_time(c1) / 10, "ours_3_passes_ms": ours,
+                       "note": "cuFFT (torch.fft.fftn + ifftn, no mask, no g build) vs this build's passes (mask, 1/V and g build included)"}
+            del f
+        except RuntimeError as e:       # out of memory on the largest lattices: the reference is optional
+            fft_ref = {"unavailable": str(e).splitlines()[0][:120]}
+
     # ---- CPU baseline: the oracle as it stands on a bounded sample of the same workload
     cpu = None
     if not args.no_cpu_baseline:
@@ -335,6 +358,7 @@ def run_ours(args):
                                    "ms_profiled": ms_prof / K},
                      "kernels": kern},
         "cpu_baseline": cpu,
+        "fft_reference": fft_ref,
     }
     print(json.dumps(out), flush=True)
     if world > 1:
@@ -354,6 +378,7 @@ def main():
     ap.add_argument("--fusion", type=int, default=1, choices=[0, 1])
     ap.add_argument("--l2-persist", type=int, default=0, choices=[0, 1])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--cufft-reference", type=int, default=1, choices=[0, 1])
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     if args.impl == "reference":
