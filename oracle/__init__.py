@@ -42,6 +42,8 @@ def _load():
         L.orc_fft4d.argtypes = [_c_int4, _vp, ctypes.c_int]
         L.orc_fourier_accelerate.argtypes = [_c_int4, _vp, _vp]
         L.orc_build_g.argtypes = [ctypes.c_int64, _vp, ctypes.c_double, _vp]
+        L.orc_build_g_exp.argtypes = [ctypes.c_int64, _vp, ctypes.c_double, _vp]
+        L.orc_set_exponential.argtypes = [ctypes.c_int]
         L.orc_update_links.argtypes = [_c_int4, _vp, _vp]
         L.orc_iterate.argtypes = [_c_int4, _vp, ctypes.c_double, ctypes.c_int64, _vp]
         L.orc_fix.argtypes = [_c_int4, _vp, ctypes.c_double, ctypes.c_double, ctypes.c_int64,
@@ -50,7 +52,8 @@ def _load():
         L.orc_plaquette.argtypes = [_c_int4, _vp]
         L.orc_plaquette.restype = ctypes.c_double
         for f in (L.orc_momentum_tables, L.orc_mask, L.orc_measure, L.orc_fft1d, L.orc_fft4d,
-                  L.orc_fourier_accelerate, L.orc_build_g, L.orc_update_links, L.orc_iterate):
+                  L.orc_fourier_accelerate, L.orc_build_g, L.orc_build_g_exp, L.orc_set_exponential,
+                  L.orc_update_links, L.orc_iterate):
             f.restype = None
         _lib = L
     return _lib
@@ -127,6 +130,19 @@ def build_g(w, alpha):
     g = np.empty((V, 3, 3), dtype=np.complex128)
     _load().orc_build_g(V, _c128(w, V * 9), float(alpha), g.ctypes.data)
     return g
+
+
+def build_g_exp(w, alpha):
+    """g(x) = exp((alpha/2) w(x)): eq. 1.2 as written, the variant of SURVEY 8(f4)."""
+    V = w.size // 9
+    g = np.empty((V, 3, 3), dtype=np.complex128)
+    _load().orc_build_g_exp(V, _c128(w, V * 9), float(alpha), g.ctypes.data)
+    return g
+
+
+def set_exponential(on):
+    """iterate / fix form g by the exact exponential (True) or by first order + reunitarisation (False, default)."""
+    _load().orc_set_exponential(1 if on else 0)
 
 
 def update_links(N, U, g):

@@ -267,6 +267,48 @@ void orc_build_g(int64_t V, const cd *w, double alpha, cd *g)
     }
 }
 
+/* Variant named by the paper: eq. 1.2 as written, g(x) = exp[(alpha/2) w(x)]
+ * (PAPER.md:49), instead of its first-order expansion followed by a reunitarisation.
+ * Textbook scaling and squaring: B = A / 2^s with |B|_F <= 1/4, exp(B) by its Taylor series
+ * summed until the terms vanish in FP64, then s squarings.  A = (alpha/2) w is anti-Hermitian and
+ * traceless, so exp(A) is in SU(3) up to rounding; no projection is applied. */
+void orc_build_g_exp(int64_t V, const cd *w, double alpha, cd *g)
+{
+    for (int64_t x = 0; x < V; x++) {
+        cd A[9], E[9], term[9], tmp[9];
+        double nrm = 0;
+        for (int k = 0; k < 9; k++) { A[k] = (alpha / 2.0) * w[x * 9 + k]; nrm += creal(A[k] * conj(A[k])); }
+        nrm = sqrt(nrm);
+        int s = 0;
+        while (nrm > 0.25) { nrm *= 0.5; s++; }
+        for (int k = 0; k < 9; k++) { A[k] = ldexp(creal(A[k]), -s) + I * ldexp(cimag(A[k]), -s); }
+        for (int k = 0; k < 9; k++) { E[k] = (k % 4 == 0) ? 1.0 : 0.0; term[k] = E[k]; }
+        for (int n = 1; n <= 40; n++) {
+            /* term <- term A / n */
+            double tn = 0;
+            for (int i = 0; i < 3; i++)
+                for (int j = 0; j < 3; j++) {
+                    cd a = 0;
+                    for (int k = 0; k < 3; k++) a += term[3 * i + k] * A[3 * k + j];
+                    tmp[3 * i + j] = a / (double)n;
+                    tn += creal(tmp[3 * i + j] * conj(tmp[3 * i + j]));
+                }
+            for (int k = 0; k < 9; k++) { term[k] = tmp[k]; E[k] += term[k]; }
+            if (tn < 1e-40) break;
+        }
+        for (int q = 0; q < s; q++) {
+            for (int i = 0; i < 3; i++)
+                for (int j = 0; j < 3; j++) {
+                    cd a = 0;
+                    for (int k = 0; k < 3; k++) a += E[3 * i + k] * E[3 * k + j];
+                    tmp[3 * i + j] = a;
+                }
+            for (int k = 0; k < 9; k++) E[k] = tmp[k];
+        }
+        for (int k = 0; k < 9; k++) g[x * 9 + k] = E[k];
+    }
+}
+
 /* ------------------------------------------------------------------ O7: link update */
 
 static void mul3(const cd *a, const cd *b, cd *c) /* c = a b */
@@ -307,10 +349,16 @@ void orc_update_links(const int N[4], cd *U, const cd *g)
 /* ------------------------------------------------------------------ Algorithm 1 */
 
 /* One pass of the loop body (Alg. 1 lines 3-16) given Delta of the current links. */
+static int g_mode = 0; /* 0: first order + reunitarisation (the paper's choice); 1: exact exponential */
+
+/* Select how g(x) is formed in orc_iterate / orc_fix (single-threaded test infrastructure: a plain global). */
+void orc_set_exponential(int on) { g_mode = on ? 1 : 0; }
+
 static void loop_body(const int N[4], cd *U, const cd *Delta, double alpha, cd *w, cd *g)
 {
     orc_fourier_accelerate(N, Delta, w);
-    orc_build_g(volume(N), w, alpha, g);
+    if (g_mode) orc_build_g_exp(volume(N), w, alpha, g);
+    else orc_build_g(volume(N), w, alpha, g);
     orc_update_links(N, U, g);
 }
 

@@ -308,3 +308,73 @@ def test_P18_iteration_count_is_robust_to_rounding_noise():
     a = oracle.fix(N, U.copy(), ALPHA, 1e-15)
     b = oracle.fix(N, np.ascontiguousarray(Un), ALPHA, 1e-15)
     assert a[0] == b[0] and abs(a[1] - b[1]) < 1e-13
+
+
+# ---------------------------------------------------------------- variant: exact exponential
+def _random_ah_traceless(rng, n, scale):
+    a = rng.normal(size=(n, 3, 3)) + 1j * rng.normal(size=(n, 3, 3))
+    a = a - np.conj(np.swapaxes(a, -1, -2))
+    a = a - (np.trace(a, axis1=-2, axis2=-1) / 3)[:, None, None] * np.eye(3)
+    return scale * a
+
+
+def test_exp_variant_closed_form_library_and_group():
+    """g = exp((alpha/2) w), eq. 1.2 as written: closed form on diagonal w, scipy's expm
+    (a library routine, Pade) on random anti-Hermitian traceless w over a wide range of norms, SU(3)."""
+    from scipy.linalg import expm
+
+    rng = np.random.default_rng(5)
+    alpha = 0.08
+    ph = rng.normal(size=(64, 2)) * 5
+    w = np.zeros((64, 3, 3), dtype=np.complex128)
+    w[:, 0, 0] = 1j * ph[:, 0]
+    w[:, 1, 1] = 1j * ph[:, 1]
+    w[:, 2, 2] = -1j * (ph[:, 0] + ph[:, 1])
+    g = oracle.build_g_exp(w, alpha)
+    want = np.zeros_like(g)
+    for k in range(3):
+        want[:, k, k] = np.exp(alpha / 2 * w[:, k, k])
+    assert np.abs(g - want).max() < 1e-15
+    for scale in (1e-3, 1.0, 10.0, 200.0):
+        w = _random_ah_traceless(rng, 50, scale)
+        g = oracle.build_g_exp(w, alpha)
+        ref = np.stack([expm(alpha / 2 * m) for m in w])
+        # squarings amplify rounding with |A|: both routines carry an error of a few |A| eps
+        assert np.abs(g - ref).max() < (2e-14 if scale <= 10 else 2e-13)
+        assert np.abs(g @ np.conj(np.swapaxes(g, -1, -2)) - np.eye(3)).max() < 1e-13
+        assert np.abs(np.linalg.det(g) - 1).max() < 1e-13
+
+
+def test_exp_variant_agrees_with_first_order_to_second_order():
+    """reunit(1 + A) and exp(A) differ at O(|A|^2): halving alpha divides the difference by 4."""
+    rng = np.random.default_rng(6)
+    w = _random_ah_traceless(rng, 200, 1.0)
+    d = [np.abs(oracle.build_g_exp(w, a) - oracle.build_g(w, a)).max() for a in (0.02, 0.01)]
+    assert 3.5 < d[0] / d[1] < 4.5 and d[0] < 0.02
+
+
+def test_exp_variant_iteration_is_a_gauge_transformation_and_converges():
+    """With the exact exponential the update is still a gauge transformation (plaquette), F rises
+    monotonically, theta reaches 1e-15, and the linear contraction factor is the same (1 - 16 alpha)^2."""
+    n = 4
+    U = gen.gen_links(n, 0.4, 21)
+    p0 = oracle.plaquette(n, U)
+    oracle.set_exponential(True)
+    try:
+        it, F, th, hist = oracle.fix(n, U, 0.08, 1e-15)
+        assert 0 < it < 200 and th <= 1e-15
+        assert np.all(np.diff(hist[:, 0]) >= -1e-15)
+        assert abs(oracle.plaquette(n, U) - p0) < 1e-12
+        eps = 1e-4
+        om = np.random.default_rng(3).normal(size=(n ** 4, 8))
+        from helpers import GELL_MANN, expm_batch, shift, dag, unit_links
+        g0 = expm_batch(1j * eps * np.einsum("xa,aij->xij", om, GELL_MANN) / 2)
+        V0 = unit_links(n)
+        for mu in range(4):
+            V0[:, mu] = g0 @ dag(shift(n, g0, mu, 1))
+        h = oracle.iterate(n, V0, 0.08, 1)
+        assert abs(h[1, 1] / h[0, 1] - (1 - 16 * 0.08) ** 2) < 1e-3
+    finally:
+        oracle.set_exponential(False)
+    it0 = oracle.fix(n, gen.gen_links(n, 0.4, 21), 0.08, 1e-15)[0]
+    assert abs(it - it0) <= 0.25 * it0            # same fixed points, trajectories differ at O(alpha^2)
