@@ -1,7 +1,7 @@
 """Variant sweep on 32^3 x n lattices: the shape of Fig. 1 of arXiv 1210.8018 (PAPER.md:140,
 165-169, 183) on one B200.
 
-    python -m paper_1210_8018_b200.sweep [--nt 8 16 32 48 64] [--steps 20] [--out sweep.md]
+    python bench_sweep.py [--nt 8 16 32 48 64] [--steps 20] [--out sweep.md]
 
 Variants: single / double precision x 18 / 12 reals per link (the paper's sp/dp and 18/12-real
 axes; its texture and ECC axes are Fermi board settings).  For every variant
@@ -19,7 +19,7 @@ import math
 import os
 import sys
 
-ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+ROOT = os.path.dirname(os.path.abspath(__file__))
 if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
