@@ -38,13 +38,16 @@ WORKLOADS = {
 }
 
 
-def algorithmic_bytes(recon, nfields, real_bytes, tiled, fusion, gbuf):
+def algorithmic_bytes(recon, nfields, real_bytes, tiled, fusion, gbuf, accum=0):
     """Bytes per site each kernel must move once:
     L = link bytes per site, W = field bytes per site, Gb = bytes of rows 0, 1 of g per site."""
     L = 4 * recon * real_bytes
     W = nfields * 2 * real_bytes
     Gb = 12 * real_bytes
     per = {}
+    if accum:
+        # LGF_OPT_ACCUM_G: links read once, never written; G read by the link kernel, read + written by the last pass
+        return {"measure_acc": L + Gb + W, "fft_xy_fwd": 2 * W, "fft_zt": 2 * W, "fft_xy_inv_gacc": W + 2 * Gb}
     if fusion:
         per["update_measure"] = (Gb if gbuf else W) + 2 * L + W
     else:
@@ -218,7 +221,8 @@ def run_ours(args):
     torch.cuda.synchronize()
 
     gf = lgf.GaugeFixer(N, precision=prec, recon=recon, fft_batch=args.fft_batch, fft_path=args.fft_path,
-                        fusion=args.fusion, l2_persist=args.l2_persist, device=f"cuda:{local}")
+                        fusion=args.fusion, l2_persist=args.l2_persist, accum_g=args.accum_g, gmap=args.gmap,
+                        device=f"cuda:{local}")
     K, W = args.steps, args.warmup
     stream = gf.stream
 
@@ -241,6 +245,7 @@ def run_ours(args):
         with torch.cuda.stream(stream):
             e0.record(stream)
             gf.iterate(ALPHA, K, sync=False)
+            gf.sync_links()                     # ACCUM_G: the one link rewrite belongs to the window; else a no-op
             e1.record(stream)
         barrier()
         return e0.elapsed_time(e1), gf.launch_count()
@@ -280,7 +285,7 @@ def run_ours(args):
 
     real_bytes = 8 if prec == "fp64" else 4
     tiled = gf.uses_tiled_fft()
-    per = algorithmic_bytes(recon, args.fft_batch, real_bytes, tiled, args.fusion, gf.uses_gbuf())
+    per = algorithmic_bytes(recon, args.fft_batch, real_bytes, tiled, args.fusion, gf.uses_gbuf(), args.accum_g)
     peak, peak_src = peaks()
     kern = {k: {"ms_total": v[0], "launches": v[1], "us_per_launch": 1e3 * v[0] / v[1]}
             for k, v in ktimes.items() if v[1] and k in per}
@@ -337,7 +342,9 @@ def run_ours(args):
         "ms_per_step": ms_all / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f64" if prec == "fp64" else "f32", "data": "synthetic",
         "config": {"workload": f"{args.workload} periodic SU(3), {prec}, {recon}-real links, {args.fft_batch} FFT fields, "
-                               f"alpha={ALPHA}, gen seed {gen.BASE_SEED + soff}, sigma={sigma}",
+                               f"alpha={ALPHA}, gen seed {gen.BASE_SEED + soff}, sigma={sigma}"
+                               + (", ACCUM_G (fixed links + accumulated G, link rewrite inside the window)" if args.accum_g else "")
+                               + (", g = exp((alpha/2) w)" if args.gmap else ""),
                    "fft": "tiled register FFT, 3 passes" if tiled else "generic per-axis transform, 8 passes",
                    "l2": "working set (links + fields) exceeds the 126 MB L2" if V >= 32 ** 4 else
                          "working set fits in L2; latency/L2-bound by design (DESIGN.md section 6)",
@@ -377,6 +384,9 @@ def main():
     ap.add_argument("--fft-path", type=int, default=0, choices=[0, 1])
     ap.add_argument("--fusion", type=int, default=1, choices=[0, 1])
     ap.add_argument("--l2-persist", type=int, default=0, choices=[0, 1])
+    ap.add_argument("--accum-g", type=int, default=0, choices=[0, 1],
+                    help="LGF_OPT_ACCUM_G: fixed links + accumulated transformation (the link rewrite at the end of the window is timed)")
+    ap.add_argument("--gmap", type=int, default=0, choices=[0, 1], help="LGF_OPT_GMAP: 1 = exact exponential")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cufft-reference", type=int, default=1, choices=[0, 1])
     args = ap.parse_args()

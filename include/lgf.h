@@ -76,13 +76,27 @@ enum {
                                    built in the last FFT pass where the tile fits;
                                    0: the three separate kernels of lgf_stage (measure, Fourier,
                                    update in place), as in the paper's kernel list */
-    LGF_OPT_L2_PERSIST = 8      /* 1: when the field buffer (Delta / w) fits in the persisting part of the
+    LGF_OPT_L2_PERSIST = 8,     /* 1: when the field buffer (Delta / w) fits in the persisting part of the
                                    L2 cache, lgf_bind sets an access-policy window on the bound stream so
                                    that the passes over the field between the link kernels are served by
                                    L2 instead of HBM (sets the device limit cudaLimitPersistingL2CacheSize;
                                    undone by lgf_destroy).  0 (default): off -- measured slower at 32^4,
                                    the set-aside takes L2 away from the link kernel's neighbour re-reads
                                    (DESIGN.md section 6). */
+    LGF_OPT_GMAP = 9,           /* how g(x) is formed from w(x).  0 (default): the paper's choice, first
+                                   order g = 1 + (alpha/2) w followed by a reunitarisation;
+                                   1: the exact exponential g = exp((alpha/2) w) of eq. 1.2 as written
+                                   (PAPER.md:49), no projection.  May be changed at any time. */
+    LGF_OPT_ACCUM_G = 10        /* 1: lgf_iterate / lgf_fix keep the loaded links fixed and accumulate the
+                                   gauge transformation instead, G(x) <- g(x) G(x) (rows 0, 1 stored, Gram-
+                                   Schmidt after every product), measuring Delta, F, theta of
+                                   G(x) U_mu(x) G^dagger(x+mu) on the fly; the links are rewritten once,
+                                   when an iterate / fix call returns control to any other call that needs
+                                   them (lgf_get_links, lgf_measure, lgf_stage, field taps).  The same
+                                   iteration as Alg. 1 lines 12-16 up to rounding, without the
+                                   per-iteration link write; one link buffer instead of two.  Needs FUSION = 1,
+                                   FFT_BATCH = 4 and a lattice the tiled FFT covers, else lgf_bind fails with
+                                   LGF_ERR_INVALID_ARG.  0 (default): links rewritten every iteration. */
 };
 
 /* lgf_get_field / lgf_set_field selectors */
@@ -110,7 +124,10 @@ enum {
     LGF_KERNEL_LAYOUT = 6,
     LGF_KERNEL_FFT_XY_INV_G = 7,   /* last FFT pass with the g build as its epilogue */
     LGF_KERNEL_UPDATE_MEASURE = 8, /* fused link update + measure */
-    LGF_KERNEL_KINDS = 9
+    LGF_KERNEL_FFT_XY_INV_GACC = 9, /* last FFT pass with g build and G <- g G as its epilogue (ACCUM_G) */
+    LGF_KERNEL_MEASURE_ACC = 10,    /* Delta, F, theta of G U G^dagger from the fixed links and G (ACCUM_G) */
+    LGF_KERNEL_APPLY_G = 11,        /* U <- G U G^dagger in place, G <- 1 (ACCUM_G, once per call) */
+    LGF_KERNEL_KINDS = 12
 };
 
 /* Create a context for an Nx*Ny*Nz*Nt lattice.  host call; allocates host memory only.
@@ -180,6 +197,11 @@ int lgf_uses_tiled_fft(const lgf_ctx *ctx);
  * shared memory of one SM or of a 2-CTA cluster), 0 if g is rebuilt from w by the link kernel.
  * Valid after lgf_bind. */
 int lgf_uses_gbuf(const lgf_ctx *ctx);
+
+/* LGF_OPT_ACCUM_G: bring the link buffer up to date now, U_mu(x) <- G(x) U_mu(x) G^dagger(x+mu), G <- 1
+ * (two launches on the bound stream, asynchronous; the calls that read the links do this
+ * themselves).  No-op, LGF_OK, when nothing is pending or ACCUM_G is off.  Needs loaded links. */
+int lgf_sync_links(lgf_ctx *ctx);
 
 /* Text of the last error of this context (or of lgf_create when ctx == NULL). Never NULL. */
 const char *lgf_last_error(const lgf_ctx *ctx);

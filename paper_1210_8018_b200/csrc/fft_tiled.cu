@@ -335,9 +335,29 @@ template <typename T, int NA, int NB> struct XYGCfg {
     static constexpr bool FITS = SMEM <= 227 * 1024 && CTA <= 1024;
 };
 
-template <typename T, int NA, int NB>
+// g -> the g buffer, or (ACC, LGF_OPT_ACCUM_G) the accumulated transformation G(x) <- g(x) G(x):
+// rows 0, 1 of G are read, row 2 rebuilt, rows 0, 1 of the product Gram-Schmidt cleaned and stored.
+template <typename T, bool ACC>
+__device__ __forceinline__ void emit_g(cx<T> (&g)[9], cx<T> *__restrict__ dst, int64_t V)
+{
+    if (ACC) {
+        cx<T> G[9], n[9];
+#pragma unroll
+        for (int k = 0; k < 6; k++) G[k] = dst[(int64_t)k * V];
+        su3_row2(G);
+        mul_rows<2>(g, G, n);
+        reunit01<T>(n);
+#pragma unroll
+        for (int k = 0; k < 6; k++) dst[(int64_t)k * V] = n[k];
+    } else {
+#pragma unroll
+        for (int k = 0; k < 6; k++) dst[(int64_t)k * V] = g[k];
+    }
+}
+
+template <typename T, int NA, int NB, bool ACC>
 __global__ void __launch_bounds__((XYGCfg<T, NA, NB>::CTA))
-k_fft_xy_inv_g(const cx<T> *__restrict__ w, cx<T> *__restrict__ gbuf, int64_t V, int64_t nplanes, T a, const Ctrl *ctrl)
+k_fft_xy_inv_g(const cx<T> *__restrict__ w, cx<T> *__restrict__ gbuf, int64_t V, int64_t nplanes, T a, int gexp, const Ctrl *ctrl)
 {
     if (*(volatile const int *)&ctrl->done) return;
     typedef XYGCfg<T, NA, NB> CF;
@@ -359,6 +379,14 @@ k_fft_xy_inv_g(const cx<T> *__restrict__ w, cx<T> *__restrict__ gbuf, int64_t V,
     const bool on_y = ok && xa < NA && l < TL::SB * NA, on_x = ok && yb < NB && l < TL::SA * NB;
     const unsigned my = __ballot_sync(0xffffffffu, on_y), mx = __ballot_sync(0xffffffffu, on_x);
 
+    if (ACC && ok) {
+        // the epilogue reads rows 0, 1 of G of this plane: ask L2 for them now, behind the transforms
+        constexpr int LINES = (int)((size_t)NA * NB * sizeof(cx<T>) / 128);
+        for (int i = t; i < 6 * LINES; i += TG) {
+            const char *p = (const char *)(gbuf + (int64_t)(i / LINES) * V + base) + (size_t)(i % LINES) * 128;
+            asm volatile("prefetch.global.L2 [%0];" ::"l"(p));
+        }
+    }
     if (ok) {
         const cx<T> *f = w + (int64_t)fld * V + base;
 #pragma unroll
@@ -391,10 +419,8 @@ k_fft_xy_inv_g(const cx<T> *__restrict__ w, cx<T> *__restrict__ gbuf, int64_t V,
             const int o = (i / NA) * TL::RS + (i % NA);
             cx<T> g[9];
             m_from_packed<T>(smp[o], smp[TL::ELEMS + o], smp[2 * TL::ELEMS + o], smp[3 * TL::ELEMS + o], a, g);
-            reunit01<T>(g);
-            cx<T> *dst = gbuf + base + i;
-#pragma unroll
-            for (int k = 0; k < 6; k++) dst[(int64_t)k * V] = g[k];
+            finish_g01<T>(g, gexp);
+            emit_g<T, ACC>(g, gbuf + base + i, V);
         }
     }
 }
@@ -411,9 +437,9 @@ template <typename T, int NA, int NB> struct XYG2Cfg {
     static constexpr bool FITS = SMEM <= 227 * 1024 && CTA <= 1024 && CTA >= 64;
 };
 
-template <typename T, int NA, int NB>
+template <typename T, int NA, int NB, bool ACC>
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__((XYG2Cfg<T, NA, NB>::CTA))
-k_fft_xy_inv_g2(const cx<T> *__restrict__ w, cx<T> *__restrict__ gbuf, int64_t V, T a, const Ctrl *ctrl)
+k_fft_xy_inv_g2(const cx<T> *__restrict__ w, cx<T> *__restrict__ gbuf, int64_t V, T a, int gexp, const Ctrl *ctrl)
 {
     namespace cg = cooperative_groups;
     if (*(volatile const int *)&ctrl->done) return;          // uniform over the grid: both CTAs of a cluster leave
@@ -469,10 +495,8 @@ k_fft_xy_inv_g2(const cx<T> *__restrict__ w, cx<T> *__restrict__ gbuf, int64_t V
         const int o = (i / NA) * TL::RS + (i % NA);
         cx<T> g[9];
         m_from_packed<T>(f01[o], f01[TL::ELEMS + o], f23[o], f23[TL::ELEMS + o], a, g);
-        reunit01<T>(g);
-        cx<T> *dst = gbuf + base + i;
-#pragma unroll
-        for (int k = 0; k < 6; k++) dst[(int64_t)k * V] = g[k];
+        finish_g01<T>(g, gexp);
+        emit_g<T, ACC>(g, gbuf + base + i, V);
     }
     cluster.sync();                                          // the peer may still be reading this CTA's fields
 }
@@ -583,10 +607,14 @@ template <typename T, int N> static int setup_xy_n()
     e = cudaFuncSetAttribute(k_fft_xy<T, N, N, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)XYCfg<T, N, N>::SMEM);
     if (e != cudaSuccess) return 1;
     if (XYGCfg<T, N, N>::FITS) {
-        e = cudaFuncSetAttribute(k_fft_xy_inv_g<T, N, N>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)XYGCfg<T, N, N>::SMEM);
+        e = cudaFuncSetAttribute(k_fft_xy_inv_g<T, N, N, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)XYGCfg<T, N, N>::SMEM);
+        if (e != cudaSuccess) return 1;
+        e = cudaFuncSetAttribute(k_fft_xy_inv_g<T, N, N, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)XYGCfg<T, N, N>::SMEM);
         if (e != cudaSuccess) return 1;
     } else if (XYG2Cfg<T, N, N>::FITS) {
-        e = cudaFuncSetAttribute(k_fft_xy_inv_g2<T, N, N>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)XYG2Cfg<T, N, N>::SMEM);
+        e = cudaFuncSetAttribute(k_fft_xy_inv_g2<T, N, N, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)XYG2Cfg<T, N, N>::SMEM);
+        if (e != cudaSuccess) return 1;
+        e = cudaFuncSetAttribute(k_fft_xy_inv_g2<T, N, N, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)XYG2Cfg<T, N, N>::SMEM);
         if (e != cudaSuccess) return 1;
     }
     return 0;
@@ -620,16 +648,18 @@ template <typename T, int N> static int launch_xy_n(const FftArgs &a, int which,
     return 0;
 }
 
-template <typename T, int N> static int launch_inv_g_n(const FftArgs &a, void *gbuf, double alpha, cudaStream_t st)
+template <typename T, int N> static int launch_inv_g_n(const FftArgs &a, void *gbuf, double alpha, int gexp, int accum, cudaStream_t st)
 {
     const int64_t nplanes = (int64_t)a.geo.N[2] * a.geo.N[3];
     if (XYGCfg<T, N, N>::FITS) {
         typedef XYGCfg<T, N, N> X;
         const unsigned grid = (unsigned)((nplanes + X::G - 1) / X::G);
-        k_fft_xy_inv_g<T, N, N><<<grid, X::CTA, X::SMEM, st>>>((const cx<T> *)a.w, (cx<T> *)gbuf, a.geo.V, nplanes, (T)(alpha / 2.0), a.ctrl);
+        if (accum) k_fft_xy_inv_g<T, N, N, true><<<grid, X::CTA, X::SMEM, st>>>((const cx<T> *)a.w, (cx<T> *)gbuf, a.geo.V, nplanes, (T)(alpha / 2.0), gexp, a.ctrl);
+        else k_fft_xy_inv_g<T, N, N, false><<<grid, X::CTA, X::SMEM, st>>>((const cx<T> *)a.w, (cx<T> *)gbuf, a.geo.V, nplanes, (T)(alpha / 2.0), gexp, a.ctrl);
     } else {
         typedef XYG2Cfg<T, N, N> X;                           // one cluster of two CTAs per plane
-        k_fft_xy_inv_g2<T, N, N><<<(unsigned)(2 * nplanes), X::CTA, X::SMEM, st>>>((const cx<T> *)a.w, (cx<T> *)gbuf, a.geo.V, (T)(alpha / 2.0), a.ctrl);
+        if (accum) k_fft_xy_inv_g2<T, N, N, true><<<(unsigned)(2 * nplanes), X::CTA, X::SMEM, st>>>((const cx<T> *)a.w, (cx<T> *)gbuf, a.geo.V, (T)(alpha / 2.0), gexp, a.ctrl);
+        else k_fft_xy_inv_g2<T, N, N, false><<<(unsigned)(2 * nplanes), X::CTA, X::SMEM, st>>>((const cx<T> *)a.w, (cx<T> *)gbuf, a.geo.V, (T)(alpha / 2.0), gexp, a.ctrl);
     }
     return 0;
 }
@@ -712,12 +742,12 @@ void launch_fft_tiled(const FftArgs &a, int which, cudaStream_t st)
 }
 
 // pass 2 fused with the g build: needs the 4 packed fields (nfields == 4)
-static int run_inv_g(const FftArgs &a, void *gbuf, double alpha, cudaStream_t st)
+static int run_inv_g(const FftArgs &a, void *gbuf, double alpha, int gexp, int accum, cudaStream_t st)
 {
     const int n = a.geo.N[0], prec = a.prec;
-    LGF_FFT_SWITCH(launch_inv_g_n, a, gbuf, alpha, st)
+    LGF_FFT_SWITCH(launch_inv_g_n, a, gbuf, alpha, gexp, accum, st)
     return 1;
 }
-void launch_fft_tiled_inv_g(const FftArgs &a, void *gbuf, double alpha, cudaStream_t st) { run_inv_g(a, gbuf, alpha, st); }
+void launch_fft_tiled_inv_g(const FftArgs &a, void *gbuf, double alpha, int gexp, int accum, cudaStream_t st) { run_inv_g(a, gbuf, alpha, gexp, accum, st); }
 
 } // namespace lgf

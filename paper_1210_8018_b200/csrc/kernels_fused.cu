@@ -46,10 +46,46 @@ __device__ __forceinline__ void acc_ah(const cx<T> (&m)[9], T sg, T (&di)[3], cx
     E[2].x += sg * (m[5].x - m[7].x); E[2].y += sg * (m[5].y + m[7].y);
 }
 
-template <typename T, int NE, int PACK, bool GBUF>
-__global__ void __launch_bounds__(FUSED_THREADS, LGF_FUSED_MINB)
+// Delta = D - (1/3) Tr D with D = A - A^dagger given as di = Im A_ii and E = (D01, D02, D12):
+// theta's Tr Delta Delta^dagger and the store of Delta in the packed (4) or full (9) field layout.
+template <typename T, int PACK>
+__device__ __forceinline__ double store_delta(const T (&di)[3], const cx<T> (&E)[3], cx<T> *__restrict__ wout, int64_t V, int64_t s)
+{
+    T d0 = 2 * di[0], d1 = 2 * di[1], d2 = 2 * di[2];
+    const T m = (d0 + d1 + d2) * (T)(1.0 / 3.0);
+    d0 -= m; d1 -= m; d2 -= m;
+    const double th = (double)(d0 * d0 + d1 * d1 + d2 * d2) + 2.0 * (double)(cnorm2(E[0]) + cnorm2(E[1]) + cnorm2(E[2]));
+    if (PACK == 4) {
+        wout[s] = mk<T>(d0, d1);
+        wout[V + s] = E[0];
+        wout[2 * V + s] = E[1];
+        wout[3 * V + s] = E[2];
+    } else {
+        wout[s] = mk<T>(0, d0);
+        wout[V + s] = E[0];
+        wout[2 * V + s] = E[1];
+        wout[3 * V + s] = mk<T>(-E[0].x, E[0].y);
+        wout[4 * V + s] = mk<T>(0, d1);
+        wout[5 * V + s] = E[2];
+        wout[6 * V + s] = mk<T>(-E[1].x, E[1].y);
+        wout[7 * V + s] = mk<T>(-E[2].x, E[2].y);
+        wout[8 * V + s] = mk<T>(0, d2);
+    }
+    return th;
+}
+
+// STORE = false (LGF_OPT_ACCUM_G): `lin` holds the links as loaded, which stay where they are, and
+// `gsrc` the accumulated transformation G(x) (rows 0, 1, updated by the last FFT pass).  The current
+// links G(x) U_mu(x) G^dagger(x+mu) (Alg. 1 lines 12-16 applied n times) are formed in
+// registers exactly as below and measured, but not written: 544 instead of 928 bytes per site
+// (FP64, 12-real).
+#ifndef LGF_ACC_MINB
+#define LGF_ACC_MINB 4
+#endif
+template <typename T, int NE, int PACK, bool GBUF, bool STORE>
+__global__ void __launch_bounds__(FUSED_THREADS, (STORE ? LGF_FUSED_MINB : LGF_ACC_MINB))
 k_update_measure(const cx<T> *__restrict__ lin, cx<T> *__restrict__ lout, const cx<T> *__restrict__ gsrc,
-                 cx<T> *__restrict__ wout, Geom geo, T a, Ctrl *ctrl, double *partials, double2 *hist, double eps)
+                 cx<T> *__restrict__ wout, Geom geo, T a, int gexp, Ctrl *ctrl, double *partials, double2 *hist, double eps)
 {
     if (*(volatile int *)&ctrl->done) return;
     const int64_t V = geo.V;
@@ -69,7 +105,7 @@ k_update_measure(const cx<T> *__restrict__ lin, cx<T> *__restrict__ lout, const 
         for (int nu = 0; nu < 4; nu++) {
             const int64_t sb = s + (c[nu] == 0 ? (int64_t)(geo.N[nu] - 1) : (int64_t)-1) * geo.st[nu];
             cx<T> gb[9], u[9], h[9];
-            load_g01<T, PACK, GBUF>(gsrc, V, sb, a, gb);
+            load_g01<T, PACK, GBUF>(gsrc, V, sb, a, gexp, gb);
             load_link_in<T, NE>(lin, V, nu, sb, u);
             mul_rows<2>(gb, u, h);
             su3_row2(h);
@@ -77,7 +113,7 @@ k_update_measure(const cx<T> *__restrict__ lin, cx<T> *__restrict__ lout, const 
             for (int k = 0; k < 9; k++) X[k] = X[k] + h[k];
         }
         cx<T> g0[9];
-        load_g01<T, PACK, GBUF>(gsrc, V, s, a, g0);
+        load_g01<T, PACK, GBUF>(gsrc, V, s, a, gexp, g0);
         su3_row2(g0);
         T di[3] = {0, 0, 0};
         cx<T> E[3] = {mk<T>(0, 0), mk<T>(0, 0), mk<T>(0, 0)};
@@ -93,39 +129,22 @@ k_update_measure(const cx<T> *__restrict__ lin, cx<T> *__restrict__ lout, const 
         for (int mu = 0; mu < 4; mu++) {
             const int64_t sp = s + (c[mu] == geo.N[mu] - 1 ? -(int64_t)(geo.N[mu] - 1) : (int64_t)1) * geo.st[mu];
             cx<T> g1[9], u[9], t[9], r[9];
-            load_g01<T, PACK, GBUF>(gsrc, V, sp, a, g1);
+            load_g01<T, PACK, GBUF>(gsrc, V, sp, a, gexp, g1);
             su3_row2(g1);
             load_link_in<T, NE>(lin, V, mu, s, u);
             mul_rows<2>(g0, u, t);
             mul_rows_dag<2>(t, g1, r);
             su3_row2(r);
-            cx<T> *p = lout + (int64_t)mu * NE * V + s;
+            if (STORE) {
+                cx<T> *p = lout + (int64_t)mu * NE * V + s;
 #pragma unroll
-            for (int k = 0; k < NE; k++) st_link(p + (int64_t)k * V, r[k]);
+                for (int k = 0; k < NE; k++) st_link(p + (int64_t)k * V, r[k]);
+            }
             tr += r[0].x + r[4].x + r[8].x;
             acc_ah<T>(r, (T)-1, di, E);
         }
         trF = (double)tr;
-        T d0 = 2 * di[0], d1 = 2 * di[1], d2 = 2 * di[2];
-        const T m = (d0 + d1 + d2) * (T)(1.0 / 3.0);
-        d0 -= m; d1 -= m; d2 -= m;
-        th = (double)(d0 * d0 + d1 * d1 + d2 * d2) + 2.0 * (double)(cnorm2(E[0]) + cnorm2(E[1]) + cnorm2(E[2]));
-        if (PACK == 4) {
-            wout[s] = mk<T>(d0, d1);
-            wout[V + s] = E[0];
-            wout[2 * V + s] = E[1];
-            wout[3 * V + s] = E[2];
-        } else {
-            wout[s] = mk<T>(0, d0);
-            wout[V + s] = E[0];
-            wout[2 * V + s] = E[1];
-            wout[3 * V + s] = mk<T>(-E[0].x, E[0].y);
-            wout[4 * V + s] = mk<T>(0, d1);
-            wout[5 * V + s] = E[2];
-            wout[6 * V + s] = mk<T>(-E[1].x, E[1].y);
-            wout[7 * V + s] = mk<T>(-E[2].x, E[2].y);
-            wout[8 * V + s] = mk<T>(0, d2);
-        }
+        th = store_delta<T, PACK>(di, E, wout, V, s);
     }
     finish_measure<FUSED_THREADS>(trF, th, V, ctrl, partials, hist, eps, 1);
 }
@@ -137,8 +156,8 @@ void launch_update_measure(const SiteArgs &a, const void *lin, void *lout, const
 {
     const int nb = fused_blocks(a.geo.V);
 #define CALL(T, NE, PACK, GB) \
-    k_update_measure<T, NE, PACK, GB><<<nb, FUSED_THREADS, 0, st>>>((const cx<T> *)lin, (cx<T> *)lout, (const cx<T> *)gsrc, \
-        (cx<T> *)wout, a.geo, (T)(alpha / 2.0), a.ctrl, a.partials, a.hist, eps)
+    k_update_measure<T, NE, PACK, GB, true><<<nb, FUSED_THREADS, 0, st>>>((const cx<T> *)lin, (cx<T> *)lout, (const cx<T> *)gsrc, \
+        (cx<T> *)wout, a.geo, (T)(alpha / 2.0), a.gexp, a.ctrl, a.partials, a.hist, eps)
 #define CALL_NE(T, NE)                                           \
     do {                                                         \
         if (gbuf) { CALL(T, NE, 4, true); }                      \
@@ -148,6 +167,17 @@ void launch_update_measure(const SiteArgs &a, const void *lin, void *lout, const
     if (a.prec == 0) { if (a.recon == 12) CALL_NE(double, 6); else CALL_NE(double, 9); }
     else             { if (a.recon == 12) CALL_NE(float, 6); else CALL_NE(float, 9); }
 #undef CALL_NE
+#undef CALL
+}
+
+void launch_measure_acc(const SiteArgs &a, const void *gacc, double eps, cudaStream_t st)
+{
+    const int nb = fused_blocks(a.geo.V);
+#define CALL(T, NE) \
+    k_update_measure<T, NE, 4, true, false><<<nb, FUSED_THREADS, 0, st>>>((const cx<T> *)a.links, (cx<T> *)nullptr, \
+        (const cx<T> *)gacc, (cx<T> *)a.w, a.geo, (T)0, 0, a.ctrl, a.partials, a.hist, eps)
+    if (a.prec == 0) { if (a.recon == 12) CALL(double, 6); else CALL(double, 9); }
+    else             { if (a.recon == 12) CALL(float, 6); else CALL(float, 9); }
 #undef CALL
 }
 

@@ -85,7 +85,7 @@ __global__ void k_ctrl_reset(Ctrl *ctrl, double2 *hist, double eps)
 // With 12-real storage only rows 0, 1 of g U g^dagger are computed and stored (reading R15).
 template <typename T, int NE, int PACK>
 __global__ void __launch_bounds__(SITE_THREADS)
-k_update(cx<T> *__restrict__ links, const cx<T> *__restrict__ w, Geom geo, T a, const Ctrl *ctrl)
+k_update(cx<T> *__restrict__ links, const cx<T> *__restrict__ w, Geom geo, T a, int gexp, const Ctrl *ctrl)
 {
     if (*(volatile const int *)&ctrl->done) return;
     const int64_t V = geo.V;
@@ -94,13 +94,13 @@ k_update(cx<T> *__restrict__ links, const cx<T> *__restrict__ w, Geom geo, T a, 
     int c[4];
     site_coords(geo, s, c);
     cx<T> g0[9];
-    build_g<T, PACK>(w, V, s, a, g0);
+    build_g<T, PACK>(w, V, s, a, gexp, g0);
     constexpr int R = (NE == 6) ? 2 : 3;
 #pragma unroll
     for (int mu = 0; mu < 4; mu++) {
         const int64_t sp = s + (c[mu] == geo.N[mu] - 1 ? -(int64_t)(geo.N[mu] - 1) : (int64_t)1) * geo.st[mu];
         cx<T> g1[9], u[9], t[9], r[9];
-        build_g<T, PACK>(w, V, sp, a, g1);
+        build_g<T, PACK>(w, V, sp, a, gexp, g1);
         load_link<T, NE>(links, V, mu, s, u);
         mul_rows<R>(g0, u, t);
         mul_rows_dag<R>(t, g1, r);
@@ -108,6 +108,47 @@ k_update(cx<T> *__restrict__ links, const cx<T> *__restrict__ w, Geom geo, T a, 
 #pragma unroll
         for (int k = 0; k < NE; k++) p[(int64_t)k * V] = r[k];
     }
+}
+
+// ------------------------------------------------------------------ ACCUM_G: apply the accumulated G
+// U_mu(x) <- G(x) U_mu(x) G^dagger(x+mu) in place, from the rows 0, 1 of G kept in the g buffer
+// (LGF_OPT_ACCUM_G; the same product as k_update, Alg. 1 lines 12-16, with the
+// accumulated transformation in place of one iteration's g).  Each thread rewrites only its own
+// four links and G is read-only here; k_g_identity resets it afterwards.
+template <typename T, int NE>
+__global__ void __launch_bounds__(SITE_THREADS)
+k_apply_g(cx<T> *__restrict__ links, const cx<T> *__restrict__ gacc, Geom geo)
+{
+    const int64_t V = geo.V;
+    const int64_t s = (int64_t)blockIdx.x * SITE_THREADS + threadIdx.x;
+    if (s >= V) return;
+    int c[4];
+    site_coords(geo, s, c);
+    cx<T> g0[9];
+    load_g01<T, 4, true>(gacc, V, s, (T)0, 0, g0);
+    su3_row2(g0);
+    constexpr int R = (NE == 6) ? 2 : 3;
+#pragma unroll
+    for (int mu = 0; mu < 4; mu++) {
+        const int64_t sp = s + (c[mu] == geo.N[mu] - 1 ? -(int64_t)(geo.N[mu] - 1) : (int64_t)1) * geo.st[mu];
+        cx<T> g1[9], u[9], t[9], r[9];
+        load_g01<T, 4, true>(gacc, V, sp, (T)0, 0, g1);
+        su3_row2(g1);
+        load_link<T, NE>(links, V, mu, s, u);
+        mul_rows<R>(g0, u, t);
+        mul_rows_dag<R>(t, g1, r);
+        cx<T> *p = links + (int64_t)mu * NE * V + s;
+#pragma unroll
+        for (int k = 0; k < NE; k++) p[(int64_t)k * V] = r[k];
+    }
+}
+
+template <typename T> __global__ void k_g_identity(cx<T> *__restrict__ gacc, int64_t V)
+{
+    const int64_t s = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (s >= V) return;
+#pragma unroll
+    for (int k = 0; k < 6; k++) gacc[(int64_t)k * V + s] = mk<T>((k == 0 || k == 4) ? (T)1 : (T)0, (T)0);
 }
 
 // ------------------------------------------------------------------ layout conversions and taps
@@ -139,14 +180,14 @@ __global__ void k_soa_to_aos(cx<T> *__restrict__ aos, const cx<T> *__restrict__ 
 }
 
 template <typename T, int PACK>
-__global__ void k_field_get(const cx<T> *__restrict__ w, int64_t V, int which, T a, cx<T> *__restrict__ aos, int64_t s0, int64_t count)
+__global__ void k_field_get(const cx<T> *__restrict__ w, int64_t V, int which, T a, int gexp, cx<T> *__restrict__ aos, int64_t s0, int64_t count)
 {
     const int64_t sl = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (sl >= count) return;
     const int64_t s = s0 + sl;
     cx<T> m[9];
     if (which == 2) {
-        build_g<T, PACK>(w, V, s, a, m);
+        build_g<T, PACK>(w, V, s, a, gexp, m);
     } else if (PACK == 9) {
 #pragma unroll
         for (int k = 0; k < 9; k++) m[k] = w[(int64_t)k * V + s];
@@ -205,9 +246,25 @@ void launch_update(const SiteArgs &a, double alpha, cudaStream_t st)
 {
     const int nb = measure_blocks(a.geo.V);
 #define CALL(T, NE, PACK) \
-    k_update<T, NE, PACK><<<nb, SITE_THREADS, 0, st>>>((cx<T> *)a.links, (const cx<T> *)a.w, a.geo, (T)(alpha / 2.0), a.ctrl)
+    k_update<T, NE, PACK><<<nb, SITE_THREADS, 0, st>>>((cx<T> *)a.links, (const cx<T> *)a.w, a.geo, (T)(alpha / 2.0), a.gexp, a.ctrl)
     LGF_DISPATCH(CALL);
 #undef CALL
+}
+
+void launch_apply_g(const SiteArgs &a, const void *gacc, cudaStream_t st)
+{
+    const int nb = measure_blocks(a.geo.V);
+#define CALL(T, NE, PACK) \
+    k_apply_g<T, NE><<<nb, SITE_THREADS, 0, st>>>((cx<T> *)a.links, (const cx<T> *)gacc, a.geo)
+    LGF_DISPATCH(CALL);
+#undef CALL
+}
+
+void launch_g_identity(const SiteArgs &a, void *gacc, cudaStream_t st)
+{
+    const int nb = (int)((a.geo.V + 255) / 256);
+    if (a.prec == 0) k_g_identity<double><<<nb, 256, 0, st>>>((cx<double> *)gacc, a.geo.V);
+    else k_g_identity<float><<<nb, 256, 0, st>>>((cx<float> *)gacc, a.geo.V);
 }
 
 void launch_ctrl_reset(const SiteArgs &a, double eps, cudaStream_t st)
@@ -237,7 +294,7 @@ void launch_field_get(const SiteArgs &a, int which, double alpha, void *aos, int
 {
     const int nb = (int)((count + 255) / 256);
 #define CALL(T, NE, PACK) \
-    k_field_get<T, PACK><<<nb, 256, 0, st>>>((const cx<T> *)a.w, a.geo.V, which, (T)(alpha / 2.0), (cx<T> *)aos, s0, count)
+    k_field_get<T, PACK><<<nb, 256, 0, st>>>((const cx<T> *)a.w, a.geo.V, which, (T)(alpha / 2.0), a.gexp, (cx<T> *)aos, s0, count)
     LGF_DISPATCH(CALL);
 #undef CALL
 }

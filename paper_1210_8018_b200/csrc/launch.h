@@ -14,6 +14,7 @@ struct SiteArgs {
     int prec;           // 0 = FP64, 1 = FP32
     int recon;          // 18 or 12
     int pack;           // 4 or 9
+    int gexp;           // LGF_OPT_GMAP: 0 first order + reunitarisation, 1 exact exponential
 };
 
 // kernel (a): Delta, F, theta (eq. 1.5, 1.1, 1.4).  eps < 0: never raise `done`.
@@ -26,6 +27,12 @@ void launch_update(const SiteArgs &a, double alpha, cudaStream_t st);
 void launch_update_measure(const SiteArgs &a, const void *lin, void *lout, const void *gsrc, int gbuf, void *wout,
                            double alpha, double eps, cudaStream_t st);
 int fused_blocks(int64_t V);
+// ACCUM_G (fixed links, accumulated transformation G in the g buffer, rows 0, 1):
+// Delta, F, theta of G(x) U_mu(x) G^dagger(x+mu) -> a.w; counts one iteration
+void launch_measure_acc(const SiteArgs &a, const void *gacc, double eps, cudaStream_t st);
+// a.links <- G U G^dagger in place; then G <- 1
+void launch_apply_g(const SiteArgs &a, const void *gacc, cudaStream_t st);
+void launch_g_identity(const SiteArgs &a, void *gacc, cudaStream_t st);
 // iter = 0, hist[0] = (F, theta), done = (theta <= eps)
 void launch_ctrl_reset(const SiteArgs &a, double eps, cudaStream_t st);
 
@@ -54,7 +61,8 @@ bool fft_tiled_supported(const int N[4], int prec);
 bool fft_tiled_gbuf_supported(const int N[4], int prec); // pass 2 with the g build fits in shared memory
 void launch_fft_tiled(const FftArgs &a, int which, cudaStream_t st);
 // pass 2 of all 4 packed fields with g(x) = reunit(1 + (alpha/2) w(x)) as its epilogue: rows 0, 1 of g -> gbuf
-void launch_fft_tiled_inv_g(const FftArgs &a, void *gbuf, double alpha, cudaStream_t st);
+// accum = 1: gbuf holds the accumulated G and receives reunit(g G) instead (LGF_OPT_ACCUM_G)
+void launch_fft_tiled_inv_g(const FftArgs &a, void *gbuf, double alpha, int gexp, int accum, cudaStream_t st);
 int fft_tiled_setup(const int N[4], int prec); // sets kernel attributes (smem opt-in); 0 on success
 
 } // namespace lgf

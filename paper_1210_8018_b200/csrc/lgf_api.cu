@@ -35,7 +35,8 @@ struct lgf_ctx {
     int N[4];
     int64_t V;
     int prec;
-    int recon = 18, pack = 4, check_interval = 8, fft_path = 0, profile = 0, fusion = 1, l2_persist = 0;
+    int recon = 18, pack = 4, check_interval = 8, fft_path = 0, profile = 0, fusion = 1, l2_persist = 0, gmap = 0, accum = 0;
+    bool acc_dirty = false;  // ACCUM_G: the g buffer holds a G != 1 that the links do not yet include
     bool l2_window = false;  // an access-policy window is set on the bound stream
     int cur = 0, wcur = 0;   // which of the two link / field buffers is current
     bool use_gbuf = false;   // last FFT pass writes g (fusion, tiled FFT, 4 packed fields)
@@ -73,7 +74,8 @@ Layout make_layout(const lgf_ctx *c)
     // fusion: links are double-buffered (the fused kernel reads old neighbours while new links
     // are written); the fields are double-buffered when g is rebuilt from w inside that kernel,
     // else the last FFT pass writes rows 0, 1 of g (6 complex per site) to gbuf
-    const int nl = c->fusion ? 2 : 1;
+    // ACCUM_G: the links are not rewritten per iteration, so one buffer; the g buffer holds G
+    const int nl = (c->fusion && !c->accum) ? 2 : 1;
     const bool gb = c->fusion && c->pack == 4 && c->fft_path == 0 && fft_tiled_gbuf_supported(c->N, c->prec);
     const int nw = (c->fusion && !gb) ? 2 : 1;
     for (int i = 0; i < 2; i++) { L.links[i] = off; if (i < nl) off = align_up(off + (size_t)4 * ne * c->V * e, 256); }
@@ -180,9 +182,31 @@ void do_update(lgf_ctx *c, double alpha)
     c->wstate = 0;
 }
 
+// ACCUM_G: bring the links up to date, U <- G U G^dagger, G <- 1.  The field buffer keeps the Delta of
+// these links (wstate unchanged).  No-op when nothing is pending.
+void materialise(lgf_ctx *c)
+{
+    if (!c->accum || !c->acc_dirty) return;
+    run_kernel(c, LGF_KERNEL_APPLY_G, 2, [&] {
+        launch_apply_g(c->sa, c->gbuf, c->st);
+        launch_g_identity(c->sa, c->gbuf, c->st);
+    });
+    c->acc_dirty = false;
+}
+
 // one execution of the loop body of Algorithm 1 (lines 3-17) on the device
 void do_iteration(lgf_ctx *c, double alpha, double eps)
 {
+    if (c->accum) {
+        // w_buf[0] holds Delta of G U G^dagger; the last FFT pass turns it into g and G <- g G
+        run_kernel(c, LGF_KERNEL_FFT_XY_FWD, 1, [&] { launch_fft_tiled(c->fa, 0, c->st); });
+        run_kernel(c, LGF_KERNEL_FFT_ZT, 1, [&] { launch_fft_tiled(c->fa, 1, c->st); });
+        run_kernel(c, LGF_KERNEL_FFT_XY_INV_GACC, 1, [&] { launch_fft_tiled_inv_g(c->fa, c->gbuf, alpha, c->gmap, 1, c->st); });
+        run_kernel(c, LGF_KERNEL_MEASURE_ACC, 1, [&] { launch_measure_acc(c->sa, c->gbuf, eps, c->st); });
+        c->acc_dirty = true;
+        c->wstate = 1;
+        return;
+    }
     if (!c->fusion) {
         do_fourier(c);
         do_update(c, alpha);
@@ -194,7 +218,7 @@ void do_iteration(lgf_ctx *c, double alpha, double eps)
     if (c->use_gbuf) {
         run_kernel(c, LGF_KERNEL_FFT_XY_FWD, 1, [&] { launch_fft_tiled(c->fa, 0, c->st); });
         run_kernel(c, LGF_KERNEL_FFT_ZT, 1, [&] { launch_fft_tiled(c->fa, 1, c->st); });
-        run_kernel(c, LGF_KERNEL_FFT_XY_INV_G, 1, [&] { launch_fft_tiled_inv_g(c->fa, c->gbuf, alpha, c->st); });
+        run_kernel(c, LGF_KERNEL_FFT_XY_INV_G, 1, [&] { launch_fft_tiled_inv_g(c->fa, c->gbuf, alpha, c->gmap, 0, c->st); });
         run_kernel(c, LGF_KERNEL_UPDATE_MEASURE, 1,
                    [&] { launch_update_measure(c->sa, lin, lout, c->gbuf, 1, c->w_buf[c->wcur], alpha, eps, c->st); });
     } else {
@@ -213,7 +237,7 @@ void do_iteration(lgf_ctx *c, double alpha, double eps)
 // current buffers are those of the `executed`-th iteration since `cur0` / `wcur0`.
 void settle_buffers(lgf_ctx *c, int cur0, int wcur0, long long executed)
 {
-    if (!c->fusion) return;
+    if (!c->fusion || c->accum) return;
     c->cur = cur0 ^ (int)(executed & 1);
     if (!c->use_gbuf) c->wcur = wcur0 ^ (int)(executed & 1);
     sync_ptrs(c);
@@ -317,7 +341,7 @@ int lgf_set_option(lgf_ctx *ctx, int key, int64_t value)
 {
     if (!ctx) return LGF_ERR_INVALID_ARG;
     const bool layout_key = (key == LGF_OPT_RECON || key == LGF_OPT_FFT_BATCH || key == LGF_OPT_FFT_PATH || key == LGF_OPT_FUSION ||
-                             key == LGF_OPT_L2_PERSIST);
+                             key == LGF_OPT_L2_PERSIST || key == LGF_OPT_ACCUM_G);
     if (layout_key && ctx->bound) return fail(ctx, LGF_ERR_INVALID_ARG, "this option must be set before lgf_bind");
     switch (key) {
     case LGF_OPT_RECON:
@@ -341,6 +365,12 @@ int lgf_set_option(lgf_ctx *ctx, int key, int64_t value)
     case LGF_OPT_L2_PERSIST:
         if (value != 0 && value != 1) return fail(ctx, LGF_ERR_INVALID_ARG, "L2_PERSIST must be 0 or 1");
         ctx->l2_persist = (int)value; break;
+    case LGF_OPT_GMAP:
+        if (value != 0 && value != 1) return fail(ctx, LGF_ERR_INVALID_ARG, "GMAP must be 0 or 1");
+        ctx->gmap = (int)value; ctx->sa.gexp = ctx->gmap; break;
+    case LGF_OPT_ACCUM_G:
+        if (value != 0 && value != 1) return fail(ctx, LGF_ERR_INVALID_ARG, "ACCUM_G must be 0 or 1");
+        ctx->accum = (int)value; break;
     case LGF_OPT_PROFILE:
         if (ctx->bound) flush_events(ctx);
         ctx->profile = value ? 1 : 0; break;
@@ -361,6 +391,8 @@ int lgf_bind(lgf_ctx *ctx, void *dev_workspace, size_t bytes, void *cuda_stream)
     if (!ctx) return LGF_ERR_INVALID_ARG;
     if (!dev_workspace) return fail(ctx, LGF_ERR_INVALID_ARG, "dev_workspace is NULL");
     if (((uintptr_t)dev_workspace) & 255) return fail(ctx, LGF_ERR_INVALID_ARG, "dev_workspace must be 256-byte aligned");
+    if (ctx->accum && !(ctx->fusion && ctx->pack == 4 && ctx->fft_path == 0 && fft_tiled_gbuf_supported(ctx->N, ctx->prec)))
+        return fail(ctx, LGF_ERR_INVALID_ARG, "ACCUM_G needs FUSION = 1, FFT_BATCH = 4 and a lattice the tiled FFT covers");
     const Layout L = make_layout(ctx);
     if (bytes < L.total) return fail(ctx, LGF_ERR_WORKSPACE_TOO_SMALL, "workspace smaller than lgf_workspace_bytes()");
     ctx->lay = L;
@@ -378,7 +410,7 @@ int lgf_bind(lgf_ctx *ctx, void *dev_workspace, size_t bytes, void *cuda_stream)
     s.partials = (double *)(ctx->base + L.partials);
     s.ctrl = (Ctrl *)(ctx->base + L.ctrl);
     s.hist = (double2 *)(ctx->base + L.hist);
-    s.prec = ctx->prec; s.recon = ctx->recon; s.pack = ctx->pack;
+    s.prec = ctx->prec; s.recon = ctx->recon; s.pack = ctx->pack; s.gexp = ctx->gmap;
     FftArgs &f = ctx->fa;
     f.geo = g; f.nfields = ctx->pack; f.prec = ctx->prec;
     sync_ptrs(ctx);
@@ -411,6 +443,7 @@ int lgf_bind(lgf_ctx *ctx, void *dev_workspace, size_t bytes, void *cuda_stream)
     ctx->use_gbuf = ctx->fusion && ctx->tiled && ctx->pack == 4 && fft_tiled_gbuf_supported(ctx->N, ctx->prec);
     l2_window_clear(ctx);
     if (ctx->use_gbuf) l2_window_set(ctx);   // one field buffer, used in place by every pass
+    ctx->acc_dirty = false;
     ctx->bound = true;
     ctx->loaded = false;
     ctx->wstate = 0;
@@ -434,6 +467,10 @@ int lgf_load_links(lgf_ctx *ctx, const void *src, int src_is_device, int src_lay
             run_kernel(ctx, LGF_KERNEL_LAYOUT, 1, [&] { launch_aos_to_soa(ctx->sa, stg, s0, n, ctx->st); });
         }
     }
+    if (ctx->accum) {
+        run_kernel(ctx, LGF_KERNEL_APPLY_G, 1, [&] { launch_g_identity(ctx->sa, ctx->gbuf, ctx->st); });
+        ctx->acc_dirty = false;
+    }
     int rc = clear_done(ctx);
     if (rc) return rc;
     do_measure(ctx, -1.0, 0);
@@ -449,6 +486,7 @@ int lgf_get_links(lgf_ctx *ctx, void *dst, int dst_is_device, int dst_layout)
     if (rc) return rc;
     if (!dst) return fail(ctx, LGF_ERR_INVALID_ARG, "dst is NULL");
     if (dst_layout != LGF_LAYOUT_AOS) return fail(ctx, LGF_ERR_INVALID_ARG, "unknown layout");
+    materialise(ctx);
     const size_t e = elem_bytes(ctx);
     if (dst_is_device) {
         run_kernel(ctx, LGF_KERNEL_LAYOUT, 1, [&] { launch_soa_to_aos(ctx->sa, dst, 0, ctx->V, ctx->st); });
@@ -470,6 +508,7 @@ int lgf_measure(lgf_ctx *ctx, double *F, double *theta)
     int rc = need_loaded(ctx);
     if (rc) return rc;
     if ((rc = clear_done(ctx))) return rc;
+    materialise(ctx);
     do_measure(ctx, -1.0, 0);
     Ctrl h;
     if ((rc = read_ctrl(ctx, &h))) return rc;
@@ -485,6 +524,7 @@ int lgf_iterate(lgf_ctx *ctx, double alpha, int64_t n, lgf_result *out)
     if (n < 0) return fail(ctx, LGF_ERR_INVALID_ARG, "n must be >= 0");
     if (ctx->wstate != 1) {
         if ((rc = clear_done(ctx))) return rc;
+        materialise(ctx);
         do_measure(ctx, -1.0, 0);
     }
     run_kernel(ctx, LGF_KERNEL_LAYOUT, 1, [&] { launch_ctrl_reset(ctx->sa, -1.0, ctx->st); });
@@ -508,6 +548,7 @@ int lgf_fix(lgf_ctx *ctx, double alpha, double eps, lgf_result *out)
     if (!(eps >= 0)) return fail(ctx, LGF_ERR_INVALID_ARG, "eps must be >= 0");
     if (ctx->wstate != 1) {
         if ((rc = clear_done(ctx))) return rc;
+        materialise(ctx);
         do_measure(ctx, -1.0, 0);
     }
     run_kernel(ctx, LGF_KERNEL_LAYOUT, 1, [&] { launch_ctrl_reset(ctx->sa, eps, ctx->st); });
@@ -535,6 +576,7 @@ int lgf_stage(lgf_ctx *ctx, int stage, double alpha)
     int rc = need_loaded(ctx);
     if (rc) return rc;
     if ((rc = clear_done(ctx))) return rc;
+    materialise(ctx);
     switch (stage) {
     case LGF_STAGE_MEASURE: do_measure(ctx, -1.0, 0); break;
     case LGF_STAGE_FOURIER:
@@ -580,6 +622,7 @@ int lgf_set_field(lgf_ctx *ctx, int which, const void *src, int src_is_device)
     if (rc) return rc;
     if (!src) return fail(ctx, LGF_ERR_INVALID_ARG, "src is NULL");
     if (which != LGF_FIELD_DELTA && which != LGF_FIELD_W) return fail(ctx, LGF_ERR_INVALID_ARG, "only DELTA and W can be set");
+    materialise(ctx);
     const size_t e = elem_bytes(ctx);
     if (src_is_device) {
         run_kernel(ctx, LGF_KERNEL_LAYOUT, 1, [&] { launch_field_set(ctx->sa, src, 0, ctx->V, ctx->st); });
@@ -643,6 +686,15 @@ int lgf_reset_counters(lgf_ctx *ctx)
 
 int lgf_uses_tiled_fft(const lgf_ctx *ctx) { return ctx && ctx->tiled ? 1 : 0; }
 int lgf_uses_gbuf(const lgf_ctx *ctx) { return ctx && ctx->bound && ctx->use_gbuf ? 1 : 0; }
+
+int lgf_sync_links(lgf_ctx *ctx)
+{
+    int rc = need_loaded(ctx);
+    if (rc) return rc;
+    materialise(ctx);
+    CK(cudaGetLastError());
+    return LGF_OK;
+}
 
 const char *lgf_last_error(const lgf_ctx *ctx) { return ctx ? ctx->err.c_str() : g_create_err.c_str(); }
 

@@ -19,16 +19,18 @@ ERR_WORKSPACE_TOO_SMALL, ERR_CUDA, ERR_NOT_CONVERGED, ERR_NUMERIC = -5, -6, -7, 
 PREC_FP64, PREC_FP32 = 0, 1
 LAYOUT_AOS = 0
 OPT_RECON, OPT_FFT_BATCH, OPT_MAX_ITER, OPT_CHECK_INTERVAL, OPT_FFT_PATH, OPT_PROFILE, OPT_FUSION, OPT_L2_PERSIST = 1, 2, 3, 4, 5, 6, 7, 8
+OPT_GMAP, OPT_ACCUM_G = 9, 10
+GMAP_FIRST_ORDER, GMAP_EXP = 0, 1
 FIELD_DELTA, FIELD_W, FIELD_G = 0, 1, 2
 STAGE_MEASURE, STAGE_FOURIER, STAGE_UPDATE = 0, 1, 2
 KERNEL_NAMES = ["measure", "fft_xy_fwd", "fft_zt", "fft_xy_inv", "update", "fft_generic", "layout", "fft_xy_inv_g",
-                "update_measure"]
+                "update_measure", "fft_xy_inv_gacc", "measure_acc", "apply_g"]
 
 #: every symbol include/lgf.h declares
 SYMBOLS = [
     "lgf_create", "lgf_set_option", "lgf_workspace_bytes", "lgf_bind", "lgf_load_links", "lgf_get_links",
     "lgf_measure", "lgf_iterate", "lgf_fix", "lgf_stage", "lgf_get_field", "lgf_set_field", "lgf_history",
-    "lgf_kernel_time", "lgf_launch_count", "lgf_reset_counters", "lgf_uses_tiled_fft", "lgf_uses_gbuf", "lgf_last_error",
+    "lgf_kernel_time", "lgf_launch_count", "lgf_reset_counters", "lgf_uses_tiled_fft", "lgf_uses_gbuf", "lgf_sync_links", "lgf_last_error",
     "lgf_destroy",
 ]
 
@@ -79,6 +81,7 @@ def lib():
     L.lgf_reset_counters.argtypes = [vp]
     L.lgf_uses_tiled_fft.argtypes = [vp]
     L.lgf_uses_gbuf.argtypes = [vp]
+    L.lgf_sync_links.argtypes = [vp]
     L.lgf_last_error.argtypes = [vp]
     L.lgf_last_error.restype = ctypes.c_char_p
     L.lgf_destroy.argtypes = [vp]
@@ -99,7 +102,8 @@ class GaugeFixer:
     torch complex tensors of the same shapes."""
 
     def __init__(self, N, precision="fp64", recon=18, fft_batch=4, fft_path=0, device="cuda:0",
-                 stream=None, max_iter=None, check_interval=None, profile=False, fusion=None, l2_persist=None):
+                 stream=None, max_iter=None, check_interval=None, profile=False, fusion=None, l2_persist=None, gmap=None,
+                 accum_g=None):
         import torch
 
         self.torch = torch
@@ -120,6 +124,10 @@ class GaugeFixer:
             self.set_option(OPT_FUSION, fusion)
         if l2_persist is not None:
             self.set_option(OPT_L2_PERSIST, l2_persist)
+        if gmap is not None:
+            self.set_option(OPT_GMAP, gmap)
+        if accum_g is not None:
+            self.set_option(OPT_ACCUM_G, accum_g)
         if max_iter is not None:
             self.set_option(OPT_MAX_ITER, max_iter)
         if check_interval is not None:
@@ -250,6 +258,9 @@ class GaugeFixer:
 
     def uses_gbuf(self):
         return bool(self.L.lgf_uses_gbuf(self.ctx))
+
+    def sync_links(self):
+        self._ck(self.L.lgf_sync_links(self.ctx))
 
     def synchronize(self):
         self.stream.synchronize()

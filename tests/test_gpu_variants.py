@@ -1,0 +1,245 @@
+"""GPU parity of the two SURVEY 8(f) variants of the hot path, through the C ABI, against the oracle:
+
+  LGF_OPT_ACCUM_G (f1): the loaded links stay fixed and the accumulated transformation G(x) is
+      carried instead; the same iteration as Alg. 1 lines 12-16 up to rounding, so
+      the tolerances are those of the default path (BASELINE.json north_star).
+  LGF_OPT_GMAP = 1 (f4): g = exp((alpha/2) w), eq. 1.2 as written; the oracle side is
+      oracle.build_g_exp / oracle.set_exponential, pinned in tests/test_oracle_pins.py.
+"""
+import numpy as np
+import pytest
+
+import gen
+import oracle
+from test_golden import golden_path, read_golden
+
+pytestmark = pytest.mark.gpu
+
+ALPHA = 0.08
+
+
+@pytest.fixture(scope="module")
+def lgf(cuda_device):
+    from paper_1210_8018_b200 import lgf as m
+
+    m.lib()
+    return m
+
+
+@pytest.fixture
+def exp_oracle():
+    oracle.set_exponential(True)
+    yield
+    oracle.set_exponential(False)
+
+
+ACC_LATTICES = [
+    ((8, 8, 8, 8), 0.3, gen.BASE_SEED + 8),
+    ((12, 12, 12, 12), 0.5, 79),
+    ((16, 16, 16, 16), 0.5, gen.BASE_SEED + 16),
+    ((32, 32, 32, 8), 0.5, 81),           # one of the paper's 32^3 x n lattices
+    ((64, 64, 8, 8), 0.5, 1234),          # 64^2 FP64 planes: the 2-CTA cluster version of the last pass
+]
+
+
+def lid(v):
+    return "x".join(map(str, v[0]))
+
+
+# ------------------------------------------------------------------ ACCUM_G
+@pytest.mark.parametrize("lat", ACC_LATTICES, ids=lid)
+@pytest.mark.parametrize("recon", [18, 12])
+def test_accum_g_iterations_match_oracle(lgf, lat, recon):
+    """1 and then 3 more iterations: links (rewritten on demand), F, theta and the history."""
+    N, sigma, seed = lat
+    U = gen.gen_links(N, sigma, seed)
+    Uo = U.copy()
+    hist = oracle.iterate(N, Uo, ALPHA, 1)
+    gf = lgf.GaugeFixer(N, recon=recon, accum_g=1)
+    gf.load_links(U)
+    r = gf.iterate(ALPHA, 1)
+    assert r.iterations == 1
+    assert abs(r.F - hist[1, 0]) <= 1e-10 * abs(hist[1, 0])
+    assert abs(r.theta - hist[1, 1]) <= 1e-10 * hist[1, 1]
+    assert np.abs(gf.get_links() - Uo).max() < 1e-12
+    # carry on from the rewritten links (G was reset to 1), three iterations with G accumulating
+    hist3 = oracle.iterate(N, Uo, ALPHA, 3)
+    r = gf.iterate(ALPHA, 3)
+    assert r.iterations == 3
+    assert np.allclose(gf.history(), hist3, rtol=1e-9, atol=0)
+    assert np.abs(gf.get_links() - Uo).max() < 1e-11
+    # a plain measure of the rewritten links agrees with what the accumulated path reported
+    F, th = gf.measure()
+    assert abs(F - r.F) <= 1e-12 and abs(th - r.theta) <= 1e-10 * r.theta
+    gf.close()
+
+
+@pytest.mark.parametrize("n,sigma,seed", [(8, 0.3, gen.BASE_SEED + 8), (8, 0.3, gen.BASE_SEED + 1008),
+                                          (16, 0.5, gen.BASE_SEED + 16)])
+@pytest.mark.parametrize("recon", [18, 12])
+def test_accum_g_convergence_matches_golden(lgf, n, sigma, seed, recon):
+    it, F, th, hist = read_golden(golden_path(n, seed))
+    U = gen.gen_links(n, sigma, seed)
+    gf = lgf.GaugeFixer(n, recon=recon, accum_g=1)
+    gf.load_links(U)
+    r = gf.fix(ALPHA, 1e-15)
+    assert r.converged == 1 and r.theta <= 1e-15
+    assert abs(r.iterations - it) <= 0.02 * it
+    assert abs(r.F - F) <= 1e-10
+    h = gf.history()
+    assert h.shape[0] == r.iterations + 1
+    k = min(h.shape[0], hist.shape[0]) - 3
+    assert np.allclose(h[:k, 0], hist[:k, 0], rtol=0, atol=1e-10)
+    assert np.allclose(h[:k, 1], hist[:k, 1], rtol=1e-6, atol=1e-25)
+    assert np.all(np.diff(h[:, 0]) >= -1e-15)
+    Ufix = gf.get_links()
+    I = np.eye(3)
+    assert np.abs(Ufix @ np.conj(np.swapaxes(Ufix, -1, -2)) - I).max() < 1e-12
+    assert np.abs(np.linalg.det(Ufix) - 1).max() < 1e-12
+    if n == 8:
+        assert abs(oracle.plaquette(n, Ufix) - oracle.plaquette(n, U)) < 1e-12
+        # the fixed links agree with the oracle's fixed links (same gauge orbit, same minimum)
+        Uo = U.copy()
+        oracle.fix(n, Uo, ALPHA, 1e-15)
+        assert np.abs(Ufix - Uo).max() < 1e-9
+    r2 = gf.fix(ALPHA, 1e-15)
+    assert r2.iterations == 0 and r2.converged == 1
+    gf.close()
+
+
+def test_accum_g_equals_default_path_and_stops_cleanly(lgf):
+    """Same trajectory as the default path; kernels launched after convergence leave G alone."""
+    n, seed = 8, gen.BASE_SEED + 2008
+    U = gen.gen_links(n, 0.3, seed)
+    a = lgf.GaugeFixer(n, recon=12)
+    b = lgf.GaugeFixer(n, recon=12, accum_g=1, check_interval=64)   # many launches after `done`
+    a.load_links(U)
+    b.load_links(U)
+    ra, rb = a.fix(ALPHA, 1e-15), b.fix(ALPHA, 1e-15)
+    assert ra.iterations == rb.iterations
+    assert abs(ra.F - rb.F) < 1e-13
+    assert np.abs(a.get_links() - b.get_links()).max() < 1e-11
+    Fb, thb = b.measure()
+    assert abs(Fb - rb.F) < 1e-13 and thb <= 2e-15
+    a.close()
+    b.close()
+
+
+def test_accum_g_fp32(lgf):
+    N, sigma, seed = (16, 16, 16, 16), 0.5, gen.BASE_SEED + 16
+    U = gen.gen_links(N, sigma, seed)
+    U32 = U.astype(np.complex64)
+    Uo = U32.astype(np.complex128)
+    hist = oracle.iterate(N, Uo, ALPHA, 1)
+    gf = lgf.GaugeFixer(N, precision="fp32", recon=12, accum_g=1)
+    gf.load_links(U32)
+    r = gf.iterate(ALPHA, 1)
+    assert np.abs(gf.get_links().astype(np.complex128) - Uo).max() < 1e-5
+    assert abs(r.theta - hist[1, 1]) <= 1e-4 * hist[1, 1]
+    gf.load_links(U32)
+    r = gf.fix(ALPHA, 1e-12)
+    assert r.converged == 1 and r.theta <= 1e-12
+    gf.close()
+
+
+def test_accum_g_needs_the_tiled_packed_path(lgf):
+    for kw in (dict(fft_batch=9), dict(fft_path=1), dict(fusion=0)):
+        with pytest.raises(lgf.LgfError) as e:
+            lgf.GaugeFixer(8, accum_g=1, **kw)
+        assert e.value.code == lgf.ERR_INVALID_ARG
+    with pytest.raises(lgf.LgfError):
+        lgf.GaugeFixer((4, 6, 8, 12), accum_g=1)           # generic FFT lattice
+
+
+def test_accum_g_headline_32_12real(lgf):
+    """BASELINE config 3 in the ACCUM_G launch configuration bench.py times."""
+    n, seed = 32, gen.BASE_SEED + 32
+    U = gen.gen_links(n, 0.5, seed)
+    gf = lgf.GaugeFixer(n, recon=12, accum_g=1)
+    gf.load_links(U)
+    r1 = gf.iterate(ALPHA, 1)
+    Uo = U.copy()
+    hist = oracle.iterate(n, Uo, ALPHA, 1)
+    assert np.abs(gf.get_links() - Uo).max() < 1e-12
+    assert abs(r1.F - hist[1, 0]) <= 1e-10 * abs(hist[1, 0])
+    assert abs(r1.theta - hist[1, 1]) <= 1e-10 * hist[1, 1]
+    it, F, th, ghist = read_golden(golden_path(n, seed))
+    gf.load_links(U)
+    r = gf.fix(ALPHA, 1e-15)
+    assert r.converged == 1 and abs(r.iterations - it) <= 0.02 * it and abs(r.F - F) <= 1e-10
+    Ufix = gf.get_links()
+    d = Ufix @ np.conj(np.swapaxes(Ufix, -1, -2)) - np.eye(3)
+    assert np.abs(d).max() < 1e-12
+    gf.close()
+
+
+# ------------------------------------------------------------------ GMAP = exact exponential
+EXP_VARIANTS = [dict(recon=18, fft_batch=4), dict(recon=12, fft_batch=4), dict(recon=18, fft_batch=9),
+                dict(recon=12, fft_batch=4, fusion=0), dict(recon=18, fft_batch=4, fft_path=1),
+                dict(recon=12, fft_batch=4, accum_g=1)]
+
+
+def vid(v):
+    return "-".join(f"{k}{x}" for k, x in v.items())
+
+
+@pytest.mark.parametrize("var", EXP_VARIANTS[:4], ids=vid)
+@pytest.mark.parametrize("scale", [1.0, 40.0])
+def test_exp_g_tap_matches_oracle(lgf, var, scale):
+    """g = exp((alpha/2) w) from an oracle w; scale = 40 makes |A| ~ 10 so that the halving and
+    squaring steps run (alpha/2 * 40 = 1.6 times the natural size)."""
+    N, sigma, seed = (8, 8, 8, 8), 0.5, 91
+    U = gen.gen_links(N, sigma, seed)
+    D, _, _ = oracle.measure(N, U)
+    w = oracle.fourier_accelerate(N, D) * scale
+    g = oracle.build_g_exp(w, ALPHA)
+    gf = lgf.GaugeFixer(N, gmap=lgf.GMAP_EXP, **var)
+    gf.load_links(U)
+    gf.set_field(lgf.FIELD_W, w)
+    g2 = gf.get_field(lgf.FIELD_G, alpha=ALPHA)
+    # every squaring doubles the rounding error of the series: 4 (here) to 6 (oracle) squarings at scale 40
+    tol = 5e-14 if scale == 1.0 else 5e-13
+    assert np.abs(g2 - g).max() < tol
+    assert np.abs(g2 @ np.conj(np.swapaxes(g2, -1, -2)) - np.eye(3)).max() < tol
+    gf.stage(lgf.STAGE_UPDATE, alpha=ALPHA)
+    U1 = oracle.update_links(N, U.copy(), g)
+    assert np.abs(gf.get_links() - U1).max() < 4 * tol
+    gf.close()
+
+
+@pytest.mark.parametrize("var", EXP_VARIANTS, ids=vid)
+@pytest.mark.parametrize("lat", [((8, 8, 8, 8), 0.3, gen.BASE_SEED + 8), ((16, 16, 16, 16), 0.5, gen.BASE_SEED + 16)], ids=lid)
+def test_exp_one_iteration_matches_oracle(lgf, exp_oracle, var, lat):
+    N, sigma, seed = lat
+    U = gen.gen_links(N, sigma, seed)
+    Uo = U.copy()
+    hist = oracle.iterate(N, Uo, ALPHA, 1)
+    gf = lgf.GaugeFixer(N, gmap=lgf.GMAP_EXP, **var)
+    gf.load_links(U)
+    r = gf.iterate(ALPHA, 1)
+    assert np.abs(gf.get_links() - Uo).max() < 1e-12
+    assert abs(r.F - hist[1, 0]) <= 1e-10 * abs(hist[1, 0])
+    assert abs(r.theta - hist[1, 1]) <= 1e-10 * hist[1, 1]
+    gf.close()
+
+
+@pytest.mark.parametrize("var", [EXP_VARIANTS[1], EXP_VARIANTS[5]], ids=vid)
+def test_exp_convergence_matches_oracle(lgf, exp_oracle, var):
+    n, seed = 8, gen.BASE_SEED + 8
+    U = gen.gen_links(n, 0.3, seed)
+    Uo = U.copy()
+    it, F, th, hist = oracle.fix(n, Uo, ALPHA, 1e-15)
+    gf = lgf.GaugeFixer(n, gmap=lgf.GMAP_EXP, **var)
+    gf.load_links(U)
+    r = gf.fix(ALPHA, 1e-15)
+    assert r.converged == 1 and abs(r.iterations - it) <= max(1, 0.02 * it)
+    assert abs(r.F - F) <= 1e-10
+    h = gf.history()
+    k = min(h.shape[0], hist.shape[0]) - 3
+    assert np.allclose(h[:k, 0], hist[:k, 0], rtol=0, atol=1e-10)
+    # and the exponential map is not the first-order map: the trajectories differ at O(alpha^2 w^2)
+    gf.set_option(lgf.OPT_GMAP, lgf.GMAP_FIRST_ORDER)
+    gf.load_links(U)
+    r0 = gf.iterate(ALPHA, 1)
+    assert abs(r0.F - hist[1, 0]) > 1e-7
+    gf.close()
