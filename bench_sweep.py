@@ -32,17 +32,52 @@ def paper_flops_per_site(N, recon):
     return k2 + k4 + k5 + k6 + fft
 
 
+def alpha_scan(alphas, sizes, gen, lgf):
+    """Iterations of Algorithm 1 until theta <= 1e-15 as a function of the step alpha (eq. 1.2,
+    PAPER.md:49; the paper fixes alpha = 0.08) for g = reunit(1 + (alpha/2) w) and for
+    g = exp((alpha/2) w), on the synthetic N^4 lattices of DESIGN.md section 4."""
+    lines = ["| lattice | alpha | g map | iterations | final F | final theta | converged |", "|---|---|---|---|---|---|---|"]
+    for n in sizes:
+        U = gen.gen_links(n, 0.5, gen.BASE_SEED + n)
+        import torch
+        Ud = torch.from_numpy(U).cuda()
+        for gmap, name in ((0, "first order + reunit"), (1, "exp")):
+            gf = lgf.GaugeFixer(n, recon=12, gmap=gmap, max_iter=400)
+            for al in alphas:
+                gf.load_links(Ud)
+                try:
+                    r = gf.fix(al, 1e-15, allow_not_converged=True)
+                except lgf.LgfError as e:       # theta became NaN/Inf: the step is too long
+                    lines.append(f"| {n}^4 | {al:.4f} | {name} | - | - | - | diverged ({e.code}) |")
+                    continue
+                lines.append(f"| {n}^4 | {al:.4f} | {name} | {r.iterations} | {r.F:.12f} | {r.theta:.3e} | {r.converged} |")
+            gf.close()
+        del Ud
+    return "\n".join(lines)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--nt", type=int, nargs="+", default=[8, 16, 32, 48, 64])
     ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--out", default=None)
+    ap.add_argument("--alpha-scan", type=float, nargs="*", default=None,
+                    help="instead of the timing sweep: iterations to theta <= 1e-15 for these alpha, both g maps")
+    ap.add_argument("--scan-n", type=int, nargs="+", default=[16, 32])
     args = ap.parse_args()
     import numpy as np
     import torch
 
     import gen
     from paper_1210_8018_b200 import lgf
+
+    if args.alpha_scan is not None:
+        text = alpha_scan(args.alpha_scan or [0.04, 0.05, 0.0625, 0.07, 0.08, 0.09, 0.10, 0.11, 0.12], args.scan_n, gen, lgf)
+        print(text)
+        if args.out:
+            with open(args.out, "w") as f:
+                f.write(text + "\n")
+        return
 
     lines = ["| lattice | precision | reals/link | FFT path | ms/iteration | site-iterations/s | paper-model GFlops |",
              "|---|---|---|---|---|---|---|"]

@@ -336,14 +336,15 @@ template <typename T, int NA, int NB> struct XYGCfg {
 };
 
 // g -> the g buffer, or (ACC, LGF_OPT_ACCUM_G) the accumulated transformation G(x) <- g(x) G(x):
-// rows 0, 1 of G are read, row 2 rebuilt, rows 0, 1 of the product Gram-Schmidt cleaned and stored.
+// rows 0, 1 of G are read (Gold, loaded by the caller ahead of time), row 2 rebuilt, rows 0, 1 of
+// the product Gram-Schmidt cleaned and stored.
 template <typename T, bool ACC>
-__device__ __forceinline__ void emit_g(cx<T> (&g)[9], cx<T> *__restrict__ dst, int64_t V)
+__device__ __forceinline__ void emit_g(cx<T> (&g)[9], const cx<T> (&Gold)[6], cx<T> *__restrict__ dst, int64_t V)
 {
     if (ACC) {
         cx<T> G[9], n[9];
 #pragma unroll
-        for (int k = 0; k < 6; k++) G[k] = dst[(int64_t)k * V];
+        for (int k = 0; k < 6; k++) G[k] = Gold[k];
         su3_row2(G);
         mul_rows<2>(g, G, n);
         reunit01<T>(n);
@@ -354,6 +355,11 @@ __device__ __forceinline__ void emit_g(cx<T> (&g)[9], cx<T> *__restrict__ dst, i
         for (int k = 0; k < 6; k++) dst[(int64_t)k * V] = g[k];
     }
 }
+// Sites of the epilogue handled per loop trip: with ACC the loads of G for all of them are issued
+// before the first product, so that the trip pays one memory latency instead of EPI_BATCH.
+#ifndef LGF_EPI_BATCH
+#define LGF_EPI_BATCH 4
+#endif
 
 template <typename T, int NA, int NB, bool ACC>
 __global__ void __launch_bounds__((XYGCfg<T, NA, NB>::CTA))
@@ -415,12 +421,28 @@ k_fft_xy_inv_g(const cx<T> *__restrict__ w, cx<T> *__restrict__ gbuf, int64_t V,
     }
     __syncthreads();
     if (ok) {
-        for (int i = t; i < NA * NB; i += TG) {
-            const int o = (i / NA) * TL::RS + (i % NA);
-            cx<T> g[9];
-            m_from_packed<T>(smp[o], smp[TL::ELEMS + o], smp[2 * TL::ELEMS + o], smp[3 * TL::ELEMS + o], a, g);
-            finish_g01<T>(g, gexp);
-            emit_g<T, ACC>(g, gbuf + base + i, V);
+        constexpr int EB = ACC ? LGF_EPI_BATCH : 1;
+        for (int i0 = t; i0 < NA * NB; i0 += EB * TG) {
+            cx<T> Gold[EB][6];
+            if (ACC) {
+#pragma unroll
+                for (int b = 0; b < EB; b++)
+                    if (i0 + b * TG < NA * NB) {
+#pragma unroll
+                        for (int k = 0; k < 6; k++) Gold[b][k] = gbuf[(int64_t)k * V + base + i0 + b * TG];
+                    }
+            }
+#pragma unroll
+            for (int b = 0; b < EB; b++) {
+                const int i = i0 + b * TG;
+                if (i < NA * NB) {
+                    const int o = (i / NA) * TL::RS + (i % NA);
+                    cx<T> g[9];
+                    m_from_packed<T>(smp[o], smp[TL::ELEMS + o], smp[2 * TL::ELEMS + o], smp[3 * TL::ELEMS + o], a, g);
+                    finish_g01<T>(g, gexp);
+                    emit_g<T, ACC>(g, Gold[b], gbuf + base + i, V);
+                }
+            }
         }
     }
 }
@@ -491,12 +513,28 @@ k_fft_xy_inv_g2(const cx<T> *__restrict__ w, cx<T> *__restrict__ gbuf, int64_t V
     const cx<T> *peer = cluster.map_shared_rank(smp, rank ^ 1);
     const cx<T> *f01 = rank == 0 ? smp : peer, *f23 = rank == 0 ? peer : smp;
     constexpr int HALF = NA * NB / 2;
-    for (int i = rank * HALF + t; i < (rank + 1) * HALF; i += CF::CTA) {
-        const int o = (i / NA) * TL::RS + (i % NA);
-        cx<T> g[9];
-        m_from_packed<T>(f01[o], f01[TL::ELEMS + o], f23[o], f23[TL::ELEMS + o], a, g);
-        finish_g01<T>(g, gexp);
-        emit_g<T, ACC>(g, gbuf + base + i, V);
+    constexpr int EB = ACC ? LGF_EPI_BATCH : 1;
+    for (int i0 = rank * HALF + t; i0 < (rank + 1) * HALF; i0 += EB * CF::CTA) {
+        cx<T> Gold[EB][6];
+        if (ACC) {
+#pragma unroll
+            for (int b = 0; b < EB; b++)
+                if (i0 + b * CF::CTA < (rank + 1) * HALF) {
+#pragma unroll
+                    for (int k = 0; k < 6; k++) Gold[b][k] = gbuf[(int64_t)k * V + base + i0 + b * CF::CTA];
+                }
+        }
+#pragma unroll
+        for (int b = 0; b < EB; b++) {
+            const int i = i0 + b * CF::CTA;
+            if (i < (rank + 1) * HALF) {
+                const int o = (i / NA) * TL::RS + (i % NA);
+                cx<T> g[9];
+                m_from_packed<T>(f01[o], f01[TL::ELEMS + o], f23[o], f23[TL::ELEMS + o], a, g);
+                finish_g01<T>(g, gexp);
+                emit_g<T, ACC>(g, Gold[b], gbuf + base + i, V);
+            }
+        }
     }
     cluster.sync();                                          // the peer may still be reading this CTA's fields
 }
@@ -507,6 +545,9 @@ k_fft_xy_inv_g2(const cx<T> *__restrict__ w, cx<T> *__restrict__ gbuf, int64_t V
 // shared (thread = (c, kz)): Dif(-), mask, Dit(+) -> shared; z-lines from shared: Dif(+),
 // stored straight to global.  p^2 = sum_mu 4 sin^2(pi k_mu/N_mu) (reading R5) from the
 // per-axis tables; the factor p_max^2/(p^2 V) is one FP64 division per mode.
+#ifndef LGF_ZT_MAXB
+#define LGF_ZT_MAXB 2
+#endif
 template <typename T, int NA, int NB, int C> struct ZTCfg {
     typedef Tile<NA, NB, C> TL;
     static constexpr int TT = TL::THREADS;
@@ -514,10 +555,13 @@ template <typename T, int NA, int NB, int C> struct ZTCfg {
     static constexpr int G = CTA / TT;
     static constexpr size_t PT = ((NB * sizeof(double) + 15) / 16) * 16;
     static constexpr size_t SMEM = PT + (size_t)G * TL::ELEMS * sizeof(cx<T>);
+    // CTAs per SM that shared memory allows (1 KB reserved each); registers are capped to match
+    static constexpr int FIT = (int)((size_t)227 * 1024 / (SMEM + 1024));
+    static constexpr int MINB = FIT < 1 ? 1 : (FIT > LGF_ZT_MAXB ? LGF_ZT_MAXB : FIT);
 };
 
 template <typename T, int NA, int NB, int C>
-__global__ void __launch_bounds__((ZTCfg<T, NA, NB, C>::CTA))
+__global__ void __launch_bounds__((ZTCfg<T, NA, NB, C>::CTA), (ZTCfg<T, NA, NB, C>::MINB))
 k_fft_zt(cx<T> *__restrict__ w, Geom geo, const double *__restrict__ ptab, double pmax2_over_V, int64_t ntiles, const Ctrl *ctrl)
 {
     if (*(volatile const int *)&ctrl->done) return;

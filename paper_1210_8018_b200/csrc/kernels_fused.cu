@@ -79,11 +79,17 @@ __device__ __forceinline__ double store_delta(const T (&di)[3], const cx<T> (&E)
 // links G(x) U_mu(x) G^dagger(x+mu) (Alg. 1 lines 12-16 applied n times) are formed in
 // registers exactly as below and measured, but not written: 544 instead of 928 bytes per site
 // (FP64, 12-real).
+// ACCUM_G tuning (measured on B200, profiles/r01d_accum_g.md): with 18-real links the forward links
+// are taken through their sum (rows 0, 1 of U suffice: 6 of 9 loads) at 3 CTAs per SM in FP64; with 12-real
+// links the per-link form below at 4 CTAs per SM is faster (the sum form spills at 128 registers).
+#ifndef LGF_ACC_QSUM
+#define LGF_ACC_QSUM(NE) ((NE) == 9)
+#endif
 #ifndef LGF_ACC_MINB
-#define LGF_ACC_MINB 4
+#define LGF_ACC_MINB(NE, T) ((NE) == 9 && sizeof(T) == 8 ? 3 : 4)
 #endif
 template <typename T, int NE, int PACK, bool GBUF, bool STORE>
-__global__ void __launch_bounds__(FUSED_THREADS, (STORE ? LGF_FUSED_MINB : LGF_ACC_MINB))
+__global__ void __launch_bounds__(FUSED_THREADS, (STORE ? LGF_FUSED_MINB : LGF_ACC_MINB(NE, T)))
 k_update_measure(const cx<T> *__restrict__ lin, cx<T> *__restrict__ lout, const cx<T> *__restrict__ gsrc,
                  cx<T> *__restrict__ wout, Geom geo, T a, int gexp, Ctrl *ctrl, double *partials, double2 *hist, double eps)
 {
@@ -94,57 +100,112 @@ k_update_measure(const cx<T> *__restrict__ lin, cx<T> *__restrict__ lout, const 
     if (s < V) {
         int c[4];
         site_coords(geo, s, c);
-        // Backward links first: only their sum enters A'(x),
-        //     sum_nu U'_nu(x-nu) = [sum_nu H_nu(x-nu)] g^dagger(x),   H_nu(y) = g(y) U_nu(y),
-        // so rows 0, 1 of each H are one product, row 2 is conj(row0 x row1) (H is special
-        // unitary) and g^dagger(x) is applied once to the sum.
-        cx<T> X[9];
+        if (!STORE && LGF_ACC_QSUM(NE)) {
+            // ACCUM_G: nothing is stored, so the forward links enter only through their sum as well,
+            //     sum_mu U'_mu(x) = G(x) [sum_mu U_mu(x) G^dagger(x+mu)]:
+            // rows 0, 1 of U_mu(x) suffice (no third-row rebuild), G(x) is applied once.  The forward
+            // bracket goes first so that G(x) is not live across both loops (registers).
+            T di[3] = {0, 0, 0};
+            cx<T> E[3] = {mk<T>(0, 0), mk<T>(0, 0), mk<T>(0, 0)};
+            cx<T> X[9];
 #pragma unroll
-        for (int k = 0; k < 9; k++) X[k] = mk<T>(0, 0);
+            for (int k = 0; k < 9; k++) X[k] = mk<T>(0, 0);
 #pragma unroll
-        for (int nu = 0; nu < 4; nu++) {
-            const int64_t sb = s + (c[nu] == 0 ? (int64_t)(geo.N[nu] - 1) : (int64_t)-1) * geo.st[nu];
-            cx<T> gb[9], u[9], h[9];
-            load_g01<T, PACK, GBUF>(gsrc, V, sb, a, gexp, gb);
-            load_link_in<T, NE>(lin, V, nu, sb, u);
-            mul_rows<2>(gb, u, h);
-            su3_row2(h);
+            for (int mu = 0; mu < 4; mu++) {
+                const int64_t sp = s + (c[mu] == geo.N[mu] - 1 ? -(int64_t)(geo.N[mu] - 1) : (int64_t)1) * geo.st[mu];
+                cx<T> g1[9], u[9], h[9];
+                load_g01<T, PACK, GBUF>(gsrc, V, sp, a, gexp, g1);
+                su3_row2(g1);
+                const cx<T> *p = lin + (int64_t)mu * NE * V + s;
 #pragma unroll
-            for (int k = 0; k < 9; k++) X[k] = X[k] + h[k];
-        }
-        cx<T> g0[9];
-        load_g01<T, PACK, GBUF>(gsrc, V, s, a, gexp, g0);
-        su3_row2(g0);
-        T di[3] = {0, 0, 0};
-        cx<T> E[3] = {mk<T>(0, 0), mk<T>(0, 0), mk<T>(0, 0)};
-        {
-            cx<T> B[9];
-            mul_rows_dag<3>(X, g0, B);
-            acc_ah<T>(B, (T)1, di, E);
-        }
-        // Forward links U'_mu(x) = g(x) U_mu(x) g^dagger(x+mu): rows 0, 1 computed and stored; row 2 is
-        // conj(row0 x row1), which is also what a later load of 12-real storage rebuilds (R15).
-        T tr = 0;
+                for (int k = 0; k < 6; k++) u[k] = ld_link(p + (int64_t)k * V);
+                mul_rows_dag<2>(u, g1, h);
+                su3_row2(h);
 #pragma unroll
-        for (int mu = 0; mu < 4; mu++) {
-            const int64_t sp = s + (c[mu] == geo.N[mu] - 1 ? -(int64_t)(geo.N[mu] - 1) : (int64_t)1) * geo.st[mu];
-            cx<T> g1[9], u[9], t[9], r[9];
-            load_g01<T, PACK, GBUF>(gsrc, V, sp, a, gexp, g1);
-            su3_row2(g1);
-            load_link_in<T, NE>(lin, V, mu, s, u);
-            mul_rows<2>(g0, u, t);
-            mul_rows_dag<2>(t, g1, r);
-            su3_row2(r);
-            if (STORE) {
-                cx<T> *p = lout + (int64_t)mu * NE * V + s;
-#pragma unroll
-                for (int k = 0; k < NE; k++) st_link(p + (int64_t)k * V, r[k]);
+                for (int k = 0; k < 9; k++) X[k] = X[k] + h[k];
             }
-            tr += r[0].x + r[4].x + r[8].x;
-            acc_ah<T>(r, (T)-1, di, E);
+            {
+                cx<T> g0[9], B[9];
+                load_g01<T, PACK, GBUF>(gsrc, V, s, a, gexp, g0);
+                su3_row2(g0);
+                mul_rows<3>(g0, X, B);
+                acc_ah<T>(B, (T)-1, di, E);
+                trF = (double)(B[0].x + B[4].x + B[8].x);
+            }
+#pragma unroll
+            for (int k = 0; k < 9; k++) X[k] = mk<T>(0, 0);
+#pragma unroll
+            for (int nu = 0; nu < 4; nu++) {
+                const int64_t sb = s + (c[nu] == 0 ? (int64_t)(geo.N[nu] - 1) : (int64_t)-1) * geo.st[nu];
+                cx<T> gb[9], u[9], h[9];
+                load_g01<T, PACK, GBUF>(gsrc, V, sb, a, gexp, gb);
+                load_link_in<T, NE>(lin, V, nu, sb, u);
+                mul_rows<2>(gb, u, h);
+                su3_row2(h);
+#pragma unroll
+                for (int k = 0; k < 9; k++) X[k] = X[k] + h[k];
+            }
+            {
+                cx<T> g0[9], B[9];
+                load_g01<T, PACK, GBUF>(gsrc, V, s, a, gexp, g0);   // again: an L1 hit, cheaper than 36 live registers
+                su3_row2(g0);
+                mul_rows_dag<3>(X, g0, B);
+                acc_ah<T>(B, (T)1, di, E);
+            }
+            th = store_delta<T, PACK>(di, E, wout, V, s);
+        } else {
+            // Backward links first: only their sum enters A'(x),
+            //     sum_nu U'_nu(x-nu) = [sum_nu H_nu(x-nu)] g^dagger(x),   H_nu(y) = g(y) U_nu(y),
+            // so rows 0, 1 of each H are one product, row 2 is conj(row0 x row1) (H is special
+            // unitary) and g^dagger(x) is applied once to the sum.
+            cx<T> X[9];
+#pragma unroll
+            for (int k = 0; k < 9; k++) X[k] = mk<T>(0, 0);
+#pragma unroll
+            for (int nu = 0; nu < 4; nu++) {
+                const int64_t sb = s + (c[nu] == 0 ? (int64_t)(geo.N[nu] - 1) : (int64_t)-1) * geo.st[nu];
+                cx<T> gb[9], u[9], h[9];
+                load_g01<T, PACK, GBUF>(gsrc, V, sb, a, gexp, gb);
+                load_link_in<T, NE>(lin, V, nu, sb, u);
+                mul_rows<2>(gb, u, h);
+                su3_row2(h);
+#pragma unroll
+                for (int k = 0; k < 9; k++) X[k] = X[k] + h[k];
+            }
+            cx<T> g0[9];
+            load_g01<T, PACK, GBUF>(gsrc, V, s, a, gexp, g0);
+            su3_row2(g0);
+            T di[3] = {0, 0, 0};
+            cx<T> E[3] = {mk<T>(0, 0), mk<T>(0, 0), mk<T>(0, 0)};
+            {
+                cx<T> B[9];
+                mul_rows_dag<3>(X, g0, B);
+                acc_ah<T>(B, (T)1, di, E);
+            }
+            // Forward links U'_mu(x) = g(x) U_mu(x) g^dagger(x+mu): rows 0, 1 computed and stored; row 2 is
+            // conj(row0 x row1), which is also what a later load of 12-real storage rebuilds (R15).
+            T tr = 0;
+#pragma unroll
+            for (int mu = 0; mu < 4; mu++) {
+                const int64_t sp = s + (c[mu] == geo.N[mu] - 1 ? -(int64_t)(geo.N[mu] - 1) : (int64_t)1) * geo.st[mu];
+                cx<T> g1[9], u[9], t[9], r[9];
+                load_g01<T, PACK, GBUF>(gsrc, V, sp, a, gexp, g1);
+                su3_row2(g1);
+                load_link_in<T, NE>(lin, V, mu, s, u);
+                mul_rows<2>(g0, u, t);
+                mul_rows_dag<2>(t, g1, r);
+                su3_row2(r);
+                if (STORE) {
+                    cx<T> *p = lout + (int64_t)mu * NE * V + s;
+#pragma unroll
+                    for (int k = 0; k < NE; k++) st_link(p + (int64_t)k * V, r[k]);
+                }
+                tr += r[0].x + r[4].x + r[8].x;
+                acc_ah<T>(r, (T)-1, di, E);
+            }
+            trF = (double)tr;
+            th = store_delta<T, PACK>(di, E, wout, V, s);
         }
-        trF = (double)tr;
-        th = store_delta<T, PACK>(di, E, wout, V, s);
     }
     finish_measure<FUSED_THREADS>(trF, th, V, ctrl, partials, hist, eps, 1);
 }

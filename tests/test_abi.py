@@ -72,6 +72,14 @@ def test_options_and_workspace_size(L):
     assert L.lgf_set_option(ctx, 99, 0) == lgf.ERR_INVALID_ARG
     assert L.lgf_set_option(ctx, lgf.OPT_CHECK_INTERVAL, 0) == lgf.ERR_INVALID_ARG
     assert L.lgf_set_option(ctx, lgf.OPT_MAX_ITER, 10) == lgf.OK
+    assert L.lgf_set_option(ctx, lgf.OPT_GMAP, 2) == lgf.ERR_INVALID_ARG
+    assert L.lgf_set_option(ctx, lgf.OPT_GMAP, lgf.GMAP_EXP) == lgf.OK
+    assert L.lgf_set_option(ctx, lgf.OPT_ACCUM_G, -1) == lgf.ERR_INVALID_ARG
+    assert L.lgf_set_option(ctx, lgf.OPT_ACCUM_G, 1) == lgf.OK
+    assert L.lgf_bind(ctx, 256, 1 << 40, None) == lgf.ERR_INVALID_ARG   # FUSION = 0, FFT_BATCH = 9 here
+    assert b"ACCUM_G" in L.lgf_last_error(ctx)
+    assert L.lgf_set_option(ctx, lgf.OPT_ACCUM_G, 0) == lgf.OK
+    assert L.lgf_sync_links(ctx) == lgf.ERR_NOT_BOUND
     assert L.lgf_workspace_bytes(None) == 0
     # nothing can run before bind / load
     r = lgf.lgf_result()
@@ -82,6 +90,11 @@ def test_options_and_workspace_size(L):
     assert L.lgf_bind(ctx, 256, 16, None) == lgf.ERR_WORKSPACE_TOO_SMALL
     assert L.lgf_bind(ctx, 257, 1 << 40, None) == lgf.ERR_INVALID_ARG   # not 256-byte aligned
     assert L.lgf_launch_count(ctx) == 0
+    assert L.lgf_destroy(ctx) == lgf.OK
+    # ACCUM_G: one link buffer instead of two, everything else as in the fused layout
+    assert L.lgf_create(32, 32, 32, 32, lgf.PREC_FP64, ctypes.byref(ctx)) == lgf.OK
+    assert L.lgf_set_option(ctx, lgf.OPT_ACCUM_G, 1) == lgf.OK
+    assert bfused - L.lgf_workspace_bytes(ctx) == 4 * 9 * V * 16
     assert L.lgf_destroy(ctx) == lgf.OK
 
 
