@@ -357,6 +357,11 @@ def run_ours(args):
         "gpu_launches": int(launches),
         "roofline": {"bound": "hbm", "kernel": dom, "achieved": kern[dom]["GBps"], "peak": peak, "unit": "GB/s",
                      "frac": kern[dom]["GBps"] / peak,
+                     **({"note": "measure_acc is bound by plain FP64 arithmetic (ncu: FP64 pipe 67 %, DRAM 51 %, "
+                                 "profiles/r01d_accum_g.md): about 1500 FP64 instructions per site against a nominal "
+                                 "148 SMs x 64 DFMA/clk x 1.965 GHz = 18.6e12/s give "
+                                 f"{1500 * V / (kern[dom]['us_per_launch'] * 1e-6) / 18.6e12:.2f} of the ALU peak"}
+                        if dom == "measure_acc" else {}),
                      "traffic": ncu_traffic(f"{args.workload}-{prec}-recon{recon}-fields{args.fft_batch}", dom),
                      "algorithmic_bytes": per[dom] * V, "peak_source": peak_src,
                      "bytes_per_site": per[dom],

@@ -333,6 +333,9 @@ template <typename T, int NA, int NB> struct XYGCfg {
     static constexpr int G = CTA / TG;
     static constexpr size_t SMEM = (size_t)G * 4 * TL::ELEMS * sizeof(cx<T>);
     static constexpr bool FITS = SMEM <= 227 * 1024 && CTA <= 1024;
+    // CTAs per SM that shared memory allows (1 KB reserved each), at most 3: registers are capped to match
+    static constexpr int FIT = (int)((size_t)227 * 1024 / (SMEM + 1024));
+    static constexpr int MINB = FIT < 1 ? 1 : (FIT > 3 ? 3 : FIT);
 };
 
 // g -> the g buffer, or (ACC, LGF_OPT_ACCUM_G) the accumulated transformation G(x) <- g(x) G(x):
@@ -362,7 +365,7 @@ __device__ __forceinline__ void emit_g(cx<T> (&g)[9], const cx<T> (&Gold)[6], cx
 #endif
 
 template <typename T, int NA, int NB, bool ACC>
-__global__ void __launch_bounds__((XYGCfg<T, NA, NB>::CTA))
+__global__ void __launch_bounds__((XYGCfg<T, NA, NB>::CTA), (ACC ? XYGCfg<T, NA, NB>::MINB : 1))
 k_fft_xy_inv_g(const cx<T> *__restrict__ w, cx<T> *__restrict__ gbuf, int64_t V, int64_t nplanes, T a, int gexp, const Ctrl *ctrl)
 {
     if (*(volatile const int *)&ctrl->done) return;
@@ -546,7 +549,7 @@ k_fft_xy_inv_g2(const cx<T> *__restrict__ w, cx<T> *__restrict__ gbuf, int64_t V
 // stored straight to global.  p^2 = sum_mu 4 sin^2(pi k_mu/N_mu) (reading R5) from the
 // per-axis tables; the factor p_max^2/(p^2 V) is one FP64 division per mode.
 #ifndef LGF_ZT_MAXB
-#define LGF_ZT_MAXB 2
+#define LGF_ZT_MAXB 2   /* 3 measured slower at 32^4 (47.6 vs 45.5 us: spills), equal at 48^4 */
 #endif
 template <typename T, int NA, int NB, int C> struct ZTCfg {
     typedef Tile<NA, NB, C> TL;
