@@ -15,8 +15,12 @@
  * Lattice and layouts
  *   extents N[0..3] = Nx, Ny, Nz, Nt;  V = Nx*Ny*Nz*Nt;  direction mu = 0..3 <-> x, y, z, t;
  *   site index s = ix + Nx*(iy + Ny*(iz + Nz*it))  (x fastest, lexicographic).
- *   Interchange layout of a link field (LGF_LAYOUT_AOS, the only one defined):
- *       real[((((s*4 + mu)*3 + row)*3 + col)*2 + {0:re, 1:im}],   18 reals per link,
+ *   Interchange layouts of a link field:
+ *     LGF_LAYOUT_AOS:    real[((((s*4 + mu)*3 + row)*3 + col)*2 + {0:re, 1:im}],   18 reals per link,
+ *     LGF_LAYOUT_AOS12:  the same with row = 0, 1 only, real[((((s*4 + mu)*2 + row)*3 + col)*2 + {re,im}],
+ *                        12 reals per link (the 12-real compression of PAPER.md:121-123 as an exchange
+ *                        format: two thirds of the bytes over PCIe); row 2 = conj(row0 x row1) is
+ *                        implied, and rebuilt on load when the context stores 18 reals,
  *   and of a site field (Delta, w, g):  real[(((s*3 + row)*3 + col)*2 + {re,im}].
  *   `real` is double for LGF_PREC_FP64 contexts and float for LGF_PREC_FP32 contexts.
  *   Inside the workspace links live as complex SoA arrays (one array over sites per matrix
@@ -55,7 +59,7 @@ enum {
 };
 
 enum { LGF_PREC_FP64 = 0, LGF_PREC_FP32 = 1 };
-enum { LGF_LAYOUT_AOS = 0 };
+enum { LGF_LAYOUT_AOS = 0, LGF_LAYOUT_AOS12 = 1 };
 
 /* lgf_set_option keys.  Options must be set before lgf_workspace_bytes / lgf_bind. */
 enum {
@@ -87,7 +91,7 @@ enum {
                                    order g = 1 + (alpha/2) w followed by a reunitarisation;
                                    1: the exact exponential g = exp((alpha/2) w) of eq. 1.2 as written
                                    (PAPER.md:49), no projection.  May be changed at any time. */
-    LGF_OPT_ACCUM_G = 10        /* 1: lgf_iterate / lgf_fix keep the loaded links fixed and accumulate the
+    LGF_OPT_ACCUM_G = 10,       /* 1: lgf_iterate / lgf_fix keep the loaded links fixed and accumulate the
                                    gauge transformation instead, G(x) <- g(x) G(x) (rows 0, 1 stored, Gram-
                                    Schmidt after every product), measuring Delta, F, theta of
                                    G(x) U_mu(x) G^dagger(x+mu) on the fly; the links are rewritten once,
@@ -97,6 +101,13 @@ enum {
                                    per-iteration link write; one link buffer instead of two.  Needs FUSION = 1,
                                    FFT_BATCH = 4 and a lattice the tiled FFT covers, else lgf_bind fails with
                                    LGF_ERR_INVALID_ARG.  0 (default): links rewritten every iteration. */
+    LGF_OPT_GRAPH = 11          /* 1 (default): lgf_iterate / lgf_fix capture min(CHECK_INTERVAL, 8) (rounded
+                                   down to even, at least 2) iterations into a CUDA graph once and replay
+                                   it, so that small lattices (8^4, 16^4: a few microseconds per kernel) are
+                                   not bound by launch overhead; leftovers and profiled runs (LGF_OPT_PROFILE)
+                                   are launched directly.  Same kernels, same results.  Falls back to direct
+                                   launches by itself when the bound stream cannot be captured (e.g. the
+                                   legacy default stream).  0: always direct launches.  Any time. */
 };
 
 /* lgf_get_field / lgf_set_field selectors */
@@ -148,13 +159,15 @@ size_t lgf_workspace_bytes(const lgf_ctx *ctx);
  * Uploads the small tables (momentum tables 4 sin^2(pi k/N), twiddles). */
 int lgf_bind(lgf_ctx *ctx, void *dev_workspace, size_t bytes, void *cuda_stream);
 
-/* Load a link field in the interchange layout from host (src_is_device = 0) or device memory
- * into the internal SoA arrays (dropping row 2 if RECON = 12), then run kernel (a) so that
+/* Load a link field in an interchange layout (LGF_LAYOUT_AOS or LGF_LAYOUT_AOS12) from host
+ * (src_is_device = 0) or device memory into the internal SoA arrays (dropping row 2 if RECON = 12,
+ * rebuilding it from an AOS12 source if RECON = 18), then run kernel (a) so that
  * Delta, F, theta of the loaded links are available.  The source is not retained.
  * Synchronises the stream before returning when the source is host memory. */
 int lgf_load_links(lgf_ctx *ctx, const void *src, int src_is_device, int src_layout);
 
-/* Inverse conversion into dst (host or device), third row rebuilt if RECON = 12.  Synchronous. */
+/* Inverse conversion into dst (host or device) in either layout, third row rebuilt if RECON = 12 and
+ * the layout carries it.  Synchronous. */
 int lgf_get_links(lgf_ctx *ctx, void *dst, int dst_is_device, int dst_layout);
 
 /* Kernel (a) only: F and theta of the current links (host out pointers, may be NULL). Synchronous. */

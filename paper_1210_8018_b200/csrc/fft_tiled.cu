@@ -333,9 +333,6 @@ template <typename T, int NA, int NB> struct XYGCfg {
     static constexpr int G = CTA / TG;
     static constexpr size_t SMEM = (size_t)G * 4 * TL::ELEMS * sizeof(cx<T>);
     static constexpr bool FITS = SMEM <= 227 * 1024 && CTA <= 1024;
-    // CTAs per SM that shared memory allows (1 KB reserved each), at most 3: registers are capped to match
-    static constexpr int FIT = (int)((size_t)227 * 1024 / (SMEM + 1024));
-    static constexpr int MINB = FIT < 1 ? 1 : (FIT > 3 ? 3 : FIT);
 };
 
 // g -> the g buffer, or (ACC, LGF_OPT_ACCUM_G) the accumulated transformation G(x) <- g(x) G(x):
@@ -365,7 +362,7 @@ __device__ __forceinline__ void emit_g(cx<T> (&g)[9], const cx<T> (&Gold)[6], cx
 #endif
 
 template <typename T, int NA, int NB, bool ACC>
-__global__ void __launch_bounds__((XYGCfg<T, NA, NB>::CTA), (ACC ? XYGCfg<T, NA, NB>::MINB : 1))
+__global__ void __launch_bounds__((XYGCfg<T, NA, NB>::CTA))
 k_fft_xy_inv_g(const cx<T> *__restrict__ w, cx<T> *__restrict__ gbuf, int64_t V, int64_t nplanes, T a, int gexp, const Ctrl *ctrl)
 {
     if (*(volatile const int *)&ctrl->done) return;

@@ -152,20 +152,26 @@ template <typename T> __global__ void k_g_identity(cx<T> *__restrict__ gacc, int
 }
 
 // ------------------------------------------------------------------ layout conversions and taps
-template <typename T, int NE>
+// PER = complex numbers per link in the interchange array: 9 (LGF_LAYOUT_AOS) or 6 (LGF_LAYOUT_AOS12,
+// rows 0, 1; row 2 = conj(row0 x row1) is rebuilt here when the links are stored with 18 reals).
+template <typename T, int NE, int PER>
 __global__ void k_aos_to_soa(const cx<T> *__restrict__ aos, cx<T> *__restrict__ links, int64_t V, int64_t s0, int64_t count)
 {
     const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= count * 4) return;
     const int mu = (int)(i / count);
     const int64_t sl = i % count;
-    const cx<T> *src = aos + (sl * 4 + mu) * 9;
+    const cx<T> *src = aos + (sl * 4 + mu) * PER;
     cx<T> *dst = links + (int64_t)mu * NE * V + s0 + sl;
+    cx<T> u[9];
 #pragma unroll
-    for (int k = 0; k < NE; k++) dst[(int64_t)k * V] = src[k];
+    for (int k = 0; k < (NE < PER ? NE : PER); k++) u[k] = src[k];
+    if (NE > PER) su3_row2(u);
+#pragma unroll
+    for (int k = 0; k < NE; k++) dst[(int64_t)k * V] = u[k];
 }
 
-template <typename T, int NE>
+template <typename T, int NE, int PER>
 __global__ void k_soa_to_aos(cx<T> *__restrict__ aos, const cx<T> *__restrict__ links, int64_t V, int64_t s0, int64_t count)
 {
     const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
@@ -174,9 +180,9 @@ __global__ void k_soa_to_aos(cx<T> *__restrict__ aos, const cx<T> *__restrict__ 
     const int64_t sl = i % count;
     cx<T> u[9];
     load_link<T, NE>(links, V, mu, s0 + sl, u);
-    cx<T> *dst = aos + (sl * 4 + mu) * 9;
+    cx<T> *dst = aos + (sl * 4 + mu) * PER;
 #pragma unroll
-    for (int k = 0; k < 9; k++) dst[k] = u[k];
+    for (int k = 0; k < PER; k++) dst[k] = u[k];
 }
 
 template <typename T, int PACK>
@@ -272,20 +278,22 @@ void launch_ctrl_reset(const SiteArgs &a, double eps, cudaStream_t st)
     k_ctrl_reset<<<1, 1, 0, st>>>(a.ctrl, a.hist, eps);
 }
 
-void launch_aos_to_soa(const SiteArgs &a, const void *aos, int64_t s0, int64_t count, cudaStream_t st)
+void launch_aos_to_soa(const SiteArgs &a, const void *aos, int per_link, int64_t s0, int64_t count, cudaStream_t st)
 {
     const int nb = (int)((count * 4 + 255) / 256);
 #define CALL(T, NE, PACK) \
-    k_aos_to_soa<T, NE><<<nb, 256, 0, st>>>((const cx<T> *)aos, (cx<T> *)a.links, a.geo.V, s0, count)
+    do { if (per_link == 6) k_aos_to_soa<T, NE, 6><<<nb, 256, 0, st>>>((const cx<T> *)aos, (cx<T> *)a.links, a.geo.V, s0, count); \
+         else k_aos_to_soa<T, NE, 9><<<nb, 256, 0, st>>>((const cx<T> *)aos, (cx<T> *)a.links, a.geo.V, s0, count); } while (0)
     LGF_DISPATCH(CALL);
 #undef CALL
 }
 
-void launch_soa_to_aos(const SiteArgs &a, void *aos, int64_t s0, int64_t count, cudaStream_t st)
+void launch_soa_to_aos(const SiteArgs &a, void *aos, int per_link, int64_t s0, int64_t count, cudaStream_t st)
 {
     const int nb = (int)((count * 4 + 255) / 256);
 #define CALL(T, NE, PACK) \
-    k_soa_to_aos<T, NE><<<nb, 256, 0, st>>>((cx<T> *)aos, (const cx<T> *)a.links, a.geo.V, s0, count)
+    do { if (per_link == 6) k_soa_to_aos<T, NE, 6><<<nb, 256, 0, st>>>((cx<T> *)aos, (const cx<T> *)a.links, a.geo.V, s0, count); \
+         else k_soa_to_aos<T, NE, 9><<<nb, 256, 0, st>>>((cx<T> *)aos, (const cx<T> *)a.links, a.geo.V, s0, count); } while (0)
     LGF_DISPATCH(CALL);
 #undef CALL
 }

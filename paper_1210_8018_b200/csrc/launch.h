@@ -36,9 +36,10 @@ void launch_g_identity(const SiteArgs &a, void *gacc, cudaStream_t st);
 // iter = 0, hist[0] = (F, theta), done = (theta <= eps)
 void launch_ctrl_reset(const SiteArgs &a, double eps, cudaStream_t st);
 
-// interchange layout <-> SoA, for `count` sites starting at site s0; aos points at site s0
-void launch_aos_to_soa(const SiteArgs &a, const void *aos, int64_t s0, int64_t count, cudaStream_t st);
-void launch_soa_to_aos(const SiteArgs &a, void *aos, int64_t s0, int64_t count, cudaStream_t st);
+// interchange layout <-> SoA, for `count` sites starting at site s0; aos points at site s0;
+// per_link = 9 (LGF_LAYOUT_AOS) or 6 (LGF_LAYOUT_AOS12: rows 0, 1) complex numbers per link
+void launch_aos_to_soa(const SiteArgs &a, const void *aos, int per_link, int64_t s0, int64_t count, cudaStream_t st);
+void launch_soa_to_aos(const SiteArgs &a, void *aos, int per_link, int64_t s0, int64_t count, cudaStream_t st);
 // site-field taps ([count][3][3] complex); which: 0 Delta / 1 w (same unpacking), 2 g
 void launch_field_get(const SiteArgs &a, int which, double alpha, void *aos, int64_t s0, int64_t count, cudaStream_t st);
 void launch_field_set(const SiteArgs &a, const void *aos, int64_t s0, int64_t count, cudaStream_t st);

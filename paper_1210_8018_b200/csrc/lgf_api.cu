@@ -36,6 +36,10 @@ struct lgf_ctx {
     int64_t V;
     int prec;
     int recon = 18, pack = 4, check_interval = 8, fft_path = 0, profile = 0, fusion = 1, l2_persist = 0, gmap = 0, accum = 0;
+    int graph = 1;           // LGF_OPT_GRAPH: replay captured iterations as a CUDA graph
+    cudaGraphExec_t gexec = nullptr;
+    struct { double alpha, eps; int cur, wcur, gmap, unit; } gkey{};
+    int64_t g_launches = 0, g_kcount[LGF_KERNEL_KINDS] = {0};
     bool acc_dirty = false;  // ACCUM_G: the g buffer holds a G != 1 that the links do not yet include
     bool l2_window = false;  // an access-policy window is set on the bound stream
     int cur = 0, wcur = 0;   // which of the two link / field buffers is current
@@ -233,6 +237,60 @@ void do_iteration(lgf_ctx *c, double alpha, double eps)
     c->wstate = 1;
 }
 
+void graph_drop(lgf_ctx *c)
+{
+    if (c->gexec) cudaGraphExecDestroy(c->gexec);
+    c->gexec = nullptr;
+}
+
+// Capture `unit` iterations (even: the double buffers are back where they started) into a graph.
+// Kernel arguments (alpha, eps, buffer pointers, g map) are baked in, so they key the cached graph.
+// Any failure switches the graph path off for this context; the direct launches remain.
+bool graph_ensure(lgf_ctx *c, double alpha, double eps, int unit)
+{
+    if (c->gexec && c->gkey.alpha == alpha && c->gkey.eps == eps && c->gkey.cur == c->cur && c->gkey.wcur == c->wcur &&
+        c->gkey.gmap == c->gmap && c->gkey.unit == unit)
+        return true;
+    graph_drop(c);
+    const int cur0 = c->cur, wcur0 = c->wcur, ws0 = c->wstate;
+    const bool dirty0 = c->acc_dirty;
+    const int64_t l0 = c->launches;
+    int64_t k0[LGF_KERNEL_KINDS];
+    for (int k = 0; k < LGF_KERNEL_KINDS; k++) k0[k] = c->kcount[k];
+    if (cudaStreamBeginCapture(c->st, cudaStreamCaptureModeRelaxed) != cudaSuccess) { cudaGetLastError(); c->graph = 0; return false; }
+    for (int i = 0; i < unit; i++) do_iteration(c, alpha, eps);
+    cudaGraph_t g = nullptr;
+    cudaError_t e = cudaStreamEndCapture(c->st, &g);
+    c->g_launches = c->launches - l0;
+    c->launches = l0;
+    for (int k = 0; k < LGF_KERNEL_KINDS; k++) { c->g_kcount[k] = c->kcount[k] - k0[k]; c->kcount[k] = k0[k]; }
+    const bool back = (c->cur == cur0 && c->wcur == wcur0);
+    c->cur = cur0; c->wcur = wcur0; c->wstate = ws0; c->acc_dirty = dirty0;
+    sync_ptrs(c);
+    if (e == cudaSuccess && g && back) e = cudaGraphInstantiate(&c->gexec, g, 0);
+    if (g) cudaGraphDestroy(g);
+    if (e != cudaSuccess || !c->gexec || !back) { cudaGetLastError(); graph_drop(c); c->graph = 0; return false; }
+    c->gkey.alpha = alpha; c->gkey.eps = eps; c->gkey.cur = cur0; c->gkey.wcur = wcur0; c->gkey.gmap = c->gmap; c->gkey.unit = unit;
+    return true;
+}
+
+// n executions of the loop body: whole units as graph replays, the rest as direct launches
+void run_iterations(lgf_ctx *c, double alpha, double eps, int64_t n)
+{
+    const int unit = 2 * std::max(1, std::min(c->check_interval, 8) / 2);
+    if (c->graph && !c->profile && n >= unit && graph_ensure(c, alpha, eps, unit)) {
+        while (n >= unit) {
+            if (cudaGraphLaunch(c->gexec, c->st) != cudaSuccess) { cudaGetLastError(); graph_drop(c); c->graph = 0; break; }
+            c->launches += c->g_launches;
+            for (int k = 0; k < LGF_KERNEL_KINDS; k++) c->kcount[k] += c->g_kcount[k];
+            c->wstate = 1;
+            if (c->accum) c->acc_dirty = true;
+            n -= unit;
+        }
+    }
+    for (int64_t i = 0; i < n; i++) do_iteration(c, alpha, eps);
+}
+
 // Kernels launched after the device raised `done` exit without writing, so after a poll the
 // current buffers are those of the `executed`-th iteration since `cur0` / `wcur0`.
 void settle_buffers(lgf_ctx *c, int cur0, int wcur0, long long executed)
@@ -371,6 +429,9 @@ int lgf_set_option(lgf_ctx *ctx, int key, int64_t value)
     case LGF_OPT_ACCUM_G:
         if (value != 0 && value != 1) return fail(ctx, LGF_ERR_INVALID_ARG, "ACCUM_G must be 0 or 1");
         ctx->accum = (int)value; break;
+    case LGF_OPT_GRAPH:
+        if (value != 0 && value != 1) return fail(ctx, LGF_ERR_INVALID_ARG, "GRAPH must be 0 or 1");
+        ctx->graph = (int)value; break;
     case LGF_OPT_PROFILE:
         if (ctx->bound) flush_events(ctx);
         ctx->profile = value ? 1 : 0; break;
@@ -443,6 +504,7 @@ int lgf_bind(lgf_ctx *ctx, void *dev_workspace, size_t bytes, void *cuda_stream)
     ctx->use_gbuf = ctx->fusion && ctx->tiled && ctx->pack == 4 && fft_tiled_gbuf_supported(ctx->N, ctx->prec);
     l2_window_clear(ctx);
     if (ctx->use_gbuf) l2_window_set(ctx);   // one field buffer, used in place by every pass
+    graph_drop(ctx);
     ctx->acc_dirty = false;
     ctx->bound = true;
     ctx->loaded = false;
@@ -455,16 +517,17 @@ int lgf_load_links(lgf_ctx *ctx, const void *src, int src_is_device, int src_lay
     if (!ctx) return LGF_ERR_INVALID_ARG;
     if (!ctx->bound) return fail(ctx, LGF_ERR_NOT_BOUND, "lgf_bind has not been called");
     if (!src) return fail(ctx, LGF_ERR_INVALID_ARG, "src is NULL");
-    if (src_layout != LGF_LAYOUT_AOS) return fail(ctx, LGF_ERR_INVALID_ARG, "unknown layout");
+    if (src_layout != LGF_LAYOUT_AOS && src_layout != LGF_LAYOUT_AOS12) return fail(ctx, LGF_ERR_INVALID_ARG, "unknown layout");
+    const int per = src_layout == LGF_LAYOUT_AOS12 ? 6 : 9;
     const size_t e = elem_bytes(ctx);
     if (src_is_device) {
-        run_kernel(ctx, LGF_KERNEL_LAYOUT, 1, [&] { launch_aos_to_soa(ctx->sa, src, 0, ctx->V, ctx->st); });
+        run_kernel(ctx, LGF_KERNEL_LAYOUT, 1, [&] { launch_aos_to_soa(ctx->sa, src, per, 0, ctx->V, ctx->st); });
     } else {
         char *stg = ctx->base + ctx->lay.staging;
         for (int64_t s0 = 0; s0 < ctx->V; s0 += ctx->lay.staging_sites) {
             const int64_t n = std::min<int64_t>(ctx->lay.staging_sites, ctx->V - s0);
-            CK(cudaMemcpyAsync(stg, (const char *)src + (size_t)s0 * 36 * e, (size_t)n * 36 * e, cudaMemcpyHostToDevice, ctx->st));
-            run_kernel(ctx, LGF_KERNEL_LAYOUT, 1, [&] { launch_aos_to_soa(ctx->sa, stg, s0, n, ctx->st); });
+            CK(cudaMemcpyAsync(stg, (const char *)src + (size_t)s0 * 4 * per * e, (size_t)n * 4 * per * e, cudaMemcpyHostToDevice, ctx->st));
+            run_kernel(ctx, LGF_KERNEL_LAYOUT, 1, [&] { launch_aos_to_soa(ctx->sa, stg, per, s0, n, ctx->st); });
         }
     }
     if (ctx->accum) {
@@ -485,17 +548,18 @@ int lgf_get_links(lgf_ctx *ctx, void *dst, int dst_is_device, int dst_layout)
     int rc = need_loaded(ctx);
     if (rc) return rc;
     if (!dst) return fail(ctx, LGF_ERR_INVALID_ARG, "dst is NULL");
-    if (dst_layout != LGF_LAYOUT_AOS) return fail(ctx, LGF_ERR_INVALID_ARG, "unknown layout");
+    if (dst_layout != LGF_LAYOUT_AOS && dst_layout != LGF_LAYOUT_AOS12) return fail(ctx, LGF_ERR_INVALID_ARG, "unknown layout");
+    const int per = dst_layout == LGF_LAYOUT_AOS12 ? 6 : 9;
     materialise(ctx);
     const size_t e = elem_bytes(ctx);
     if (dst_is_device) {
-        run_kernel(ctx, LGF_KERNEL_LAYOUT, 1, [&] { launch_soa_to_aos(ctx->sa, dst, 0, ctx->V, ctx->st); });
+        run_kernel(ctx, LGF_KERNEL_LAYOUT, 1, [&] { launch_soa_to_aos(ctx->sa, dst, per, 0, ctx->V, ctx->st); });
     } else {
         char *stg = ctx->base + ctx->lay.staging;
         for (int64_t s0 = 0; s0 < ctx->V; s0 += ctx->lay.staging_sites) {
             const int64_t n = std::min<int64_t>(ctx->lay.staging_sites, ctx->V - s0);
-            run_kernel(ctx, LGF_KERNEL_LAYOUT, 1, [&] { launch_soa_to_aos(ctx->sa, stg, s0, n, ctx->st); });
-            CK(cudaMemcpyAsync((char *)dst + (size_t)s0 * 36 * e, stg, (size_t)n * 36 * e, cudaMemcpyDeviceToHost, ctx->st));
+            run_kernel(ctx, LGF_KERNEL_LAYOUT, 1, [&] { launch_soa_to_aos(ctx->sa, stg, per, s0, n, ctx->st); });
+            CK(cudaMemcpyAsync((char *)dst + (size_t)s0 * 4 * per * e, stg, (size_t)n * 4 * per * e, cudaMemcpyDeviceToHost, ctx->st));
         }
     }
     CK(cudaStreamSynchronize(ctx->st));
@@ -529,7 +593,7 @@ int lgf_iterate(lgf_ctx *ctx, double alpha, int64_t n, lgf_result *out)
     }
     run_kernel(ctx, LGF_KERNEL_LAYOUT, 1, [&] { launch_ctrl_reset(ctx->sa, -1.0, ctx->st); });
     const int cur0 = ctx->cur, wcur0 = ctx->wcur;
-    for (int64_t i = 0; i < n; i++) do_iteration(ctx, alpha, -1.0);
+    run_iterations(ctx, alpha, -1.0, n);
     CK(cudaGetLastError());
     if (out) {
         Ctrl h;
@@ -558,7 +622,7 @@ int lgf_fix(lgf_ctx *ctx, double alpha, double eps, lgf_result *out)
     const int cur0 = ctx->cur, wcur0 = ctx->wcur;
     while (!h.done && launched < ctx->max_iter) {
         const int64_t n = std::min<int64_t>(ctx->check_interval, ctx->max_iter - launched);
-        for (int64_t i = 0; i < n; i++) do_iteration(ctx, alpha, eps);
+        run_iterations(ctx, alpha, eps, n);
         launched += n;
         CK(cudaGetLastError());
         if ((rc = read_ctrl(ctx, &h))) return rc;
@@ -702,6 +766,7 @@ int lgf_destroy(lgf_ctx *ctx)
 {
     if (!ctx) return LGF_OK;
     l2_window_clear(ctx);
+    graph_drop(ctx);
     for (auto &p : ctx->evs) { cudaEventDestroy(p.a); cudaEventDestroy(p.b); }
     delete ctx;
     return LGF_OK;

@@ -17,9 +17,9 @@ OK = 0
 ERR_INVALID_ARG, ERR_UNSUPPORTED_SIZE, ERR_NOT_BOUND, ERR_NOT_LOADED = -1, -2, -3, -4
 ERR_WORKSPACE_TOO_SMALL, ERR_CUDA, ERR_NOT_CONVERGED, ERR_NUMERIC = -5, -6, -7, -8
 PREC_FP64, PREC_FP32 = 0, 1
-LAYOUT_AOS = 0
+LAYOUT_AOS, LAYOUT_AOS12 = 0, 1
 OPT_RECON, OPT_FFT_BATCH, OPT_MAX_ITER, OPT_CHECK_INTERVAL, OPT_FFT_PATH, OPT_PROFILE, OPT_FUSION, OPT_L2_PERSIST = 1, 2, 3, 4, 5, 6, 7, 8
-OPT_GMAP, OPT_ACCUM_G = 9, 10
+OPT_GMAP, OPT_ACCUM_G, OPT_GRAPH = 9, 10, 11
 GMAP_FIRST_ORDER, GMAP_EXP = 0, 1
 FIELD_DELTA, FIELD_W, FIELD_G = 0, 1, 2
 STAGE_MEASURE, STAGE_FOURIER, STAGE_UPDATE = 0, 1, 2
@@ -103,7 +103,7 @@ class GaugeFixer:
 
     def __init__(self, N, precision="fp64", recon=18, fft_batch=4, fft_path=0, device="cuda:0",
                  stream=None, max_iter=None, check_interval=None, profile=False, fusion=None, l2_persist=None, gmap=None,
-                 accum_g=None):
+                 accum_g=None, graph=None):
         import torch
 
         self.torch = torch
@@ -128,6 +128,8 @@ class GaugeFixer:
             self.set_option(OPT_GMAP, gmap)
         if accum_g is not None:
             self.set_option(OPT_ACCUM_G, accum_g)
+        if graph is not None:
+            self.set_option(OPT_GRAPH, graph)
         if max_iter is not None:
             self.set_option(OPT_MAX_ITER, max_iter)
         if check_interval is not None:
@@ -184,17 +186,21 @@ class GaugeFixer:
         return self.L.lgf_workspace_bytes(self.ctx)
 
     def load_links(self, U):
-        p, dev, keep = self._src(U, 36)
-        self._ck(self.L.lgf_load_links(self.ctx, p, dev, LAYOUT_AOS))
+        """U: [V,4,3,3] (LAYOUT_AOS) or [V,4,2,3] (LAYOUT_AOS12: rows 0, 1), host or device."""
+        rows2 = tuple(U.shape[-2:]) == (2, 3)
+        p, dev, keep = self._src(U, 24 if rows2 else 36)
+        self._ck(self.L.lgf_load_links(self.ctx, p, dev, LAYOUT_AOS12 if rows2 else LAYOUT_AOS))
         if dev:
             self.stream.synchronize()
 
-    def get_links(self, out=None, device=False):
+    def get_links(self, out=None, device=False, rows=3):
+        """rows = 3: [V,4,3,3] (LAYOUT_AOS); rows = 2: [V,4,2,3] (LAYOUT_AOS12)."""
         if out is None:
-            out = (self.torch.empty((self.V, 4, 3, 3), dtype=self.torch_dtype, device=self.device) if device
-                   else np.empty((self.V, 4, 3, 3), dtype=self.np_dtype))
-        p, dev, keep = self._src(out, 36)
-        self._ck(self.L.lgf_get_links(self.ctx, p, dev, LAYOUT_AOS))
+            out = (self.torch.empty((self.V, 4, rows, 3), dtype=self.torch_dtype, device=self.device) if device
+                   else np.empty((self.V, 4, rows, 3), dtype=self.np_dtype))
+        rows2 = tuple(out.shape[-2:]) == (2, 3)
+        p, dev, keep = self._src(out, 24 if rows2 else 36)
+        self._ck(self.L.lgf_get_links(self.ctx, p, dev, LAYOUT_AOS12 if rows2 else LAYOUT_AOS))
         return out
 
     def measure(self):

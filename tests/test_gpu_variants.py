@@ -243,3 +243,70 @@ def test_exp_convergence_matches_oracle(lgf, exp_oracle, var):
     r0 = gf.iterate(ALPHA, 1)
     assert abs(r0.F - hist[1, 0]) > 1e-7
     gf.close()
+
+
+# ------------------------------------------------------------------ LGF_LAYOUT_AOS12 interchange layout
+@pytest.mark.parametrize("recon", [18, 12])
+@pytest.mark.parametrize("prec", ["fp64", "fp32"])
+def test_aos12_interchange_layout(lgf, recon, prec):
+    """Rows 0, 1 as the exchange format: exact round trip of what was sent, row 2 is
+    conj(row0 x row1), and an iteration from it matches the oracle run on the full links."""
+    import torch
+
+    N, sigma, seed = (8, 8, 8, 8), 0.3, gen.BASE_SEED + 8
+    U = gen.gen_links(N, sigma, seed)
+    cdt = np.complex128 if prec == "fp64" else np.complex64
+    Uc = U.astype(cdt)
+    U12 = np.ascontiguousarray(Uc[:, :, :2, :])
+    gf = lgf.GaugeFixer(N, precision=prec, recon=recon)
+    for src in (U12, torch.from_numpy(U12).cuda()):
+        gf.load_links(src)
+        two = gf.get_links(rows=2)
+        assert two.shape == (8 ** 4, 4, 2, 3) and np.array_equal(two, U12)
+        full = gf.get_links()
+        assert np.array_equal(full[:, :, :2, :], U12)
+        assert np.abs(full[:, :, 2, :] - Uc[:, :, 2, :]).max() < (5e-15 if prec == "fp64" else 1e-6)
+        dev = gf.get_links(device=True, rows=2)
+        assert np.array_equal(dev.cpu().numpy(), U12)
+    r = gf.iterate(ALPHA, 1)
+    Uo = Uc.astype(np.complex128)
+    hist = oracle.iterate(N, Uo, ALPHA, 1)
+    assert np.abs(gf.get_links().astype(np.complex128) - Uo).max() < (1e-12 if prec == "fp64" else 1e-5)
+    assert abs(r.theta - hist[1, 1]) <= (1e-10 if prec == "fp64" else 1e-4) * hist[1, 1]
+    gf.close()
+
+
+# ------------------------------------------------------------------ LGF_OPT_GRAPH: graph replay == direct launches
+@pytest.mark.parametrize("var", [dict(recon=12), dict(recon=18, fft_batch=9), dict(recon=12, fusion=0),
+                                 dict(recon=18, fft_path=1), dict(recon=12, accum_g=1)], ids=vid)
+def test_graph_replay_is_bitwise_the_direct_path(lgf, var):
+    """The captured graph holds the same kernels with the same arguments: histories, links and launch
+    counts are identical, for odd and even iteration counts and across fix / iterate / reload."""
+    n, seed = 8, gen.BASE_SEED + 1008
+    U = gen.gen_links(n, 0.3, seed)
+    a = lgf.GaugeFixer(n, graph=1, **var)
+    b = lgf.GaugeFixer(n, graph=0, **var)
+    for gf in (a, b):
+        gf.load_links(U)
+    for steps in (19, 8, 1):
+        ra, rb = a.iterate(ALPHA, steps), b.iterate(ALPHA, steps)
+        assert ra.iterations == rb.iterations == steps
+        assert ra.F == rb.F and ra.theta == rb.theta
+        assert np.array_equal(a.history(), b.history())
+    assert np.array_equal(a.get_links(), b.get_links())
+    assert a.launch_count() == b.launch_count()
+    ka, kb = a.kernel_times(), b.kernel_times()
+    assert {k: v[1] for k, v in ka.items()} == {k: v[1] for k, v in kb.items()}
+    for gf in (a, b):
+        gf.load_links(U)
+    ra, rb = a.fix(ALPHA, 1e-15), b.fix(ALPHA, 1e-15)
+    assert ra.iterations == rb.iterations and ra.F == rb.F and ra.theta == rb.theta and ra.converged == 1
+    assert np.array_equal(a.history(), b.history())
+    assert np.array_equal(a.get_links(), b.get_links())
+    # a different alpha re-captures; results still those of the direct path
+    for gf in (a, b):
+        gf.load_links(U)
+    ra, rb = a.iterate(0.06, 10), b.iterate(0.06, 10)
+    assert ra.F == rb.F and ra.theta == rb.theta
+    a.close()
+    b.close()
