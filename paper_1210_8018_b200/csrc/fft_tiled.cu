@@ -209,8 +209,11 @@ template <int S> __device__ __forceinline__ void line_of_thread(int t, int &line
     if (S == 1) { line = t; h = 0; }
     else { h = (t >> 4) & 1; line = (t & 15) | ((t >> 5) << 4); }
 }
+// Lines of at least LGF_SPLIT_MIN points are shared by two lanes.  48 and 64 must be (registers);
+// 32 measured 3.6 % faster per iteration at 32^4 FP64 in a same-run A/B (0.3164 vs 0.3279 ms: twice the
+// warps per tile at 84-128 instead of 146-196 registers), profiles/r01e_final.md.
 #ifndef LGF_SPLIT_MIN
-#define LGF_SPLIT_MIN 48
+#define LGF_SPLIT_MIN 32
 #endif
 constexpr int split_of(int n) { return n >= LGF_SPLIT_MIN ? 2 : 1; }
 

@@ -24,7 +24,41 @@ static const int FUSED_THREADS = 128;
 
 // links are streamed: read (twice, the second time from L2) and written once per iteration
 template <typename V> __device__ __forceinline__ V ld_link(const V *p) { return __ldg(p); }
-template <typename V> __device__ __forceinline__ void st_link(V *p, V v) { *p = v; }
+#ifndef LGF_LINK_STCS
+#define LGF_LINK_STCS 0
+#endif
+#ifndef LGF_W_EVICT_LAST
+#define LGF_W_EVICT_LAST 0
+#endif
+template <typename V> __device__ __forceinline__ void st_link(V *p, V v)
+{
+#if LGF_LINK_STCS
+    __stcs(p, v);       // written once, not read again before the next iteration: evict first
+#else
+    *p = v;
+#endif
+}
+// Delta is read back by the first FFT pass right after this kernel: ask L2 to keep it
+__device__ __forceinline__ void st_field(double2 *p, double2 v)
+{
+#if LGF_W_EVICT_LAST
+    unsigned long long pol;
+    asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(pol));
+    asm volatile("st.global.L2::cache_hint.v2.f64 [%0], {%1, %2}, %3;" ::"l"(p), "d"(v.x), "d"(v.y), "l"(pol) : "memory");
+#else
+    *p = v;
+#endif
+}
+__device__ __forceinline__ void st_field(float2 *p, float2 v)
+{
+#if LGF_W_EVICT_LAST
+    unsigned long long pol;
+    asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(pol));
+    asm volatile("st.global.L2::cache_hint.v2.f32 [%0], {%1, %2}, %3;" ::"l"(p), "f"(v.x), "f"(v.y), "l"(pol) : "memory");
+#else
+    *p = v;
+#endif
+}
 
 template <typename T, int NE>
 __device__ __forceinline__ void load_link_in(const cx<T> *__restrict__ links, int64_t V, int mu, int64_t s, cx<T> (&u)[9])
@@ -56,10 +90,10 @@ __device__ __forceinline__ double store_delta(const T (&di)[3], const cx<T> (&E)
     d0 -= m; d1 -= m; d2 -= m;
     const double th = (double)(d0 * d0 + d1 * d1 + d2 * d2) + 2.0 * (double)(cnorm2(E[0]) + cnorm2(E[1]) + cnorm2(E[2]));
     if (PACK == 4) {
-        wout[s] = mk<T>(d0, d1);
-        wout[V + s] = E[0];
-        wout[2 * V + s] = E[1];
-        wout[3 * V + s] = E[2];
+        st_field(wout + s, mk<T>(d0, d1));
+        st_field(wout + V + s, E[0]);
+        st_field(wout + 2 * V + s, E[1]);
+        st_field(wout + 3 * V + s, E[2]);
     } else {
         wout[s] = mk<T>(0, d0);
         wout[V + s] = E[0];
