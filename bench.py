@@ -221,7 +221,7 @@ def run_ours(args):
     torch.cuda.synchronize()
 
     gf = lgf.GaugeFixer(N, precision=prec, recon=recon, fft_batch=args.fft_batch, fft_path=args.fft_path,
-                        fusion=args.fusion, l2_persist=args.l2_persist, accum_g=args.accum_g, gmap=args.gmap,
+                        fusion=args.fusion, l2_persist=args.l2_persist, accum_g=args.accum_g, gmap=args.gmap, graph=args.graph,
                         device=f"cuda:{local}")
     K, W = args.steps, args.warmup
     stream = gf.stream
@@ -397,6 +397,7 @@ def main():
     ap.add_argument("--l2-persist", type=int, default=0, choices=[0, 1])
     ap.add_argument("--accum-g", type=int, default=0, choices=[0, 1],
                     help="LGF_OPT_ACCUM_G: fixed links + accumulated transformation (the link rewrite at the end of the window is timed)")
+    ap.add_argument("--graph", type=int, default=1, choices=[0, 1], help="LGF_OPT_GRAPH (default on)")
     ap.add_argument("--gmap", type=int, default=0, choices=[0, 1], help="LGF_OPT_GMAP: 1 = exact exponential")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cufft-reference", type=int, default=1, choices=[0, 1])

@@ -102,10 +102,12 @@ enum {
                                    FFT_BATCH = 4 and a lattice the tiled FFT covers, else lgf_bind fails with
                                    LGF_ERR_INVALID_ARG.  0 (default): links rewritten every iteration. */
     LGF_OPT_GRAPH = 11          /* 1 (default): lgf_iterate / lgf_fix capture min(CHECK_INTERVAL, 8) (rounded
-                                   down to even, at least 2) iterations into a CUDA graph once and replay
-                                   it, so that small lattices (8^4, 16^4: a few microseconds per kernel) are
-                                   not bound by launch overhead; leftovers and profiled runs (LGF_OPT_PROFILE)
-                                   are launched directly.  Same kernels, same results.  Falls back to direct
+                                   down to even, at least 2) iterations into a CUDA graph and replay it, so
+                                   that small lattices (8^4, 16^4: a few microseconds per kernel) are not
+                                   bound by launch overhead.  The first batch with given (alpha, eps) is
+                                   launched directly and the graph captured behind it (host work hidden by
+                                   the running kernels); later batches and later calls replay it.  Leftovers
+                                   and profiled runs (LGF_OPT_PROFILE) are launched directly.  Same kernels, same results.  Falls back to direct
                                    launches by itself when the bound stream cannot be captured (e.g. the
                                    legacy default stream).  0: always direct launches.  Any time. */
 };

@@ -209,21 +209,25 @@ template <int S> __device__ __forceinline__ void line_of_thread(int t, int &line
     if (S == 1) { line = t; h = 0; }
     else { h = (t >> 4) & 1; line = (t & 15) | ((t >> 5) << 4); }
 }
-// Lines of at least LGF_SPLIT_MIN points are shared by two lanes.  48 and 64 must be (registers);
-// 32 measured 3.6 % faster per iteration at 32^4 FP64 in a same-run A/B (0.3164 vs 0.3279 ms: twice the
-// warps per tile at 84-128 instead of 146-196 registers), profiles/r01e_final.md.
-#ifndef LGF_SPLIT_MIN
-#define LGF_SPLIT_MIN 32
+// Lines of at least SMIN points are shared by two lanes.  48 and 64 must be (registers).  32-point
+// lines are split for FP64 tiles with NA == NB only: a same-run A/B at 32^4 FP64 gave 0.3164 against
+// 0.3279 ms per iteration (twice the warps per tile at 84-128 instead of 146-196 registers), while FP32
+// tiles and the (32, 48) / (32, 64) (z,t) tiles of 32^3 x n lattices got 5-15 % slower
+// (profiles/r01e_final.md).  LGF_SPLIT_MIN overrides the rule for tuning sweeps.
+#ifdef LGF_SPLIT_MIN
+template <typename T> constexpr int split_min(int, int) { return LGF_SPLIT_MIN; }
+#else
+template <typename T> constexpr int split_min(int na, int nb) { return (sizeof(T) == 8 && na == nb) ? 32 : 48; }
 #endif
-constexpr int split_of(int n) { return n >= LGF_SPLIT_MIN ? 2 : 1; }
+constexpr int split_of(int n, int smin) { return n >= smin ? 2 : 1; }
 
 // ---------------------------------------------------------------- tile geometry
 // Shared tile of a group: element (c, a, b) at (b*RS + a*C + c), RS = NA*C + C (one padding
 // column block per row keeps 16-byte accesses of 8 consecutive threads on distinct banks).
 // Lines along a: C*NB of them, SA threads each; lines along b: C*NA, SB threads each.
 constexpr int imax(int a, int b) { return a > b ? a : b; }
-template <int NA, int NB, int C> struct Tile {
-    static constexpr int SA = split_of(NA), SB = split_of(NB);
+template <int NA, int NB, int C, int SMIN> struct Tile {
+    static constexpr int SA = split_of(NA, SMIN), SB = split_of(NB, SMIN);
     static constexpr int RS = NA * C + C;
     static constexpr int ELEMS = RS * NB;
     static constexpr int THREADS = C * imax(SA * NB, SB * NA);
@@ -237,7 +241,7 @@ constexpr int cta_threads(int group) { return group >= 128 ? group : (128 / grou
 // INVERSE = 1: coalesced load into shared memory, Dif(+) along x, shared, Dif(+) along y,
 //              store straight from registers.  Natural order in global memory in both cases.
 template <typename T, int NA, int NB> struct XYCfg {
-    typedef Tile<NA, NB, 1> TL;
+    typedef Tile<NA, NB, 1, split_min<T>(NA, NB)> TL;
     static constexpr int TP = TL::THREADS;             // threads of one plane
     static constexpr int CTA = cta_threads(TP);
     static constexpr int G = CTA / TP;                 // planes per CTA
@@ -328,7 +332,7 @@ k_fft_xy(cx<T> *__restrict__ w, int64_t nplanes, const Ctrl *ctrl)
 // memory: w never goes back to HBM, rows 0, 1 of g (12 reals) do.  The fused link kernel
 // (kernels_fused.cu) then reads g at x and its 8 neighbours instead of rebuilding it 9 times.
 template <typename T, int NA, int NB> struct XYGCfg {
-    typedef Tile<NA, NB, 1> TL;
+    typedef Tile<NA, NB, 1, split_min<T>(NA, NB)> TL;
     // threads of one field of one plane; whole warps when lines are split (the halves shuffle)
     static constexpr int TP = (TL::SA > 1 || TL::SB > 1) ? (TL::THREADS + 31) / 32 * 32 : TL::THREADS;
     static constexpr int TG = 4 * TP;                         // threads of one plane
@@ -455,7 +459,7 @@ k_fft_xy_inv_g(const cx<T> *__restrict__ w, cx<T> *__restrict__ gbuf, int64_t V,
 // transforms each CTA builds g for half of the sites, reading its own two fields locally and
 // the other two from the peer's shared memory (DSMEM).
 template <typename T, int NA, int NB> struct XYG2Cfg {
-    typedef Tile<NA, NB, 1> TL;
+    typedef Tile<NA, NB, 1, split_min<T>(NA, NB)> TL;
     static constexpr int TP = (TL::SA > 1 || TL::SB > 1) ? (TL::THREADS + 31) / 32 * 32 : TL::THREADS;
     static constexpr int CTA = 2 * TP;                        // two fields per CTA
     static constexpr size_t SMEM = (size_t)2 * TL::ELEMS * sizeof(cx<T>);
@@ -552,7 +556,7 @@ k_fft_xy_inv_g2(const cx<T> *__restrict__ w, cx<T> *__restrict__ gbuf, int64_t V
 #define LGF_ZT_MAXB 2   /* 3 measured slower at 32^4 (47.6 vs 45.5 us: spills), equal at 48^4 */
 #endif
 template <typename T, int NA, int NB, int C> struct ZTCfg {
-    typedef Tile<NA, NB, C> TL;
+    typedef Tile<NA, NB, C, split_min<T>(NA, NB)> TL;
     static constexpr int TT = TL::THREADS;
     static constexpr int CTA = cta_threads(TT);
     static constexpr int G = CTA / TT;

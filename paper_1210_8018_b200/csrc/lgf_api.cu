@@ -243,21 +243,25 @@ void graph_drop(lgf_ctx *c)
     c->gexec = nullptr;
 }
 
+bool graph_matches(const lgf_ctx *c, double alpha, double eps, int unit)
+{
+    return c->gexec && c->gkey.alpha == alpha && c->gkey.eps == eps && c->gkey.cur == c->cur && c->gkey.wcur == c->wcur &&
+           c->gkey.gmap == c->gmap && c->gkey.unit == unit;
+}
+
 // Capture `unit` iterations (even: the double buffers are back where they started) into a graph.
 // Kernel arguments (alpha, eps, buffer pointers, g map) are baked in, so they key the cached graph.
-// Any failure switches the graph path off for this context; the direct launches remain.
-bool graph_ensure(lgf_ctx *c, double alpha, double eps, int unit)
+// Nothing is enqueued.  Any failure switches the graph path off for this context; the direct
+// launches remain.
+void graph_capture(lgf_ctx *c, double alpha, double eps, int unit)
 {
-    if (c->gexec && c->gkey.alpha == alpha && c->gkey.eps == eps && c->gkey.cur == c->cur && c->gkey.wcur == c->wcur &&
-        c->gkey.gmap == c->gmap && c->gkey.unit == unit)
-        return true;
     graph_drop(c);
     const int cur0 = c->cur, wcur0 = c->wcur, ws0 = c->wstate;
     const bool dirty0 = c->acc_dirty;
     const int64_t l0 = c->launches;
     int64_t k0[LGF_KERNEL_KINDS];
     for (int k = 0; k < LGF_KERNEL_KINDS; k++) k0[k] = c->kcount[k];
-    if (cudaStreamBeginCapture(c->st, cudaStreamCaptureModeRelaxed) != cudaSuccess) { cudaGetLastError(); c->graph = 0; return false; }
+    if (cudaStreamBeginCapture(c->st, cudaStreamCaptureModeRelaxed) != cudaSuccess) { cudaGetLastError(); c->graph = 0; return; }
     for (int i = 0; i < unit; i++) do_iteration(c, alpha, eps);
     cudaGraph_t g = nullptr;
     cudaError_t e = cudaStreamEndCapture(c->st, &g);
@@ -269,16 +273,19 @@ bool graph_ensure(lgf_ctx *c, double alpha, double eps, int unit)
     sync_ptrs(c);
     if (e == cudaSuccess && g && back) e = cudaGraphInstantiate(&c->gexec, g, 0);
     if (g) cudaGraphDestroy(g);
-    if (e != cudaSuccess || !c->gexec || !back) { cudaGetLastError(); graph_drop(c); c->graph = 0; return false; }
+    if (e != cudaSuccess || !c->gexec || !back) { cudaGetLastError(); graph_drop(c); c->graph = 0; return; }
     c->gkey.alpha = alpha; c->gkey.eps = eps; c->gkey.cur = cur0; c->gkey.wcur = wcur0; c->gkey.gmap = c->gmap; c->gkey.unit = unit;
-    return true;
 }
 
-// n executions of the loop body: whole units as graph replays, the rest as direct launches
+// n executions of the loop body.  With a cached graph of the same arguments: whole units as graph
+// replays, the rest as direct launches.  Without one: direct launches now, and the graph for the
+// next call (or the next poll interval of lgf_fix) is captured afterwards, while the GPU is busy with
+// these launches, so that capture and instantiation never sit in front of the work.
 void run_iterations(lgf_ctx *c, double alpha, double eps, int64_t n)
 {
     const int unit = 2 * std::max(1, std::min(c->check_interval, 8) / 2);
-    if (c->graph && !c->profile && n >= unit && graph_ensure(c, alpha, eps, unit)) {
+    const bool want = c->graph && !c->profile && n >= unit;
+    if (want && graph_matches(c, alpha, eps, unit)) {
         while (n >= unit) {
             if (cudaGraphLaunch(c->gexec, c->st) != cudaSuccess) { cudaGetLastError(); graph_drop(c); c->graph = 0; break; }
             c->launches += c->g_launches;
@@ -287,8 +294,11 @@ void run_iterations(lgf_ctx *c, double alpha, double eps, int64_t n)
             if (c->accum) c->acc_dirty = true;
             n -= unit;
         }
+        for (int64_t i = 0; i < n; i++) do_iteration(c, alpha, eps);
+        return;
     }
     for (int64_t i = 0; i < n; i++) do_iteration(c, alpha, eps);
+    if (want && c->graph) graph_capture(c, alpha, eps, unit);
 }
 
 // Kernels launched after the device raised `done` exit without writing, so after a poll the

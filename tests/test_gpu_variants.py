@@ -310,3 +310,23 @@ def test_graph_replay_is_bitwise_the_direct_path(lgf, var):
     assert ra.F == rb.F and ra.theta == rb.theta
     a.close()
     b.close()
+
+
+def test_graph_falls_back_on_the_legacy_default_stream(lgf):
+    """The legacy default stream cannot be captured: the library must fall back to direct launches by
+    itself and give the same results as on a capturable stream."""
+    import torch
+
+    n, seed = 8, gen.BASE_SEED + 8
+    U = gen.gen_links(n, 0.3, seed)
+    a = lgf.GaugeFixer(n, recon=12, stream=torch.cuda.default_stream())
+    b = lgf.GaugeFixer(n, recon=12)
+    for gf in (a, b):
+        gf.load_links(U)
+    ra, rb = a.iterate(ALPHA, 16), b.iterate(ALPHA, 16)
+    assert ra.iterations == rb.iterations == 16 and ra.F == rb.F and ra.theta == rb.theta
+    ra, rb = a.fix(ALPHA, 1e-15), b.fix(ALPHA, 1e-15)
+    assert ra.iterations == rb.iterations and ra.F == rb.F and ra.converged == 1
+    assert np.array_equal(a.get_links(), b.get_links())
+    a.close()
+    b.close()
