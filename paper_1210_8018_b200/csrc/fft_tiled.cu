@@ -367,6 +367,9 @@ __device__ __forceinline__ void emit_g(cx<T> (&g)[9], const cx<T> (&Gold)[6], cx
 #ifndef LGF_EPI_BATCH
 #define LGF_EPI_BATCH 4
 #endif
+#ifndef LGF_EPI_ALL
+#define LGF_EPI_ALL 0   /* 1: unroll the epilogue by LGF_EPI_BATCH without ACCUM_G too */
+#endif
 
 template <typename T, int NA, int NB, bool ACC>
 __global__ void __launch_bounds__((XYGCfg<T, NA, NB>::CTA))
@@ -428,7 +431,7 @@ k_fft_xy_inv_g(const cx<T> *__restrict__ w, cx<T> *__restrict__ gbuf, int64_t V,
     }
     __syncthreads();
     if (ok) {
-        constexpr int EB = ACC ? LGF_EPI_BATCH : 1;
+        constexpr int EB = (ACC || LGF_EPI_ALL) ? LGF_EPI_BATCH : 1;
         for (int i0 = t; i0 < NA * NB; i0 += EB * TG) {
             cx<T> Gold[EB][6];
             if (ACC) {
@@ -520,7 +523,7 @@ k_fft_xy_inv_g2(const cx<T> *__restrict__ w, cx<T> *__restrict__ gbuf, int64_t V
     const cx<T> *peer = cluster.map_shared_rank(smp, rank ^ 1);
     const cx<T> *f01 = rank == 0 ? smp : peer, *f23 = rank == 0 ? peer : smp;
     constexpr int HALF = NA * NB / 2;
-    constexpr int EB = ACC ? LGF_EPI_BATCH : 1;
+    constexpr int EB = (ACC || LGF_EPI_ALL) ? LGF_EPI_BATCH : 1;
     for (int i0 = rank * HALF + t; i0 < (rank + 1) * HALF; i0 += EB * CF::CTA) {
         cx<T> Gold[EB][6];
         if (ACC) {
