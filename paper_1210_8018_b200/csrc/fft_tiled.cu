@@ -8,9 +8,10 @@
 // (four passes per direction change); here the reorder is tile
 // addressing and the mask and 1/V ride on the middle pass.
 //
-// Every 1D transform is done on a whole line held in registers -- by ONE thread for lengths up
-// to 32, by TWO threads (lanes l and l^16, half a line each, one shuffle exchange) for 48 and
-// 64, where a line would not fit the register file -- as a fully
+// Every 1D transform is done on a whole line held in registers -- by ONE thread for short
+// lines, by TWO threads (lanes l and l^16, half a line each, one shuffle exchange) for 48 and
+// 64, where a line would not fit the register file, and for 32 in FP64 square tiles, where
+// halving the registers doubles the warps per tile (split_min below) -- as a fully
 // unrolled decimation-in-frequency network (natural order in, digit-reversed slots out)
 // with compile-time twiddles; the inverse right after the mask is the transposed
 // (decimation-in-time) network, which takes digit-reversed slots and returns natural order,

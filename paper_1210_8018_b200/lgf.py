@@ -157,6 +157,7 @@ class GaugeFixer:
         if getattr(self, "ctx", None) is not None and self.ctx:
             self.L.lgf_destroy(self.ctx)
             self.ctx = ctypes.c_void_p()
+            self.workspace = None       # hand the device memory back to torch
 
     def __del__(self):
         try:

@@ -373,6 +373,19 @@ def test_full_size_48_fp32(lgf):
     Ufix = gf.get_links()
     assert _unitarity_defect(Ufix) < 5e-5                     # no reunitarisation of links (reading R18)
     assert abs(oracle.plaquette(n, Ufix.astype(np.complex128)) - oracle.plaquette(n, U)) < 1e-5
+    # LGF_OPT_ACCUM_G at the same size (the configuration `bench.py --accum-g 1 --workload 48^4` times)
+    gf.close()
+    ga = fixer(lgf, n, precision="fp32", recon=18, accum_g=1)
+    ga.load_links(U32)
+    ra1 = ga.iterate(ALPHA, 1)
+    assert abs(ra1.F - hist[1, 0]) < 1e-5 and abs(ra1.theta - hist[1, 1]) <= 1e-4 * hist[1, 1]
+    ga.load_links(U32)
+    ra = ga.fix(ALPHA, 1e-12)
+    assert ra.converged == 1 and abs(ra.iterations - r.iterations) <= 2 and abs(ra.F - r.F) < 1e-5
+    Ua = ga.get_links()
+    assert _unitarity_defect(Ua) < 5e-5
+    assert np.abs(Ua - Ufix).max() < 5e-3                     # same minimum; FP32 rounding differs along the way
+    ga.close()
 
 
 @pytest.mark.slow
@@ -411,3 +424,20 @@ def test_full_size_64_fp64(lgf):
     Ufix = gf.get_links()
     assert _unitarity_defect(Ufix) < 1e-12
     assert abs(oracle.plaquette(n, Ufix) - p0) < 1e-12
+    # LGF_OPT_ACCUM_G at the same size against the default path, from the same start (whatever U holds now)
+    gf.load_links(U)
+    rb = gf.fix(ALPHA, 1e-15)
+    Ub = gf.get_links(out=Ufix)
+    gf.close()
+    ga = fixer(lgf, n, recon=18, accum_g=1)
+    ga.load_links(U)
+    ra = ga.fix(ALPHA, 1e-15)
+    assert ra.converged == 1 and ra.iterations == rb.iterations and abs(ra.F - rb.F) <= 1e-10
+    del U
+    Ua = ga.get_links()
+    assert _unitarity_defect(Ua) < 1e-12
+    worst = 0.0
+    for lo in range(0, Ua.shape[0], 1 << 20):
+        worst = max(worst, float(np.abs(Ua[lo:lo + (1 << 20)] - Ub[lo:lo + (1 << 20)]).max()))
+    assert worst < 1e-9
+    ga.close()
