@@ -17,7 +17,10 @@
 
 namespace lgf {
 
-static const int FUSED_THREADS = 128;
+#ifndef LGF_FUSED_THREADS
+#define LGF_FUSED_THREADS 128
+#endif
+static const int FUSED_THREADS = LGF_FUSED_THREADS;
 #ifndef LGF_FUSED_MINB
 #define LGF_FUSED_MINB 4
 #endif
