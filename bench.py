@@ -320,6 +320,32 @@ def run_ours(args):
 
     # ---- side-by-side reference only (never on the product path): cuFFT through torch.fft on the same
     # number of fields, forward + inverse 4D transforms, against the three hand-written passes
+    # ---- the ACCUM_G variant of the same workload, same run, same window (context: faster, moves fewer bytes)
+    variants = None
+    if world == 1 and not args.accum_g and tiled and gf.uses_gbuf() and args.variants:
+        try:
+            ga = lgf.GaugeFixer(N, precision=prec, recon=recon, fft_batch=args.fft_batch, accum_g=1, gmap=args.gmap,
+                                graph=args.graph, device=f"cuda:{local}")
+            ga.load_links(dev)
+            ga.iterate(ALPHA, W)
+            ga.load_links(dev)
+            a0, a1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            torch.cuda.synchronize()
+            with torch.cuda.stream(ga.stream):
+                a0.record(ga.stream)
+                ga.iterate(ALPHA, K, sync=False)
+                ga.sync_links()                 # the one link rewrite belongs to the window
+                a1.record(ga.stream)
+            torch.cuda.synchronize()
+            ams = a0.elapsed_time(a1)
+            variants = {"accum_g": {"ms_per_step": ams / K, "value": V * K / (ams * 1e-3), "unit": UNIT,
+                                    "bytes_per_site_this_build": 4 * recon * real_bytes + 6 * Wb + 3 * 12 * real_bytes,
+                                    "what": "LGF_OPT_ACCUM_G = 1: fixed links + accumulated transformation, link rewrite "
+                                            "inside the window (bench.py --accum-g 1 makes it the timed path)"}}
+            ga.close()
+        except Exception as e:                  # noqa: BLE001
+            variants = {"accum_g": {"unavailable": str(e).splitlines()[0][:160]}}
+
     fft_ref = None
     if tiled and args.cufft_reference:
         try:
@@ -387,6 +413,7 @@ def run_ours(args):
                      "kernels": kern},
         "cpu_baseline": cpu,
         "fft_reference": fft_ref,
+        "variants": variants,
     }
     print(json.dumps(out), flush=True)
     if world > 1:
@@ -407,6 +434,7 @@ def main():
     ap.add_argument("--l2-persist", type=int, default=0, choices=[0, 1])
     ap.add_argument("--accum-g", type=int, default=0, choices=[0, 1],
                     help="LGF_OPT_ACCUM_G: fixed links + accumulated transformation (the link rewrite at the end of the window is timed)")
+    ap.add_argument("--variants", type=int, default=1, choices=[0, 1], help="also time the ACCUM_G variant (N = 1)")
     ap.add_argument("--graph", type=int, default=1, choices=[0, 1], help="LGF_OPT_GRAPH (default on)")
     ap.add_argument("--gmap", type=int, default=0, choices=[0, 1], help="LGF_OPT_GMAP: 1 = exact exponential")
     ap.add_argument("--no-cpu-baseline", action="store_true")

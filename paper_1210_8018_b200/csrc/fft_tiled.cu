@@ -365,11 +365,13 @@ __device__ __forceinline__ void emit_g(cx<T> (&g)[9], const cx<T> (&Gold)[6], cx
 }
 // Sites of the epilogue handled per loop trip: with ACC the loads of G for all of them are issued
 // before the first product, so that the trip pays one memory latency instead of EPI_BATCH.
+// 2: measured best with split 32-point lines (122 registers, two 256-thread CTAs per SM; 4 needs 160
+// registers and leaves one CTA per SM: 70 instead of 56 us at 32^4, profiles/r01e_final.md).
 #ifndef LGF_EPI_BATCH
-#define LGF_EPI_BATCH 4
+#define LGF_EPI_BATCH 2
 #endif
 #ifndef LGF_EPI_ALL
-#define LGF_EPI_ALL 0   /* 1: unroll the epilogue by LGF_EPI_BATCH without ACCUM_G too */
+#define LGF_EPI_ALL 0   /* 1: unroll the epilogue by LGF_EPI_BATCH without ACCUM_G too (measured: no gain) */
 #endif
 
 template <typename T, int NA, int NB, bool ACC>
