@@ -9,8 +9,11 @@ With N > 1 (torchrun) every rank fixes its own lattice (replicas, no data-path c
 DESIGN.md section 9), `value` is the sum over ranks / max time over ranks.
 
 One JSON line on stdout (rank 0).  `value` is device-resident; `e2e` goes through the C ABI
-with pinned HOST buffers (load links, iterate, read the result) every step.
+with pinned HOST buffers every step: lgf_load_links (H2D), lgf_iterate(1), lgf_get_links (D2H);
+`e2e.fix` is the time to solution the same way (load, lgf_fix to theta <= eps, get the links).
 `--impl reference` times the CPU oracle (oracle/) instead, as it stands, on the host cores.
+`--gpus N` without a torchrun environment starts the N ranks itself (re-exec under
+`python -m torch.distributed.run`, rendezvous on 127.0.0.1).
 """
 import argparse
 import json
@@ -36,6 +39,14 @@ WORKLOADS = {
     "48^4": ((48,) * 4, 0.5, 48, "fp32", 18),
     "64^4": ((64,) * 4, 0.6, 64, "fp64", 18),
 }
+
+
+def workload_label(args, prec, recon, seed, sigma):
+    """config.workload: the same string in both arms (--impl ours / reference time the same named workload)."""
+    return (f"{args.workload} periodic SU(3), {prec}, {recon}-real links, {args.fft_batch} FFT fields, "
+            f"alpha={ALPHA}, gen seed {seed}, sigma={sigma}"
+            + (", ACCUM_G (fixed links + accumulated G, link rewrite inside the window)" if args.accum_g else "")
+            + (", g = exp((alpha/2) w)" if args.gmap else ""))
 
 
 def algorithmic_bytes(recon, nfields, real_bytes, tiled, fusion, gbuf, accum=0):
@@ -118,17 +129,27 @@ def peaks():
 
 
 def ncu_traffic(workload_key, kernel):
-    """DRAM bytes per launch of `kernel` from the committed ncu summary (profiles/*_traffic.csv), or None."""
+    """(DRAM bytes per launch of `kernel`, where the number comes from) out of the committed ncu summaries
+    (profiles/*_traffic.csv; the latest file that has the row wins), or (None, None).  The bench run itself
+    cannot measure DRAM traffic (that takes ncu, and a number taken under a profiler is never a bench value),
+    so `traffic_source` names the csv file, the capture the row belongs to and the commit that added the file."""
     import csv
     import glob
 
-    best = None
+    best, src = None, None
     for path in sorted(glob.glob(os.path.join(ROOT, "profiles", "*_traffic.csv"))):
         with open(path) as f:
             for row in csv.DictReader(f):
                 if row["workload"] == workload_key and row["kernel"] == kernel:
                     best = int(row["dram_read_bytes"]) + int(row["dram_write_bytes"])
-    return best
+                    src = {"file": os.path.relpath(path, ROOT), "capture": row.get("capture") or os.path.basename(path).split("_")[0]}
+    if src:
+        try:
+            src["commit"] = subprocess.run(["git", "-C", ROOT, "log", "-1", "--format=%h", "--", src["file"]],
+                                           capture_output=True, text=True, timeout=10).stdout.strip() or None
+        except (OSError, subprocess.SubprocessError):
+            src["commit"] = None
+    return best, src
 
 
 def time_oracle(N, sigma, seed, iters):
@@ -153,9 +174,10 @@ def run_reference(args):
     import gen
 
     N, sigma, soff, prec, recon = WORKLOADS[args.workload]
-    # a step = one oracle iteration on a lattice of the same generator, bounded to 16^4 sites so
-    # that K + W steps end within minutes (a 32^4 oracle iteration takes several seconds)
-    Ns = tuple(min(n, 16) for n in N)
+    # a step = one oracle iteration (about 3 s at 32^4 on one core) on the lattice the line names.  Lattices
+    # above 32^4 (tens of seconds per oracle iteration) are bounded to their 32^4 corner of the same generator,
+    # and config.workload then says so.
+    Ns = tuple(min(n, 32) for n in N)
     seed = gen.BASE_SEED + soff
     import oracle
 
@@ -168,12 +190,17 @@ def run_reference(args):
         oracle.iterate(Ns, U, ALPHA, 1)
     dt = time.perf_counter() - t
     val = Vs * args.steps / dt
-    sample = f"{args.steps} single-thread oracle iterations on {'x'.join(map(str, Ns))} (same generator, sigma={sigma})"
+    sample = f"{args.steps} single-thread oracle iterations on {'x'.join(map(str, Ns))} (same generator, sigma={sigma}, seed {seed})"
+    ran = "x".join(map(str, Ns))
+    workload = workload_label(args, prec, args.recon or recon, seed, sigma)
+    if Ns != tuple(N):
+        workload += f" [oracle timed on its {ran} corner: bounded sample]"
+    sample += "; the oracle as it stands: FP64, 18-real AoS links, one FFT per element of Delta (9), one thread"
     print(json.dumps({
         "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": args.workload, "sample": sample},
+        "config": {"workload": workload, "lattice": list(Ns), "sample": sample},
         "cpu_baseline": {"value": val, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
         "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
@@ -193,6 +220,8 @@ def run_ours(args):
     torch.cuda.set_device(local)
     if world > 1:
         os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        os.environ.setdefault("NCCL_DEBUG", "INFO")          # the communicator log (stderr) shows the ranks that joined
+        os.environ.setdefault("NCCL_DEBUG_SUBSYS", "INIT")
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
 
     from paper_1210_8018_b200 import build as lgf_build
@@ -222,7 +251,7 @@ def run_ours(args):
 
     gf = lgf.GaugeFixer(N, precision=prec, recon=recon, fft_batch=args.fft_batch, fft_path=args.fft_path,
                         fusion=args.fusion, l2_persist=args.l2_persist, accum_g=args.accum_g, gmap=args.gmap, graph=args.graph,
-                        device=f"cuda:{local}")
+                        zblock=args.zblock, zt_pipe=args.zt_pipe, device=f"cuda:{local}")
     K, W = args.steps, args.warmup
     stream = gf.stream
 
@@ -281,17 +310,32 @@ def run_ours(args):
         host12 = torch.empty((V, 4, 2, 3), dtype=tdt).pin_memory()
         host12.copy_(host[:, :, :2, :])
         host = host12
+    host_out = torch.empty_like(host).pin_memory()
     gf.load_links(host.numpy())
+    gf.get_links(out=host_out.numpy())
     barrier()
     te = time.perf_counter()
     for _ in range(e2e_steps):
         gf.load_links(host.numpy())             # H2D of the step's input (4 x per_link complex per site)
         gf.iterate(ALPHA, 1)                    # one iteration + D2H of (iterations, F, theta)
+        gf.get_links(out=host_out.numpy())      # D2H of the step's result: the transformed links, same layout
     torch.cuda.synchronize()
     e2e_s = time.perf_counter() - te
+    # time to solution through the same calls: load -> lgf_fix -> get (how the library is used)
+    barrier()
+    tf2 = time.perf_counter()
+    gf.load_links(host.numpy())
+    r_fix2 = gf.fix(ALPHA, fix_eps, allow_not_converged=True)
+    gf.get_links(out=host_out.numpy())
+    torch.cuda.synchronize()
+    fix_e2e_s = time.perf_counter() - tf2
     clocks = sampler.stop(t0, t1) if sampler else None
+    try:
+        dfma_rate = lgf.debug_dfma_rate(stream.cuda_stream)     # measured FP64 FMA rate: the "alu" denominator
+    except Exception:                                           # noqa: BLE001
+        dfma_rate = None
 
-    (ms_all, e2e_all), _ = replicas.reduce_timing([ms, e2e_s], V * K, device=f"cuda:{local}")
+    (ms_all, e2e_all, fix_e2e_all), _ = replicas.reduce_timing([ms, e2e_s, fix_e2e_s], V * K, device=f"cuda:{local}")
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
@@ -377,14 +421,24 @@ def run_ours(args):
                "sample": f"{iters} oracle iterations on {'x'.join(map(str, Ns))} ({dt:.1f} s, single thread, "
                          f"{os.cpu_count()} cores on the box)"}
 
+    traffic, traffic_src = ncu_traffic(f"{args.workload}-{prec}-recon{recon}-fields{args.fft_batch}", dom)
+    # FP64 instruction counts per site of the two link kernels (cuobjdump -sass of this build, profiles/r02_sass.md)
+    fp64_per_site = {"update_measure": 1722, "measure_acc": 1500}
+    alu = None
+    if dfma_rate:
+        nominal = 148 * 64 * 1.965e9
+        alu = {"peak": dfma_rate, "unit": "FP64 instructions/s (DFMA rate measured by lgf_debug_dfma_rate in this run)",
+               "nominal": nominal, "nominal_what": "148 SMs x 64 DFMA/clk x 1.965 GHz", "kernels": {}}
+        for k in kern:
+            if k in fp64_per_site and prec == "fp64":
+                a = fp64_per_site[k] * V / (kern[k]["us_per_launch"] * 1e-6)
+                alu["kernels"][k] = {"fp64_instructions_per_site": fp64_per_site[k], "achieved": a, "frac": a / dfma_rate}
     out = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
         "ms_per_step": ms_all / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f64" if prec == "fp64" else "f32", "data": "synthetic",
-        "config": {"workload": f"{args.workload} periodic SU(3), {prec}, {recon}-real links, {args.fft_batch} FFT fields, "
-                               f"alpha={ALPHA}, gen seed {gen.BASE_SEED + soff}, sigma={sigma}"
-                               + (", ACCUM_G (fixed links + accumulated G, link rewrite inside the window)" if args.accum_g else "")
-                               + (", g = exp((alpha/2) w)" if args.gmap else ""),
+        "config": {"workload": workload_label(args, prec, recon, gen.BASE_SEED + soff, sigma),
+                   "lattice": list(N), "zblock": gf.zblock(), "zt_pipe": args.zt_pipe,
                    "fft": "tiled register FFT, 3 passes" if tiled else "generic per-axis transform, 8 passes",
                    "l2": "working set (links + fields) exceeds the 126 MB L2" if V >= 32 ** 4 else
                          "working set fits in L2; latency/L2-bound by design (DESIGN.md section 6)",
@@ -393,23 +447,33 @@ def run_ours(args):
                    "fix": {"eps": fix_eps, "iterations": int(r_fix.iterations), "converged": int(r_fix.converged),
                            "F": r_fix.F, "theta": r_fix.theta, "wall_ms": fix_ms}},
         "clocks": clocks,
-        "e2e": {"value": e2e_val, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": 32,
+        "e2e": {"value": e2e_val, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": h2d + 32,
                 "ms_per_step": 1e3 * e2e_all / e2e_steps,
-                "what": "lgf_load_links(pinned host, " + ("12-real rows 0-1 layout" if per_link == 6 else "18-real layout") + ") + lgf_iterate(1) + result readback, every step"},
+                "what": "every step: lgf_load_links(pinned host, " + ("12-real rows 0-1 layout" if per_link == 6 else "18-real layout")
+                        + ") + lgf_iterate(1) with its (iterations, F, theta) readback + lgf_get_links(pinned host, same layout)",
+                "fix": {"what": "time to solution through the same calls: lgf_load_links(host) + lgf_fix(alpha, eps) + lgf_get_links(host)",
+                        "eps": fix_eps, "iterations": int(r_fix2.iterations), "converged": int(r_fix2.converged),
+                        "ms": 1e3 * fix_e2e_all, "value": world * V * int(r_fix2.iterations) / fix_e2e_all, "unit": UNIT,
+                        "h2d_bytes": h2d, "d2h_bytes": h2d + 32}},
         "gpu_launches": int(launches),
         "roofline": {"bound": "hbm", "kernel": dom, "achieved": kern[dom]["GBps"], "peak": peak, "unit": "GB/s",
                      "frac": kern[dom]["GBps"] / peak,
-                     **({"note": "measure_acc is bound by plain FP64 arithmetic (ncu: FP64 pipe 67 %, DRAM 51 %, "
-                                 "profiles/r01d_accum_g.md): about 1500 FP64 instructions per site against a nominal "
-                                 "148 SMs x 64 DFMA/clk x 1.965 GHz = 18.6e12/s give "
-                                 f"{1500 * V / (kern[dom]['us_per_launch'] * 1e-6) / 18.6e12:.2f} of the ALU peak"}
-                        if dom == "measure_acc" else {}),
-                     "traffic": ncu_traffic(f"{args.workload}-{prec}-recon{recon}-fields{args.fft_batch}", dom),
+                     "traffic": traffic, "traffic_source": traffic_src,
                      "algorithmic_bytes": per[dom] * V, "peak_source": peak_src,
                      "bytes_per_site": per[dom],
-                     "iteration": {"bytes_per_site": iter_bytes, "bytes_per_site_this_build": moved_bytes, "GBps": iter_bytes * V * K / (ms_all * 1e-3) / 1e9,
-                                   "frac": iter_bytes * V * K / (ms_all * 1e-3) / 1e9 / peak,
+                     # the whole iteration against the bytes THIS build must move (sum of the kernels' algorithmic
+                     # bytes); the three-kernel yardstick of SURVEY 8(d) (3 L + 8 W) is kept as a separate, named field
+                     "iteration": {"bytes_per_site": moved_bytes, "GBps": moved_bytes * V * K / (ms_all * 1e-3) / 1e9,
+                                   "frac": moved_bytes * V * K / (ms_all * 1e-3) / 1e9 / peak,
+                                   "survey_yardstick": {"bytes_per_site": iter_bytes,
+                                                        "GBps_equivalent": iter_bytes * V * K / (ms_all * 1e-3) / 1e9,
+                                                        "frac_equivalent": iter_bytes * V * K / (ms_all * 1e-3) / 1e9 / peak,
+                                                        "what": "SURVEY 8(d) row for this config (3 L + 8 W bytes per site): what a "
+                                                                "three-kernel design would have to move in the same time; not real traffic"},
                                    "ms_profiled": ms_prof / K},
+                     # second roofline, plain FP64 arithmetic: FP64 instructions per site of the link kernels (SASS
+                     # count, profiles/) against the DFMA rate measured in this run by lgf_debug_dfma_rate
+                     "alu": alu,
                      "kernels": kern},
         "cpu_baseline": cpu,
         "fft_reference": fft_ref,
@@ -418,6 +482,49 @@ def run_ours(args):
     print(json.dumps(out), flush=True)
     if world > 1:
         dist.destroy_process_group()
+
+
+def run_launch_selftest(args):
+    """--launch-selftest: what `--gpus N` starts, without the lattice work: every rank joins the process
+    group (nccl on GPUs, gloo when there is none: the CPU test of the launcher), the step-time reduction
+    of DESIGN.md section 9 runs once, rank 0 prints how many ranks took part."""
+    import torch
+    import torch.distributed as dist
+
+    from paper_1210_8018_b200 import replicas
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    cuda = torch.cuda.is_available() and torch.cuda.device_count() >= world
+    if world > 1:
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        if cuda:
+            torch.cuda.set_device(local)
+            dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+        else:
+            dist.init_process_group("gloo")
+    times, units = replicas.reduce_timing([1.0 + rank], 1.0, device=f"cuda:{local}" if cuda else "cpu")
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+    if rank == 0:
+        print(json.dumps({"launch_selftest": True, "n_gpus": world, "ranks_counted": int(units), "max_ms": times[0],
+                          "backend": "nccl" if cuda else "gloo"}), flush=True)
+
+
+def spawn_ranks(n):
+    """`python bench.py --gpus N` outside torchrun: start the N ranks (one per GPU) by re-executing this
+    command line under `python -m torch.distributed.run` with a rendezvous on 127.0.0.1, pass their
+    output through and return their exit code.  Rank 0 prints the JSON line."""
+    import socket
+
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={n}",
+           "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+    return subprocess.call(cmd)
 
 
 def main():
@@ -439,9 +546,18 @@ def main():
     ap.add_argument("--gmap", type=int, default=0, choices=[0, 1], help="LGF_OPT_GMAP: 1 = exact exponential")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cufft-reference", type=int, default=1, choices=[0, 1])
+    ap.add_argument("--zblock", type=int, default=None, help="LGF_OPT_ZBLOCK (default: chosen from the L2 size)")
+    ap.add_argument("--zt-pipe", type=int, default=None, choices=[0, 1], help="LGF_OPT_ZT_PIPE")
+    ap.add_argument("--launch-selftest", action="store_true", help="start the ranks, reduce one timing, print the rank count")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
-    if args.impl == "reference":
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        sys.exit(spawn_ranks(args.gpus))
+    if "WORLD_SIZE" in os.environ and int(os.environ["WORLD_SIZE"]) != args.gpus:
+        raise SystemExit(f"bench.py: --gpus {args.gpus} but WORLD_SIZE={os.environ['WORLD_SIZE']}")
+    if args.launch_selftest:
+        run_launch_selftest(args)
+    elif args.impl == "reference":
         run_reference(args)
     else:
         run_ours(args)

@@ -101,7 +101,7 @@ enum {
                                    per-iteration link write; one link buffer instead of two.  Needs FUSION = 1,
                                    FFT_BATCH = 4 and a lattice the tiled FFT covers, else lgf_bind fails with
                                    LGF_ERR_INVALID_ARG.  0 (default): links rewritten every iteration. */
-    LGF_OPT_GRAPH = 11          /* 1 (default): lgf_iterate / lgf_fix capture min(CHECK_INTERVAL, 8) (rounded
+    LGF_OPT_GRAPH = 11,         /* 1 (default): lgf_iterate / lgf_fix capture min(CHECK_INTERVAL, 8) (rounded
                                    down to even, at least 2) iterations into a CUDA graph and replay it, so
                                    that small lattices (8^4, 16^4: a few microseconds per kernel) are not
                                    bound by launch overhead.  The first batch with given (alpha, eps) is
@@ -110,6 +110,21 @@ enum {
                                    and profiled runs (LGF_OPT_PROFILE) are launched directly.  Same kernels, same results.  Falls back to direct
                                    launches by itself when the bound stream cannot be captured (e.g. the
                                    legacy default stream).  0: always direct launches.  Any time. */
+    LGF_OPT_ZBLOCK = 12,        /* order in which the per-site kernels (measure, update, fused link kernel) walk
+                                   the lattice: the (z,t) planes are visited in blocks of ZBLOCK consecutive z,
+                                   all Nt time slices of a z-block before the next one, so that the -mu / +mu
+                                   neighbours of a site (Alg. 1 lines 12-16) were touched a few
+                                   planes ago and are still in L2 even when one time slice of links is larger
+                                   than L2 (64^4).  0 (default): chosen by lgf_bind from the L2 size of the device
+                                   (the largest divisor of Nz whose block of planes takes at most about a third
+                                   of L2); a positive value must divide Nz (Nz = plain storage order).  Changes
+                                   only the order of the FP64 partial sums of F and theta (1e-16 relative), not
+                                   what is computed.  Before lgf_bind. */
+    LGF_OPT_ZT_PIPE = 13        /* middle pass of the tiled FFT ((z,t) forward, mask, (z,t) inverse; Alg. 1 lines 3-8,
+                                   PAPER.md:80-90).  1: persistent CTAs that keep their shared-memory tile and fetch
+                                   the next tile with asynchronous copies (cp.async) while the current one is
+                                   finished; 0: one tile per thread group, loaded straight into registers.  Same
+                                   arithmetic in the same order: bitwise the same w.  Any time. */
 };
 
 /* lgf_get_field / lgf_set_field selectors */
@@ -196,7 +211,11 @@ int lgf_get_field(lgf_ctx *ctx, int which, double alpha, void *dst, int dst_is_d
 int lgf_set_field(lgf_ctx *ctx, int which, const void *src, int src_is_device);
 
 /* (F, theta) after the initial measure and after each iteration of the last lgf_fix /
- * lgf_iterate call: up to cap pairs into host arrays F[], theta[]; *n (host) = pairs written. */
+ * lgf_iterate call: up to cap pairs into host arrays F[], theta[]; *n (host) = pairs written.
+ * The device keeps the first LGF_HISTORY_CAP = 4096 pairs of a call only (iterations 0..4095): a run
+ * that takes more iterations (MAX_ITER defaults to 100000) returns the truncated prefix, *n <= 4096,
+ * while lgf_result still carries the true iteration count and the final F, theta. */
+#define LGF_HISTORY_CAP 4096
 int lgf_history(lgf_ctx *ctx, double *F, double *theta, int cap, int *n);
 
 /* With LGF_OPT_PROFILE = 1: total milliseconds and launch count of one kernel kind since
@@ -212,11 +231,20 @@ int lgf_uses_tiled_fft(const lgf_ctx *ctx);
  * shared memory of one SM or of a 2-CTA cluster), 0 if g is rebuilt from w by the link kernel.
  * Valid after lgf_bind. */
 int lgf_uses_gbuf(const lgf_ctx *ctx);
+/* The z-block of the site walk in use (LGF_OPT_ZBLOCK after lgf_bind resolved 0 = auto); 0 before lgf_bind. */
+int lgf_zblock(const lgf_ctx *ctx);
 
 /* LGF_OPT_ACCUM_G: bring the link buffer up to date now, U_mu(x) <- G(x) U_mu(x) G^dagger(x+mu), G <- 1
  * (two launches on the bound stream, asynchronous; the calls that read the links do this
  * themselves).  No-op, LGF_OK, when nothing is pending or ACCUM_G is off.  Needs loaded links. */
 int lgf_sync_links(lgf_ctx *ctx);
+
+/* Debug entry point, not on the gauge-fixing path: the measured FP64 fused-multiply-add rate of the
+ * current device (DFMA per second, best of 4 timed launches of a register-only FMA kernel on the given
+ * stream, a cudaStream_t passed as void*, may be NULL).  bench.py uses it as the denominator of the "alu"
+ * roofline of the one kernel that is bound by FP64 arithmetic (Table 1 flop counts).
+ * Allocates and frees 8 bytes of device memory; synchronises.  *dfma_per_second: host. */
+int lgf_debug_dfma_rate(void *cuda_stream, double *dfma_per_second);
 
 /* Text of the last error of this context (or of lgf_create when ctx == NULL). Never NULL. */
 const char *lgf_last_error(const lgf_ctx *ctx);

@@ -15,7 +15,12 @@ CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "liblgf.so")
 INCLUDE = os.path.join(os.path.dirname(HERE), "include")
-SOURCES = ["lgf_api.cu", "kernels_site.cu", "kernels_fused.cu", "fft_generic.cu", "fft_tiled.cu"]
+ZT_EXTENTS = [8, 12, 16, 24, 32, 48, 64]
+# (source, extra flags, object name); fft_zt_inst.cu is compiled once per Nz (the (z,t) pass of the tiled FFT
+# for that Nz and every Nt), so that the 7 x 7 extent pairs build in parallel
+SOURCES = [(f, [], f.replace(".cu", ".o")) for f in
+           ["lgf_api.cu", "kernels_site.cu", "kernels_fused.cu", "fft_generic.cu", "fft_tiled.cu", "microbench.cu"]]
+SOURCES += [("fft_zt_inst.cu", [f"-DLGF_ZT_NA={n}"], f"fft_zt_na{n}.o") for n in ZT_EXTENTS]
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
     "-Xcompiler", "-fPIC", "-Wno-deprecated-gpu-targets", "-I", INCLUDE,
@@ -45,20 +50,21 @@ def build(force: bool = False, verbose: bool = False) -> str:
     os.makedirs(OBJ, exist_ok=True)
     nvcc = _nvcc()
 
-    def compile_one(src):
-        obj = os.path.join(OBJ, src.replace(".cu", ".o"))
+    def compile_one(item):
+        src, flags, objname = item
+        obj = os.path.join(OBJ, objname)
         if not force and os.path.exists(obj) and os.path.getmtime(obj) >= newest:
             return obj
-        extra = os.environ.get("LGF_EXTRA_NVCC_FLAGS", "").split()    # tuning experiments (-DLGF_FUSED_NBUF=3 ...)
+        extra = flags + os.environ.get("LGF_EXTRA_NVCC_FLAGS", "").split()    # tuning macros of csrc/*.cu for same-run A/B builds (-DLGF_FUSED_BWD_REV=1 ...)
         cmd = [nvcc] + NVCC_FLAGS + extra + (["-Xptxas", "-v"] if verbose else []) + ["-c", os.path.join(CSRC, src), "-o", obj]
         r = subprocess.run(cmd, capture_output=True, text=True)
         if verbose or r.returncode:
             sys.stderr.write(r.stdout + r.stderr)
         if r.returncode:
-            raise RuntimeError(f"nvcc failed on {src}")
+            raise RuntimeError(f"nvcc failed on {src} {' '.join(flags)}")
         return obj
 
-    with ThreadPoolExecutor(max_workers=len(SOURCES)) as ex:
+    with ThreadPoolExecutor(max_workers=min(len(SOURCES), os.cpu_count() or 4)) as ex:
         objs = list(ex.map(compile_one, SOURCES))
     subprocess.check_call([nvcc, "-shared", "-o", LIB] + objs + ["-lcudart"])
     return LIB

@@ -85,6 +85,7 @@ struct Geom {
     int N[4];        // Nx, Ny, Nz, Nt
     int64_t V;       // sites
     int64_t st[4];   // site-index stride of each direction: 1, Nx, Nx*Ny, Nx*Ny*Nz
+    int zb;          // z-block of the site walk (divides Nz; Nz = plain lexicographic order), see walk_site
 };
 
 __device__ __forceinline__ void site_coords(const Geom &g, int64_t s, int c[4])
@@ -96,11 +97,36 @@ __device__ __forceinline__ void site_coords(const Geom &g, int64_t s, int c[4])
     c[3] = (int)u;
 }
 
+// Walk order of the per-site kernels: grid thread r (= blockIdx.x * blockDim.x + threadIdx.x) -> site.
+// Inside one (z,t) plane the order is the storage order (x fastest), so warps still read contiguous
+// runs.  The planes are visited in blocks of geo.zb consecutive z: all Nt time slices of one z-block
+// before the next z-block,
+//     r -> (o, q) = (r mod NxNy, r div NxNy),   q -> (zblk, t, zin),   z = zblk*zb + zin.
+// CTAs that are resident together then cover neighbouring z AND neighbouring t: the -t and +t
+// neighbours of a site are zb planes away in the walk instead of Nz planes, so that the re-reads of
+// U_nu(x-nu), g(x-nu), g(x+mu) (Alg. 1 lines 12-16) are L2 hits even when one time
+// slice of links is larger than L2 (64^4: 151 MB per slice).  Only the first
+// plane of a z-block misses its -z neighbours (1/zb of the sites).  zb = Nz is the lexicographic order.
+// Returns the site index and fills c[0..3]; valid for r < V.
+__device__ __forceinline__ int64_t walk_site(const Geom &g, int64_t r, int c[4])
+{
+    const unsigned P = (unsigned)(g.N[0] * g.N[1]);
+    const unsigned u = (unsigned)r;          // V <= 64^4 = 2^24
+    const unsigned o = u % P, q = u / P;
+    c[0] = (int)(o % (unsigned)g.N[0]);
+    c[1] = (int)(o / (unsigned)g.N[0]);
+    const unsigned per = (unsigned)(g.zb * g.N[3]);
+    const unsigned zblk = q / per, rem = q % per;
+    c[3] = (int)(rem / (unsigned)g.zb);
+    c[2] = (int)(zblk * (unsigned)g.zb + rem % (unsigned)g.zb);
+    return (int64_t)o + (int64_t)P * (c[2] + g.N[2] * c[3]);
+}
+
 // ---------------------------------------------------------------- device control block
 // One per context, in the workspace.  The stop decision of Algorithm 1 is
 // taken by the last block of kernel (a) and kept here, so that the host need not read
 // theta back after every iteration.
-#define LGF_HIST_CAP 4096
+#define LGF_HIST_CAP 4096   /* = LGF_HISTORY_CAP of include/lgf.h (static_assert in lgf_api.cu) */
 struct Ctrl {
     double F;                 // eq. 1.1 of the current links
     double theta;             // eq. 1.4

@@ -19,222 +19,11 @@
 // addressing and for the mask.  Lines along the second axis of a tile go through shared
 // memory (padded rows, conflict-free for 16-byte accesses); the first axis of a pass is
 // loaded straight from global memory into registers and the last one stored straight back.
-#include "launch.h"
-#include "twiddles.cuh"
+#include "fft_lines.cuh"
 #include "su3.cuh"
 #include <cooperative_groups.h>
 
 namespace lgf {
-
-// ---------------------------------------------------------------- twiddles
-// exp(SIGN 2 pi i k / L) from the literal tables; L divides 64 or 48.
-template <typename T, int L, int SIGN> __device__ __forceinline__ cx<T> twiddle(int k)
-{
-    constexpr bool b64 = (64 % L == 0);
-    constexpr int B = b64 ? 64 : 48;
-    static_assert(B % L == 0, "line length must divide 64 or 48");
-    const int i = (k % L) * (B / L);
-    const double c = b64 ? TW_COS64[b64 ? i : 0] : TW_COS48[b64 ? 0 : i];
-    const double s = b64 ? TW_SIN64[b64 ? i : 0] : TW_SIN48[b64 ? 0 : i];
-    return mk<T>((T)c, (T)(SIGN * s));
-}
-
-// x * exp(SIGN 2 pi i k / L), trivial factors resolved at compile time (k is known after unrolling)
-template <typename T, int L, int SIGN> __device__ __forceinline__ cx<T> mul_tw(cx<T> x, int k)
-{
-    k %= L;
-    if (k == 0) return x;
-    if (2 * k == L) return mk<T>(-x.x, -x.y);
-    if (4 * k == L) return SIGN > 0 ? mk<T>(-x.y, x.x) : mk<T>(x.y, -x.x);       // * (+-i)
-    if (4 * k == 3 * L) return SIGN > 0 ? mk<T>(x.y, -x.x) : mk<T>(-x.y, x.x);   // * (-+i)
-    return cmul(x, twiddle<T, L, SIGN>(k));
-}
-
-// ---------------------------------------------------------------- radix-p butterflies
-template <typename T, int SIGN> __device__ __forceinline__ void bfly3(cx<T> &a0, cx<T> &a1, cx<T> &a2)
-{
-    const T h = (T)0.86602540378443865; // sqrt(3)/2
-    const cx<T> t1 = a1 + a2;
-    const cx<T> t2 = mk<T>(a0.x - (T)0.5 * t1.x, a0.y - (T)0.5 * t1.y);
-    const cx<T> d = a1 - a2;
-    // SIGN * i * h * d
-    const cx<T> t3 = SIGN > 0 ? mk<T>(-h * d.y, h * d.x) : mk<T>(h * d.y, -h * d.x);
-    a0 = a0 + t1;
-    a1 = t2 + t3;
-    a2 = t2 - t3;
-}
-
-// One decimation-in-frequency stage on blocks of length L (L = p m): butterfly over the p
-// sub-blocks, then multiply sub-block q by exp(SIGN 2 pi i j q / L); recurse on length m.
-template <typename T, int N, int L, int SIGN> struct Dif {
-    static __device__ __forceinline__ void run(cx<T> (&x)[N])
-    {
-        constexpr int p = (L % 2 == 0) ? 2 : 3;
-        constexpr int m = L / p;
-#pragma unroll
-        for (int b = 0; b < N; b += L)
-#pragma unroll
-            for (int j = 0; j < m; j++) {
-                if (p == 2) {
-                    const cx<T> a = x[b + j], c = x[b + j + m];
-                    x[b + j] = a + c;
-                    x[b + j + m] = mul_tw<T, L, SIGN>(a - c, j);
-                } else {
-                    bfly3<T, SIGN>(x[b + j], x[b + j + m], x[b + j + 2 * m]);
-                    x[b + j + m] = mul_tw<T, L, SIGN>(x[b + j + m], j);
-                    x[b + j + 2 * m] = mul_tw<T, L, SIGN>(x[b + j + 2 * m], 2 * j);
-                }
-            }
-        Dif<T, N, m, SIGN>::run(x);
-    }
-};
-template <typename T, int N, int SIGN> struct Dif<T, N, 1, SIGN> {
-    static __device__ __forceinline__ void run(cx<T> (&)[N]) {}
-};
-
-// The transposed network: stages in the opposite order, twiddles before the butterfly.
-// Takes the slot order Dif produces and returns natural order.
-template <typename T, int N, int L, int SIGN> struct Dit {
-    static __device__ __forceinline__ void run(cx<T> (&x)[N])
-    {
-        constexpr int p = (L % 2 == 0) ? 2 : 3;
-        constexpr int m = L / p;
-        Dit<T, N, m, SIGN>::run(x);
-#pragma unroll
-        for (int b = 0; b < N; b += L)
-#pragma unroll
-            for (int j = 0; j < m; j++) {
-                if (p == 2) {
-                    const cx<T> a = x[b + j], c = mul_tw<T, L, SIGN>(x[b + j + m], j);
-                    x[b + j] = a + c;
-                    x[b + j + m] = a - c;
-                } else {
-                    x[b + j + m] = mul_tw<T, L, SIGN>(x[b + j + m], j);
-                    x[b + j + 2 * m] = mul_tw<T, L, SIGN>(x[b + j + 2 * m], 2 * j);
-                    bfly3<T, SIGN>(x[b + j], x[b + j + m], x[b + j + 2 * m]);
-                }
-            }
-    }
-};
-template <typename T, int N, int SIGN> struct Dit<T, N, 1, SIGN> {
-    static __device__ __forceinline__ void run(cx<T> (&)[N]) {}
-};
-
-// frequency index held by slot s after Dif<N> (mixed-radix digit reversal)
-template <int N> __host__ __device__ constexpr int slot_freq(int s)
-{
-    int L = N, k = 0, mult = 1;
-    while (L > 1) {
-        const int p = (L % 2 == 0) ? 2 : 3, m = L / p;
-        k += (s / m) * mult;
-        s %= m;
-        mult *= p;
-        L = m;
-    }
-    return k;
-}
-
-// ---------------------------------------------------------------- a line held by S threads
-// S = 1: one thread holds the whole line.  S = 2: the line is shared by the lanes l and l^16 of
-// a warp (half h = 0, 1).  The first radix-2 stage of the decimation-in-frequency network,
-//     y[j] = x[j] + x[j+N/2],   z[j] = (x[j] - x[j+N/2]) exp(SIGN 2 pi i j/N),   j < N/2,
-// is done on the pairs each thread holds (j in [h N/4, (h+1) N/4)); then the two threads swap
-// half of their results by warp shuffle so that h = 0 owns all of y (even frequencies) and
-// h = 1 all of z (odd frequencies), and each runs the N/2-point network on its own.
-// The transposed (decimation-in-time) network runs the same steps backwards.
-// nat(i, h): line position held in local element i on the natural-order side;
-// slot(s, h): frequency (or position, for an inverse written as Dif) held in local slot s on the other side.
-template <typename T, int N, int S> struct Line;
-
-template <typename T, int N> struct Line<T, N, 1> {
-    static constexpr int NL = N;
-    static __device__ __forceinline__ int nat(int i, int) { return i; }
-    static __device__ __forceinline__ int slot(int s, int) { return slot_freq<N>(s); }
-    template <int SIGN> static __device__ __forceinline__ void dif(cx<T> (&v)[NL], int, unsigned) { Dif<T, N, N, SIGN>::run(v); }
-    template <int SIGN> static __device__ __forceinline__ void dit(cx<T> (&v)[NL], int, unsigned) { Dit<T, N, N, SIGN>::run(v); }
-};
-
-template <typename V> __device__ __forceinline__ V shfl16(unsigned mask, V v)
-{
-    v.x = __shfl_xor_sync(mask, v.x, 16);
-    v.y = __shfl_xor_sync(mask, v.y, 16);
-    return v;
-}
-// x * (SIGN i)
-template <int SIGN, typename V> __device__ __forceinline__ V rot90(V x)
-{
-    V r;
-    if (SIGN > 0) { r.x = -x.y; r.y = x.x; } else { r.x = x.y; r.y = -x.x; }
-    return r;
-}
-
-template <typename T, int N> struct Line<T, N, 2> {
-    static_assert(N % 4 == 0, "split lines need N divisible by 4");
-    static constexpr int NL = N / 2, Q = N / 4;
-    static __device__ __forceinline__ int nat(int i, int h) { return h * Q + i + (i >= Q ? Q : 0); }
-    static __device__ __forceinline__ int slot(int s, int h) { return 2 * slot_freq<NL>(s) + h; }
-    template <int SIGN> static __device__ __forceinline__ void dif(cx<T> (&v)[NL], int h, unsigned mask)
-    {
-#pragma unroll
-        for (int i = 0; i < Q; i++) {
-            const cx<T> a = v[i], b = v[Q + i];
-            const cx<T> y = a + b;
-            cx<T> z = mul_tw<T, N, SIGN>(a - b, i);
-            if (h) z = rot90<SIGN>(z);                       // exp(SIGN 2 pi i (N/4)/N) = SIGN i
-            const cx<T> got = shfl16(mask, h ? y : z);       // h = 0 gives z away, h = 1 gives y away
-            v[i] = h ? got : y;
-            v[Q + i] = h ? z : got;
-        }
-        Dif<T, NL, NL, SIGN>::run(v);
-    }
-    template <int SIGN> static __device__ __forceinline__ void dit(cx<T> (&v)[NL], int h, unsigned mask)
-    {
-        Dit<T, NL, NL, SIGN>::run(v);
-#pragma unroll
-        for (int i = 0; i < Q; i++) {
-            const cx<T> got = shfl16(mask, h ? v[i] : v[Q + i]);
-            const cx<T> y = h ? got : v[i];
-            cx<T> z = h ? v[Q + i] : got;
-            z = mul_tw<T, N, SIGN>(z, i);
-            if (h) z = rot90<SIGN>(z);
-            v[i] = y + z;
-            v[Q + i] = y - z;
-        }
-    }
-};
-
-// thread t of a group -> (line, half).  S = 2 keeps the two halves of a line 16 lanes apart, so
-// that the 8 lanes of a shared-memory wavefront still belong to 8 consecutive lines.
-template <int S> __device__ __forceinline__ void line_of_thread(int t, int &line, int &h)
-{
-    if (S == 1) { line = t; h = 0; }
-    else { h = (t >> 4) & 1; line = (t & 15) | ((t >> 5) << 4); }
-}
-// Lines of at least SMIN points are shared by two lanes.  48 and 64 must be (registers).  32-point
-// lines are split for FP64 tiles with NA == NB only: a same-run A/B at 32^4 FP64 gave 0.3164 against
-// 0.3279 ms per iteration (twice the warps per tile at 84-128 instead of 146-196 registers), while FP32
-// tiles and the (32, 48) / (32, 64) (z,t) tiles of 32^3 x n lattices got 5-15 % slower
-// (profiles/r01e_final.md).  LGF_SPLIT_MIN overrides the rule for tuning sweeps.
-#ifdef LGF_SPLIT_MIN
-template <typename T> constexpr int split_min(int, int) { return LGF_SPLIT_MIN; }
-#else
-template <typename T> constexpr int split_min(int na, int nb) { return (sizeof(T) == 8 && na == nb) ? 32 : 48; }
-#endif
-constexpr int split_of(int n, int smin) { return n >= smin ? 2 : 1; }
-
-// ---------------------------------------------------------------- tile geometry
-// Shared tile of a group: element (c, a, b) at (b*RS + a*C + c), RS = NA*C + C (one padding
-// column block per row keeps 16-byte accesses of 8 consecutive threads on distinct banks).
-// Lines along a: C*NB of them, SA threads each; lines along b: C*NA, SB threads each.
-constexpr int imax(int a, int b) { return a > b ? a : b; }
-template <int NA, int NB, int C, int SMIN> struct Tile {
-    static constexpr int SA = split_of(NA, SMIN), SB = split_of(NB, SMIN);
-    static constexpr int RS = NA * C + C;
-    static constexpr int ELEMS = RS * NB;
-    static constexpr int THREADS = C * imax(SA * NB, SB * NA);
-};
-// CTA size: at least 128 threads, whole groups
-constexpr int cta_threads(int group) { return group >= 128 ? group : (128 / group) * group; }
 
 // ---------------------------------------------------------------- pass 0 / pass 2: (x,y) planes
 // INVERSE = 0: load columns (lines along y) straight from global, Dif along y, through shared
@@ -552,110 +341,7 @@ k_fft_xy_inv_g2(const cx<T> *__restrict__ w, cx<T> *__restrict__ gbuf, int64_t V
     cluster.sync();                                          // the peer may still be reading this CTA's fields
 }
 
-// ---------------------------------------------------------------- pass 1: (z,t) tiles
-// Tile = C consecutive x at fixed (field, y): element (c, z, t) at global x0 + c + sz*z + st*t.
-// z-lines straight from global (thread = (c, t)), Dif(-) along z -> shared; t-lines from
-// shared (thread = (c, kz)): Dif(-), mask, Dit(+) -> shared; z-lines from shared: Dif(+),
-// stored straight to global.  p^2 = sum_mu 4 sin^2(pi k_mu/N_mu) (reading R5) from the
-// per-axis tables; the factor p_max^2/(p^2 V) is one FP64 division per mode.
-#ifndef LGF_ZT_MAXB
-#define LGF_ZT_MAXB 2   /* 3 measured slower at 32^4 (47.6 vs 45.5 us: spills), equal at 48^4 */
-#endif
-template <typename T, int NA, int NB, int C> struct ZTCfg {
-    typedef Tile<NA, NB, C, split_min<T>(NA, NB)> TL;
-    static constexpr int TT = TL::THREADS;
-    static constexpr int CTA = cta_threads(TT);
-    static constexpr int G = CTA / TT;
-    static constexpr size_t PT = ((NB * sizeof(double) + 15) / 16) * 16;
-    static constexpr size_t SMEM = PT + (size_t)G * TL::ELEMS * sizeof(cx<T>);
-    // CTAs per SM that shared memory allows (1 KB reserved each); registers are capped to match
-    static constexpr int FIT = (int)((size_t)227 * 1024 / (SMEM + 1024));
-    static constexpr int MINB = FIT < 1 ? 1 : (FIT > LGF_ZT_MAXB ? LGF_ZT_MAXB : FIT);
-};
-
-template <typename T, int NA, int NB, int C>
-__global__ void __launch_bounds__((ZTCfg<T, NA, NB, C>::CTA), (ZTCfg<T, NA, NB, C>::MINB))
-k_fft_zt(cx<T> *__restrict__ w, Geom geo, const double *__restrict__ ptab, double pmax2_over_V, int64_t ntiles, const Ctrl *ctrl)
-{
-    if (*(volatile const int *)&ctrl->done) return;
-    typedef ZTCfg<T, NA, NB, C> CF;
-    typedef typename CF::TL TL;
-    typedef Line<T, NA, TL::SA> LA;
-    typedef Line<T, NB, TL::SB> LB;
-    constexpr int TT = CF::TT, G = CF::G;
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    double *pt = (double *)smem_raw;                                  // 4 sin^2(pi kt/Nt), NB entries
-    cx<T> *sm0 = (cx<T> *)(smem_raw + CF::PT);
-    const int grp = threadIdx.x / TT, t = threadIdx.x % TT;
-    cx<T> *sm = sm0 + (size_t)grp * TL::ELEMS;
-    const int64_t tile = (int64_t)blockIdx.x * G + grp;
-    const bool ok = tile < ntiles && grp < G;
-    const int Nx = geo.N[0], Ny = geo.N[1];
-    const int xchunks = Nx / C;
-    // tile -> (field, y, xchunk)
-    const int xc = (int)(tile % xchunks);
-    const int y = (int)((tile / xchunks) % Ny);
-    const int64_t fld = tile / ((int64_t)xchunks * Ny);
-    const int x0 = xc * C;
-    cx<T> *f = w + fld * geo.V + x0 + (int64_t)Nx * y;
-    const int64_t sz = geo.st[2], st = geo.st[3];
-    for (int i = threadIdx.x; i < NB; i += CF::CTA) pt[i] = ptab[Nx + Ny + NA + i];
-    int la, ha, lb, hb;                                                // z-line (c, t) / t-line (c, kz) of this thread
-    line_of_thread<TL::SA>(t, la, ha);
-    line_of_thread<TL::SB>(t, lb, hb);
-    const int ca = la % C, ta = la / C, cb = lb % C, zb = lb / C;
-    const bool on_z = ok && ta < NB && t < TL::SA * C * NB, on_t = ok && zb < NA && t < TL::SB * C * NA;
-    const unsigned mz = __ballot_sync(0xffffffffu, on_z), mt = __ballot_sync(0xffffffffu, on_t);
-
-    if (on_z) {                                                        // z-line at (c, t) = (ca, ta)
-        cx<T> v[LA::NL];
-        const cx<T> *g = f + ca + st * ta;
-#pragma unroll
-        for (int i = 0; i < LA::NL; i++) v[i] = g[sz * LA::nat(i, ha)];
-        LA::template dif<-1>(v, ha, mz);
-#pragma unroll
-        for (int q = 0; q < LA::NL; q++) sm[ta * TL::RS + LA::slot(q, ha) * C + ca] = v[q];
-    }
-    __syncthreads();
-    if (on_t) {                                                        // t-line at (c, kz) = (cb, zb)
-        cx<T> v[LB::NL];
-#pragma unroll
-        for (int i = 0; i < LB::NL; i++) v[i] = sm[LB::nat(i, hb) * TL::RS + zb * C + cb];
-        LB::template dif<-1>(v, hb, mt);
-        const double pxyz = ptab[x0 + cb] + ptab[Nx + y] + ptab[Nx + Ny + zb];
-#pragma unroll
-        for (int q = 0; q < LB::NL; q++) {
-            const double p2 = pxyz + pt[LB::slot(q, hb)];
-            const T fac = (p2 > 0.0) ? (T)(pmax2_over_V / p2) : (T)0;  // zero mode -> 0 (reading R7)
-            v[q] = cscale(v[q], fac);
-        }
-        LB::template dit<+1>(v, hb, mt);
-#pragma unroll
-        for (int i = 0; i < LB::NL; i++) sm[LB::nat(i, hb) * TL::RS + zb * C + cb] = v[i];
-    }
-    __syncthreads();
-    if (on_z) {
-        cx<T> v[LA::NL];
-#pragma unroll
-        for (int i = 0; i < LA::NL; i++) v[i] = sm[ta * TL::RS + LA::nat(i, ha) * C + ca];
-        LA::template dif<+1>(v, ha, mz);
-        cx<T> *g = f + ca + st * ta;
-#pragma unroll
-        for (int q = 0; q < LA::NL; q++) g[sz * LA::slot(q, ha)] = v[q];
-    }
-}
-
 // ---------------------------------------------------------------- dispatch
-// x-columns per (z,t) tile: 64-byte runs in global memory (FP64), unless the tile would not fit
-#ifndef LGF_ZT_BYTES
-#define LGF_ZT_BYTES 64
-#endif
-template <typename T, int NA, int NB> struct ZTC {
-    static constexpr int WANT = LGF_ZT_BYTES / (int)sizeof(cx<T>);
-    static constexpr size_t tile_bytes(int c) { return (size_t)(NA * c + c) * NB * sizeof(cx<T>); }
-    static constexpr int C = tile_bytes(WANT) <= 200 * 1024 && NA % WANT == 0 ? WANT : (tile_bytes(WANT / 2) <= 200 * 1024 && NA % (WANT / 2) == 0 ? WANT / 2 : WANT / 4);
-};
-
 template <typename T, int N> static int setup_xy_n()
 {
     cudaError_t e;
@@ -674,24 +360,6 @@ template <typename T, int N> static int setup_xy_n()
         e = cudaFuncSetAttribute(k_fft_xy_inv_g2<T, N, N, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)XYG2Cfg<T, N, N>::SMEM);
         if (e != cudaSuccess) return 1;
     }
-    return 0;
-}
-
-template <typename T, int NA, int NB> static int setup_zt_n()
-{
-    constexpr int C = ZTC<T, NA, NB>::C;
-    typedef ZTCfg<T, NA, NB, C> Z;
-    cudaError_t e = cudaFuncSetAttribute(k_fft_zt<T, NA, NB, C>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Z::SMEM);
-    return e == cudaSuccess ? 0 : 1;
-}
-
-template <typename T, int NA, int NB> static int launch_zt_n(const FftArgs &a, cudaStream_t st)
-{
-    constexpr int C = ZTC<T, NA, NB>::C;
-    typedef ZTCfg<T, NA, NB, C> Z;
-    const int64_t ntiles = (int64_t)a.nfields * a.geo.N[1] * (a.geo.N[0] / C);
-    const unsigned grid = (unsigned)((ntiles + Z::G - 1) / Z::G);
-    k_fft_zt<T, NA, NB, C><<<grid, Z::CTA, Z::SMEM, st>>>((cx<T> *)a.w, a.geo, a.ptab, a.pmax2 / (double)a.geo.V, ntiles, a.ctrl);
     return 0;
 }
 
@@ -723,21 +391,42 @@ template <typename T, int N> static int launch_inv_g_n(const FftArgs &a, void *g
 
 template <typename T, int N> static int gbuf_fits_n() { return (XYGCfg<T, N, N>::FITS || XYG2Cfg<T, N, N>::FITS) ? 1 : 0; }
 
-// Lattices with Nx = Ny in {8, 12, 16, 24, 32, 48, 64} and (Nz, Nt) either equal and in the same
-// set or (32, n), n in {8, 16, 48, 64} (the paper's 32^3 x n lattices): the (x,y)
-// passes are instantiated per Nx and the (z,t) pass per (Nz, Nt).  The x-columns of a (z,t) tile
-// must divide Nx (2 or 4).  Everything else takes the generic path.
-static bool tiled_extent(int n) { return n == 8 || n == 16 || n == 32 || n == 64 || n == 12 || n == 24 || n == 48; }
-static bool tiled_zt(int nz, int nt)
+// Lattices with Nx = Ny and every extent in {8, 12, 16, 24, 32, 48, 64}: the (x,y) passes are instantiated
+// per Nx (= Ny) and the (z,t) pass per (Nz, Nt) pair (fft_zt_inst.cu, one translation unit per Nz), which
+// covers the cubic lattices, the N_s^3 x N_t shapes (16^3 x 32, 24^3 x 48, the paper's 32^3 x n)
+// and (x,y) != (z,t) shapes alike.  The x-columns of a (z,t) tile (2, 4 or 8, chosen per (precision, Nz,
+// Nt)) must divide Nx; the one family that fails this, FP32 with Nx = 12 and Nz != 12, takes the generic path
+// like every other extent.
+#define LGF_ZT_DECL(N)                                            \
+    int zt_columns_na##N(int nt, int prec);                       \
+    int zt_setup_na##N(int nt, int prec);                         \
+    int zt_launch_na##N(const FftArgs &a, cudaStream_t st);
+LGF_ZT_DECL(8) LGF_ZT_DECL(12) LGF_ZT_DECL(16) LGF_ZT_DECL(24) LGF_ZT_DECL(32) LGF_ZT_DECL(48) LGF_ZT_DECL(64)
+#undef LGF_ZT_DECL
+#define LGF_NZ_SWITCH(FN, ...)                \
+    switch (nz) {                             \
+    case 8: return FN##8(__VA_ARGS__);        \
+    case 12: return FN##12(__VA_ARGS__);      \
+    case 16: return FN##16(__VA_ARGS__);      \
+    case 24: return FN##24(__VA_ARGS__);      \
+    case 32: return FN##32(__VA_ARGS__);      \
+    case 48: return FN##48(__VA_ARGS__);      \
+    case 64: return FN##64(__VA_ARGS__);      \
+    default: break;                           \
+    }
+static int zt_columns(int nz, int nt, int prec)
 {
-    if (nz == nt) return tiled_extent(nz);
-    return nz == 32 && (nt == 8 || nt == 16 || nt == 48 || nt == 64);
+    LGF_NZ_SWITCH(zt_columns_na, nt, prec)
+    return 0;
 }
+static bool tiled_extent(int n) { return n == 8 || n == 16 || n == 32 || n == 64 || n == 12 || n == 24 || n == 48; }
 bool fft_tiled_supported(const int N[4], int prec)
 {
-    (void)prec;
-    return N[0] == N[1] && tiled_extent(N[0]) && tiled_zt(N[2], N[3]);
+    if (!(N[0] == N[1] && tiled_extent(N[0]) && tiled_extent(N[2]) && tiled_extent(N[3]))) return false;
+    const int c = zt_columns(N[2], N[3], prec);
+    return c > 0 && N[0] % c == 0;
 }
+int fft_tiled_zt_columns(const int N[4], int prec) { return fft_tiled_supported(N, prec) ? zt_columns(N[2], N[3], prec) : 0; }
 
 #define LGF_FFT_SWITCH(FN, ...)                                         \
     switch (n) {                                                        \
@@ -756,18 +445,9 @@ static int setup_xy(int n, int prec)
     LGF_FFT_SWITCH(setup_xy_n)
     return 1;
 }
-// (z,t) pass: FN<T, Nz, Nt> for the supported pairs
-#define LGF_ZT_CASE(FN, A, B, ...) \
-    if (nz == A && nt == B) return prec == 0 ? FN<double, A, B>(__VA_ARGS__) : FN<float, A, B>(__VA_ARGS__);
-#define LGF_ZT_SWITCH(FN, ...)                                                                              \
-    LGF_ZT_CASE(FN, 8, 8, __VA_ARGS__) LGF_ZT_CASE(FN, 12, 12, __VA_ARGS__) LGF_ZT_CASE(FN, 16, 16, __VA_ARGS__) \
-    LGF_ZT_CASE(FN, 24, 24, __VA_ARGS__) LGF_ZT_CASE(FN, 32, 32, __VA_ARGS__) LGF_ZT_CASE(FN, 48, 48, __VA_ARGS__) \
-    LGF_ZT_CASE(FN, 64, 64, __VA_ARGS__) LGF_ZT_CASE(FN, 32, 8, __VA_ARGS__) LGF_ZT_CASE(FN, 32, 16, __VA_ARGS__) \
-    LGF_ZT_CASE(FN, 32, 48, __VA_ARGS__) LGF_ZT_CASE(FN, 32, 64, __VA_ARGS__)
-
 static int setup_zt(int nz, int nt, int prec)
 {
-    LGF_ZT_SWITCH(setup_zt_n)
+    LGF_NZ_SWITCH(zt_setup_na, nt, prec)
     return 1;
 }
 int fft_tiled_setup(const int N[4], int prec) { return setup_xy(N[0], prec) | setup_zt(N[2], N[3], prec); }
@@ -789,8 +469,8 @@ static int run_xy(const FftArgs &a, int which, cudaStream_t st)
 }
 static int run_zt(const FftArgs &a, cudaStream_t st)
 {
-    const int nz = a.geo.N[2], nt = a.geo.N[3], prec = a.prec;
-    LGF_ZT_SWITCH(launch_zt_n, a, st)
+    const int nz = a.geo.N[2];
+    LGF_NZ_SWITCH(zt_launch_na, a, st)
     return 1;
 }
 void launch_fft_tiled(const FftArgs &a, int which, cudaStream_t st)

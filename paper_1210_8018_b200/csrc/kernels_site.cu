@@ -25,11 +25,11 @@ k_measure(const cx<T> *__restrict__ links, cx<T> *__restrict__ w, Geom geo, Ctrl
 {
     if (*(volatile int *)&ctrl->done) return;
     const int64_t V = geo.V;
-    const int64_t s = (int64_t)blockIdx.x * SITE_THREADS + threadIdx.x;
+    const int64_t rr = (int64_t)blockIdx.x * SITE_THREADS + threadIdx.x;
     double trF = 0, th = 0;
-    if (s < V) {
+    if (rr < V) {
         int c[4];
-        site_coords(geo, s, c);
+        const int64_t s = walk_site(geo, rr, c);
         cx<T> A[9];
 #pragma unroll
         for (int k = 0; k < 9; k++) A[k] = mk<T>(0, 0);
@@ -89,10 +89,10 @@ k_update(cx<T> *__restrict__ links, const cx<T> *__restrict__ w, Geom geo, T a, 
 {
     if (*(volatile const int *)&ctrl->done) return;
     const int64_t V = geo.V;
-    const int64_t s = (int64_t)blockIdx.x * SITE_THREADS + threadIdx.x;
-    if (s >= V) return;
+    const int64_t rr = (int64_t)blockIdx.x * SITE_THREADS + threadIdx.x;
+    if (rr >= V) return;
     int c[4];
-    site_coords(geo, s, c);
+    const int64_t s = walk_site(geo, rr, c);
     cx<T> g0[9];
     build_g<T, PACK>(w, V, s, a, gexp, g0);
     constexpr int R = (NE == 6) ? 2 : 3;
@@ -120,10 +120,10 @@ __global__ void __launch_bounds__(SITE_THREADS)
 k_apply_g(cx<T> *__restrict__ links, const cx<T> *__restrict__ gacc, Geom geo)
 {
     const int64_t V = geo.V;
-    const int64_t s = (int64_t)blockIdx.x * SITE_THREADS + threadIdx.x;
-    if (s >= V) return;
+    const int64_t rr = (int64_t)blockIdx.x * SITE_THREADS + threadIdx.x;
+    if (rr >= V) return;
     int c[4];
-    site_coords(geo, s, c);
+    const int64_t s = walk_site(geo, rr, c);
     cx<T> g0[9];
     load_g01<T, 4, true>(gacc, V, s, (T)0, 0, g0);
     su3_row2(g0);

@@ -54,11 +54,13 @@ struct FftArgs {
     double pmax2;       // max_k p^2(k)
     const void *tw;     // device: cx<T> forward twiddles exp(-2 pi i k/N_mu), four tables back to back
     const Ctrl *ctrl;
+    int zt_pipe;        // LGF_OPT_ZT_PIPE: (z,t) pass as the persistent kernel with cp.async prefetch
 };
 // generic per-axis transform: any extent, O(N^2) per line.  Returns launches issued.
 int launch_fft_generic(const FftArgs &a, cudaStream_t st);
 // tiled register FFT: three passes.  which = 0 (x,y) forward, 1 (z,t) forward*mask*inverse, 2 (x,y) inverse
 bool fft_tiled_supported(const int N[4], int prec);
+int fft_tiled_zt_columns(const int N[4], int prec);      // x-columns per (z,t) tile, 0 if the lattice is not tiled
 bool fft_tiled_gbuf_supported(const int N[4], int prec); // pass 2 with the g build fits in shared memory
 void launch_fft_tiled(const FftArgs &a, int which, cudaStream_t st);
 // pass 2 of all 4 packed fields with g(x) = reunit(1 + (alpha/2) w(x)) as its epilogue: rows 0, 1 of g -> gbuf

@@ -15,6 +15,8 @@
 
 using namespace lgf;
 
+static_assert(LGF_HIST_CAP == LGF_HISTORY_CAP, "history capacity: common.cuh and lgf.h must agree");
+
 namespace {
 
 const double kTwoPi = 6.283185307179586476925286766559;
@@ -37,6 +39,8 @@ struct lgf_ctx {
     int prec;
     int recon = 18, pack = 4, check_interval = 8, fft_path = 0, profile = 0, fusion = 1, l2_persist = 0, gmap = 0, accum = 0;
     int graph = 1;           // LGF_OPT_GRAPH: replay captured iterations as a CUDA graph
+    int zblock = 0;          // LGF_OPT_ZBLOCK: 0 = auto (resolved by lgf_bind into sa.geo.zb)
+    int zt_pipe = 0;         // LGF_OPT_ZT_PIPE
     cudaGraphExec_t gexec = nullptr;
     struct { double alpha, eps; int cur, wcur, gmap, unit; } gkey{};
     int64_t g_launches = 0, g_kcount[LGF_KERNEL_KINDS] = {0};
@@ -361,6 +365,31 @@ void l2_window_clear(lgf_ctx *c)
     c->l2_window = false;
 }
 
+// LGF_OPT_ZBLOCK = 0: the largest divisor of Nz such that one z-block of (x,y) planes, with everything the
+// link kernel streams per site (links in and out, g, Delta), takes at most LGF_ZBLOCK_L2_FRACTION of L2.
+// The reuse distance of a -t / +t neighbour is one z-block of planes, so it has to stay well inside L2
+// together with the write-back lines of the new links.  Falls back to Nz (storage order) when the L2 size
+// cannot be read.
+#ifndef LGF_ZBLOCK_L2_FRACTION
+#define LGF_ZBLOCK_L2_FRACTION 0.38
+#endif
+int auto_zblock(const lgf_ctx *c)
+{
+    int dev = 0, l2 = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&l2, cudaDevAttrL2CacheSize, dev) != cudaSuccess || l2 <= 0) {
+        cudaGetLastError();
+        return c->N[2];
+    }
+    const size_t e = elem_bytes(c);
+    const int ne = c->recon == 12 ? 6 : 9;
+    const size_t per_site = (size_t)(2 * 4 * ne + 6 + c->pack) * e;
+    const double plane = (double)c->N[0] * c->N[1] * (double)per_site;
+    int best = 1;
+    for (int zb = 1; zb <= c->N[2]; zb++)
+        if (c->N[2] % zb == 0 && zb * plane <= LGF_ZBLOCK_L2_FRACTION * (double)l2) best = zb;
+    return best;
+}
+
 int need_loaded(lgf_ctx *ctx)
 {
     if (!ctx) return LGF_ERR_INVALID_ARG;
@@ -409,7 +438,7 @@ int lgf_set_option(lgf_ctx *ctx, int key, int64_t value)
 {
     if (!ctx) return LGF_ERR_INVALID_ARG;
     const bool layout_key = (key == LGF_OPT_RECON || key == LGF_OPT_FFT_BATCH || key == LGF_OPT_FFT_PATH || key == LGF_OPT_FUSION ||
-                             key == LGF_OPT_L2_PERSIST || key == LGF_OPT_ACCUM_G);
+                             key == LGF_OPT_L2_PERSIST || key == LGF_OPT_ACCUM_G || key == LGF_OPT_ZBLOCK);
     if (layout_key && ctx->bound) return fail(ctx, LGF_ERR_INVALID_ARG, "this option must be set before lgf_bind");
     switch (key) {
     case LGF_OPT_RECON:
@@ -442,6 +471,12 @@ int lgf_set_option(lgf_ctx *ctx, int key, int64_t value)
     case LGF_OPT_GRAPH:
         if (value != 0 && value != 1) return fail(ctx, LGF_ERR_INVALID_ARG, "GRAPH must be 0 or 1");
         ctx->graph = (int)value; break;
+    case LGF_OPT_ZBLOCK:
+        if (value < 0 || (value > 0 && ctx->N[2] % value != 0)) return fail(ctx, LGF_ERR_INVALID_ARG, "ZBLOCK must be 0 (auto) or a divisor of Nz");
+        ctx->zblock = (int)value; break;
+    case LGF_OPT_ZT_PIPE:
+        if (value != 0 && value != 1) return fail(ctx, LGF_ERR_INVALID_ARG, "ZT_PIPE must be 0 or 1");
+        ctx->zt_pipe = (int)value; ctx->fa.zt_pipe = ctx->zt_pipe; graph_drop(ctx); break;
     case LGF_OPT_PROFILE:
         if (ctx->bound) flush_events(ctx);
         ctx->profile = value ? 1 : 0; break;
@@ -473,6 +508,7 @@ int lgf_bind(lgf_ctx *ctx, void *dev_workspace, size_t bytes, void *cuda_stream)
     for (int d = 0; d < 4; d++) g.N[d] = ctx->N[d];
     g.V = ctx->V;
     g.st[0] = 1; g.st[1] = g.N[0]; g.st[2] = (int64_t)g.N[0] * g.N[1]; g.st[3] = (int64_t)g.N[0] * g.N[1] * g.N[2];
+    g.zb = ctx->zblock > 0 ? ctx->zblock : auto_zblock(ctx);
     SiteArgs &s = ctx->sa;
     s.geo = g;
     for (int i = 0; i < 2; i++) { ctx->links_buf[i] = ctx->base + L.links[i]; ctx->w_buf[i] = ctx->base + L.w[i]; }
@@ -483,7 +519,7 @@ int lgf_bind(lgf_ctx *ctx, void *dev_workspace, size_t bytes, void *cuda_stream)
     s.hist = (double2 *)(ctx->base + L.hist);
     s.prec = ctx->prec; s.recon = ctx->recon; s.pack = ctx->pack; s.gexp = ctx->gmap;
     FftArgs &f = ctx->fa;
-    f.geo = g; f.nfields = ctx->pack; f.prec = ctx->prec;
+    f.geo = g; f.nfields = ctx->pack; f.prec = ctx->prec; f.zt_pipe = ctx->zt_pipe;
     sync_ptrs(ctx);
     f.ptab = (const double *)(ctx->base + L.ptab);
     f.pmax2 = ctx->pmax2;
@@ -760,6 +796,7 @@ int lgf_reset_counters(lgf_ctx *ctx)
 
 int lgf_uses_tiled_fft(const lgf_ctx *ctx) { return ctx && ctx->tiled ? 1 : 0; }
 int lgf_uses_gbuf(const lgf_ctx *ctx) { return ctx && ctx->bound && ctx->use_gbuf ? 1 : 0; }
+int lgf_zblock(const lgf_ctx *ctx) { return ctx && ctx->bound ? ctx->sa.geo.zb : 0; }
 
 int lgf_sync_links(lgf_ctx *ctx)
 {

@@ -11,7 +11,8 @@ import os
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_HERE, "liblgf.so")
+# LGF_LIB_PATH: another build of the same library (same-run A/B of tuning macros); default: the in-tree build
+LIB_PATH = os.environ.get("LGF_LIB_PATH") or os.path.join(_HERE, "liblgf.so")
 
 OK = 0
 ERR_INVALID_ARG, ERR_UNSUPPORTED_SIZE, ERR_NOT_BOUND, ERR_NOT_LOADED = -1, -2, -3, -4
@@ -19,7 +20,7 @@ ERR_WORKSPACE_TOO_SMALL, ERR_CUDA, ERR_NOT_CONVERGED, ERR_NUMERIC = -5, -6, -7, 
 PREC_FP64, PREC_FP32 = 0, 1
 LAYOUT_AOS, LAYOUT_AOS12 = 0, 1
 OPT_RECON, OPT_FFT_BATCH, OPT_MAX_ITER, OPT_CHECK_INTERVAL, OPT_FFT_PATH, OPT_PROFILE, OPT_FUSION, OPT_L2_PERSIST = 1, 2, 3, 4, 5, 6, 7, 8
-OPT_GMAP, OPT_ACCUM_G, OPT_GRAPH = 9, 10, 11
+OPT_GMAP, OPT_ACCUM_G, OPT_GRAPH, OPT_ZBLOCK, OPT_ZT_PIPE = 9, 10, 11, 12, 13
 GMAP_FIRST_ORDER, GMAP_EXP = 0, 1
 FIELD_DELTA, FIELD_W, FIELD_G = 0, 1, 2
 STAGE_MEASURE, STAGE_FOURIER, STAGE_UPDATE = 0, 1, 2
@@ -30,8 +31,8 @@ KERNEL_NAMES = ["measure", "fft_xy_fwd", "fft_zt", "fft_xy_inv", "update", "fft_
 SYMBOLS = [
     "lgf_create", "lgf_set_option", "lgf_workspace_bytes", "lgf_bind", "lgf_load_links", "lgf_get_links",
     "lgf_measure", "lgf_iterate", "lgf_fix", "lgf_stage", "lgf_get_field", "lgf_set_field", "lgf_history",
-    "lgf_kernel_time", "lgf_launch_count", "lgf_reset_counters", "lgf_uses_tiled_fft", "lgf_uses_gbuf", "lgf_sync_links", "lgf_last_error",
-    "lgf_destroy",
+    "lgf_kernel_time", "lgf_launch_count", "lgf_reset_counters", "lgf_uses_tiled_fft", "lgf_uses_gbuf", "lgf_zblock", "lgf_sync_links", "lgf_last_error",
+    "lgf_destroy", "lgf_debug_dfma_rate",
 ]
 
 
@@ -81,12 +82,23 @@ def lib():
     L.lgf_reset_counters.argtypes = [vp]
     L.lgf_uses_tiled_fft.argtypes = [vp]
     L.lgf_uses_gbuf.argtypes = [vp]
+    L.lgf_zblock.argtypes = [vp]
     L.lgf_sync_links.argtypes = [vp]
     L.lgf_last_error.argtypes = [vp]
     L.lgf_last_error.restype = ctypes.c_char_p
     L.lgf_destroy.argtypes = [vp]
+    L.lgf_debug_dfma_rate.argtypes = [vp, dp]
     _lib = L
     return L
+
+
+def debug_dfma_rate(stream=None):
+    """Measured FP64 FMA rate of the current device in DFMA/s (lgf_debug_dfma_rate)."""
+    out = ctypes.c_double()
+    rc = lib().lgf_debug_dfma_rate(stream, ctypes.byref(out))
+    if rc:
+        raise LgfError(rc, "lgf_debug_dfma_rate failed")
+    return out.value
 
 
 def _dims(N):
@@ -103,7 +115,7 @@ class GaugeFixer:
 
     def __init__(self, N, precision="fp64", recon=18, fft_batch=4, fft_path=0, device="cuda:0",
                  stream=None, max_iter=None, check_interval=None, profile=False, fusion=None, l2_persist=None, gmap=None,
-                 accum_g=None, graph=None):
+                 accum_g=None, graph=None, zblock=None, zt_pipe=None):
         import torch
 
         self.torch = torch
@@ -130,6 +142,10 @@ class GaugeFixer:
             self.set_option(OPT_ACCUM_G, accum_g)
         if graph is not None:
             self.set_option(OPT_GRAPH, graph)
+        if zblock is not None:
+            self.set_option(OPT_ZBLOCK, zblock)
+        if zt_pipe is not None:
+            self.set_option(OPT_ZT_PIPE, zt_pipe)
         if max_iter is not None:
             self.set_option(OPT_MAX_ITER, max_iter)
         if check_interval is not None:
@@ -265,6 +281,9 @@ class GaugeFixer:
 
     def uses_gbuf(self):
         return bool(self.L.lgf_uses_gbuf(self.ctx))
+
+    def zblock(self):
+        return int(self.L.lgf_zblock(self.ctx))
 
     def sync_links(self):
         self._ck(self.L.lgf_sync_links(self.ctx))

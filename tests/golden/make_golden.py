@@ -1,10 +1,13 @@
 """Writes the stored expected values under tests/golden/ by calling ONLY gen/ and oracle/.
 
-    python tests/golden/make_golden.py [8 16 32]
+    python tests/golden/make_golden.py [8 16 32 48 64]
 
 For each listed N^4 BASELINE.json config (and the two extra seeds +1000, +2000 at 8^4 and
 16^4) it runs the oracle's Algorithm 1 (orc_fix, alpha = 0.08, eps = 1e-15) and writes
 fix_<N>_<seed>.txt: iteration count, final F and theta, and the (F, theta) history.
+48^4 (about 15 s per oracle iteration) and 64^4 (about 50 s per iteration, 25 GB) are run on request only;
+the FP32 configuration (BASELINE config 4, eps = 1e-12) reads its iteration count off the same FP64
+trajectory: the first row with theta <= 1e-12.
 These are ORACLE values (the paper prints none): "parity unpinned" as values,
 pinned through tests/test_oracle_pins.py.  The CUDA path is never called here.
 """
@@ -18,7 +21,7 @@ import gen  # noqa: E402
 import oracle  # noqa: E402
 
 HERE = os.path.dirname(os.path.abspath(__file__))
-SIGMA = {8: 0.3, 16: 0.5, 32: 0.5}
+SIGMA = {8: 0.3, 16: 0.5, 32: 0.5, 48: 0.5, 64: 0.6}
 
 
 def run(n, seed):

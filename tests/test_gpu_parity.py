@@ -235,11 +235,18 @@ def test_fp32_variant(lgf, lat, var):
 
 def test_tiled_fft_is_taken_where_expected(lgf):
     for n, want in [(8, True), (12, True), (16, True), (24, True), (32, True), (48, True), (64, True), ((16, 16, 8, 8), True), ((32, 32, 32, 16), True), ((8, 8, 32, 64), True),
-                    ((8, 8, 16, 32), False),
-                    ((8, 8, 8, 16), False), ((8, 16, 8, 8), False), (4, False), (36, False)]:
+                    # N_s^3 x N_t and every other (Nz, Nt) pair of tiled extents
+                    ((8, 8, 16, 32), True), ((8, 8, 8, 16), True), ((16, 16, 16, 32), True), ((24, 24, 24, 48), True),
+                    ((32, 32, 32, 12), True), ((32, 32, 32, 24), True), ((12, 12, 32, 32), True), ((12, 12, 64, 8), True),
+                    ((8, 16, 8, 8), False), (4, False), (36, False), ((8, 8, 8, 6), False), ((8, 8, 36, 8), False)]:
         gf = fixer(lgf, n)
         assert gf.uses_tiled_fft() == want, n
     assert not fixer(lgf, 16, fft_path=1).uses_tiled_fft()
+    # FP32 tiles are 8 x-columns wide unless Nz = 12 (then 4): Nx = 12 with another Nz does not divide into
+    # them and must take the generic transform instead of silently skipping x = 8..11
+    for n, want in [(12, True), ((12, 12, 32, 32), False), ((12, 12, 16, 16), False), ((12, 12, 12, 48), True),
+                    ((24, 24, 32, 32), True), ((8, 8, 12, 12), True)]:
+        assert fixer(lgf, n, precision="fp32").uses_tiled_fft() == want, n
 
 
 # Lines of 48 and 64 are shared by two threads (fft_tiled.cu, Line<T, N, 2>); lattices with
@@ -247,7 +254,15 @@ def test_tiled_fft_is_taken_where_expected(lgf):
 # finishes in about a second.
 SPLIT_LATTICES = [((64, 64, 8, 8), 81), ((8, 8, 64, 64), 82), ((48, 48, 12, 12), 83), ((16, 16, 48, 48), 84),
                   # (z,t) tiles with Nz = 32 != Nt: the paper's 32^3 x n lattices
-                  ((32, 32, 32, 8), 85), ((8, 8, 32, 16), 86), ((8, 8, 32, 48), 87), ((8, 8, 32, 64), 88)]
+                  ((32, 32, 32, 8), 85), ((8, 8, 32, 16), 86), ((8, 8, 32, 48), 87), ((8, 8, 32, 64), 88),
+                  # every other (Nz, Nt) pair of tiled extents: N_s^3 x N_t shapes (T = 2L), mixed radix-3 / split
+                  # lines on either axis, tiles that run one CTA per SM
+                  ((16, 16, 16, 32), 89), ((8, 8, 24, 48), 90), ((8, 8, 32, 12), 91), ((8, 8, 32, 24), 92),
+                  ((8, 8, 16, 64), 93), ((8, 8, 64, 16), 94), ((8, 8, 48, 64), 95), ((8, 8, 64, 48), 96),
+                  ((16, 16, 8, 12), 97), ((8, 8, 12, 24), 98), ((8, 8, 48, 32), 99),
+                  # Nx = 12: FP64 tiles (4 columns) divide it, FP32 tiles (8 columns) do not -> generic path in FP32
+                  ((12, 12, 32, 32), 100), ((12, 12, 16, 16), 101)]
+FP32_GENERIC = {(12, 12, 32, 32), (12, 12, 16, 16)}
 
 
 @pytest.mark.parametrize("lat", SPLIT_LATTICES, ids=lambda v: "x".join(map(str, v[0])))
@@ -259,7 +274,7 @@ def test_split_line_fourier_matches_oracle(lgf, lat, fft_batch):
     w = oracle.fourier_accelerate(N, D)
     for prec, tol in (("fp64", 2e-13), ("fp32", 2e-5)):
         gf = fixer(lgf, N, precision=prec, fft_batch=fft_batch)
-        assert gf.uses_tiled_fft()
+        assert gf.uses_tiled_fft() == (not (prec == "fp32" and tuple(N) in FP32_GENERIC))
         gf.load_links(U if prec == "fp64" else U.astype(np.complex64))
         gf.set_field(lgf.FIELD_DELTA, D if prec == "fp64" else D.astype(np.complex64))
         gf.stage(lgf.STAGE_FOURIER)

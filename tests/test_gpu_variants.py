@@ -330,3 +330,90 @@ def test_graph_falls_back_on_the_legacy_default_stream(lgf):
     assert np.array_equal(a.get_links(), b.get_links())
     a.close()
     b.close()
+
+
+# ------------------------------------------------------------------ LGF_OPT_ZBLOCK: (z,t)-blocked site walk
+@pytest.mark.parametrize("var", [dict(recon=12), dict(recon=18, fusion=0), dict(recon=18, fft_batch=9, fft_path=1),
+                                 dict(recon=12, accum_g=1)], ids=vid)
+@pytest.mark.parametrize("N", [(8, 8, 8, 8), (12, 12, 12, 6), (4, 6, 8, 12)], ids=lambda n: "x".join(map(str, n)))
+def test_site_walk_order_changes_nothing_but_the_sum_order(lgf, var, N):
+    """Every z-block that divides Nz visits every site exactly once: the links after 3 iterations are
+    bitwise those of the storage-order walk (same arithmetic per site), F and theta agree to rounding
+    of the FP64 partial sums, and the first iteration matches the oracle."""
+    if var.get("accum_g") and N != (8, 8, 8, 8):
+        pytest.skip("ACCUM_G needs a lattice the tiled FFT covers")
+    U = gen.gen_links(N, 0.5, 4242)
+    Uo = U.copy()
+    hist = oracle.iterate(N, Uo, ALPHA, 1)
+    ref = None
+    for zb in [N[2]] + [d for d in (1, 2, 3, 4, 6) if N[2] % d == 0 and d < N[2]]:
+        gf = lgf.GaugeFixer(N, zblock=zb, **var)
+        assert gf.zblock() == zb
+        gf.load_links(U)
+        r1 = gf.iterate(ALPHA, 1)
+        assert np.abs(gf.get_links() - Uo).max() < 1e-12
+        assert abs(r1.F - hist[1, 0]) <= 1e-10 * abs(hist[1, 0]) and abs(r1.theta - hist[1, 1]) <= 1e-10 * hist[1, 1]
+        r3 = gf.iterate(ALPHA, 2)
+        U3 = gf.get_links()
+        if ref is None:
+            ref = (U3, r3)
+        else:
+            assert np.array_equal(U3, ref[0]), zb
+            assert abs(r3.F - ref[1].F) <= 1e-14 and abs(r3.theta - ref[1].theta) <= 1e-13 * ref[1].theta
+        gf.close()
+
+
+def test_zblock_option_validation_and_auto(lgf):
+    gf = lgf.GaugeFixer((8, 8, 12, 8))
+    assert gf.zblock() == 12                         # whole lattice far below the L2 budget: storage order
+    gf.close()
+    with pytest.raises(lgf.LgfError):
+        lgf.GaugeFixer((8, 8, 12, 8), zblock=5)     # must divide Nz
+    with pytest.raises(lgf.LgfError):
+        lgf.GaugeFixer((8, 8, 12, 8), zblock=-1)
+    big = lgf.GaugeFixer(64)                          # 64^4 FP64, 18-real: one time slice of links exceeds L2
+    zb = big.zblock()
+    big.close()
+    assert 1 <= zb < 64 and 64 % zb == 0
+
+
+# ------------------------------------------------------------------ LGF_OPT_ZT_PIPE: persistent (z,t) pass
+@pytest.mark.parametrize("N", [(16, 16, 16, 16), (12, 12, 12, 12), (8, 8, 32, 16), (8, 8, 64, 64), (24, 24, 24, 24),
+                               (8, 8, 16, 32)], ids=lambda n: "x".join(map(str, n)))
+@pytest.mark.parametrize("prec", ["fp64", "fp32"])
+def test_zt_pipe_is_bitwise_the_plain_pass(lgf, N, prec):
+    """The persistent (z,t) pass with cp.async prefetch does the same arithmetic in the same order: w is
+    bitwise that of the plain kernel (and within the usual tolerance of the oracle); a pair without a
+    persistent instantiation ((16, 32)) runs the plain kernel whatever the option says."""
+    U = gen.gen_links(N, 0.5, 777)
+    D, _, _ = oracle.measure(N, U)
+    w = oracle.fourier_accelerate(N, D)
+    cdt = np.complex128 if prec == "fp64" else np.complex64
+    out = []
+    for pipe in (0, 1):
+        gf = lgf.GaugeFixer(N, precision=prec, zt_pipe=pipe)
+        assert gf.uses_tiled_fft()
+        gf.load_links(U.astype(cdt))
+        gf.set_field(lgf.FIELD_DELTA, D.astype(cdt))
+        gf.stage(lgf.STAGE_FOURIER)
+        out.append(gf.get_field(lgf.FIELD_W))
+        gf.load_links(U.astype(cdt))
+        r = gf.iterate(ALPHA, 5)                   # several tiles per persistent CTA, graph replay on top
+        out.append((r.F, r.theta))
+        gf.close()
+    assert np.array_equal(out[0], out[2]) and out[1] == out[3]
+    assert np.abs(out[2].astype(np.complex128) - w).max() < (2e-13 if prec == "fp64" else 2e-5) * np.abs(w).max()
+
+
+def test_zt_pipe_full_size_32(lgf):
+    """The headline lattice: 1024 tiles over 296 persistent CTAs, three or four tiles each."""
+    N = (32, 32, 32, 32)
+    U = gen.gen_links(N, 0.5, gen.BASE_SEED + 32)
+    res = []
+    for pipe in (0, 1):
+        gf = lgf.GaugeFixer(N, recon=12, zt_pipe=pipe)
+        gf.load_links(U)
+        r = gf.iterate(ALPHA, 3)
+        res.append((r.F, r.theta, gf.get_links()))
+        gf.close()
+    assert res[0][0] == res[1][0] and res[0][1] == res[1][1] and np.array_equal(res[0][2], res[1][2])
