@@ -13,6 +13,15 @@ site-iterations/s, and the GFlops the PAPER'S flop model would credit for that r
 (PAPER.md:185).  This build executes fewer operations than that model counts (4 packed FFT fields,
 rows-only link products), so the figure is a rate in the paper's currency, not an operation count.
 Inputs are the seeded synthetic generator of DESIGN.md section 4 (sigma = 0.5).
+
+    python bench_sweep.py --passes [--nt ...]
+
+times the paper's third axis instead, the decomposition of the 4D FFT ("The best choice for our
+4D problem is two 2D FFTs"), same run, same lattices, FP64 12-real and FP32 18-real: the fused
+three-pass default (2D | 2D * mask * 2D | 2D), 2D + 2D as four passes (LGF_OPT_FFT_PASSES = 4, the paper's best),
+4 x 1D as eight passes with the same register lines (= 8), and the generic per-axis O(N^2) transform
+(LGF_OPT_FFT_PATH = 1).  3D + 1D is not built (it needs a cluster-wide DSMEM transpose).
+Columns: ms per iteration and the time of the FFT passes alone (CUDA events around every launch).
 """
 import argparse
 import math
@@ -56,6 +65,50 @@ def alpha_scan(alphas, sizes, gen, lgf):
     return "\n".join(lines)
 
 
+def passes_sweep(nts, steps, gen, lgf):
+    import numpy as np
+    import torch
+
+    structures = [("3 passes: 2D | 2D mask 2D | 2D (default)", dict()),
+                  ("4 passes: 2D + 2D (the paper's best, P:119)", dict(fft_passes=4)),
+                  ("8 passes: 4 x 1D, register lines", dict(fft_passes=8)),
+                  ("8 passes: per-axis O(N^2) transform (generic path)", dict(fft_path=1))]
+    lines = ["| lattice | precision | reals/link | FFT structure | FFT launches/iteration | ms/iteration | FFT passes alone, ms | site-iterations/s |",
+             "|---|---|---|---|---|---|---|---|"]
+    for nt in nts:
+        N = (32, 32, 32, nt)
+        V = 32 * 32 * 32 * nt
+        U = gen.gen_links(N, 0.5, gen.BASE_SEED + 3200 + nt)
+        for prec, recon in (("fp64", 12), ("fp32", 18)):
+            Ud = torch.from_numpy(U.astype(np.complex64 if prec == "fp32" else np.complex128)).cuda()
+            for name, opt in structures:
+                try:
+                    gf = lgf.GaugeFixer(N, precision=prec, recon=recon, **opt)
+                except lgf.LgfError as e:
+                    lines.append(f"| 32^3 x {nt} | {prec} | {recon} | {name} | - | not available ({e.code}) | - | - |")
+                    continue
+                gf.load_links(Ud)
+                gf.iterate(0.08, 5)
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                torch.cuda.synchronize()
+                with torch.cuda.stream(gf.stream):
+                    e0.record(gf.stream)
+                    gf.iterate(0.08, steps, sync=False)
+                    e1.record(gf.stream)
+                torch.cuda.synchronize()
+                ms = e0.elapsed_time(e1) / steps
+                gf.set_option(lgf.OPT_PROFILE, 1)
+                gf.reset_counters()
+                gf.iterate(0.08, steps)
+                kt = gf.kernel_times()
+                fft_ms = sum(v[0] for k, v in kt.items() if k.startswith("fft_")) / steps
+                nl = sum(v[1] for k, v in kt.items() if k.startswith("fft_")) // steps
+                lines.append(f"| 32^3 x {nt} | {prec} | {recon} | {name} | {nl} | {ms:.4f} | {fft_ms:.4f} | {V / (ms * 1e-3):.3e} |")
+                gf.close()
+            del Ud
+    return "\n".join(lines)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--nt", type=int, nargs="+", default=[8, 16, 32, 48, 64])
@@ -64,6 +117,7 @@ def main():
     ap.add_argument("--alpha-scan", type=float, nargs="*", default=None,
                     help="instead of the timing sweep: iterations to theta <= 1e-15 for these alpha, both g maps")
     ap.add_argument("--scan-n", type=int, nargs="+", default=[16, 32])
+    ap.add_argument("--passes", action="store_true", help="instead of the precision / storage sweep: the FFT pass-structure axis")
     args = ap.parse_args()
     import numpy as np
     import torch
@@ -73,6 +127,14 @@ def main():
 
     if args.alpha_scan is not None:
         text = alpha_scan(args.alpha_scan or [0.04, 0.05, 0.0625, 0.07, 0.08, 0.09, 0.10, 0.11, 0.12], args.scan_n, gen, lgf)
+        print(text)
+        if args.out:
+            with open(args.out, "w") as f:
+                f.write(text + "\n")
+        return
+
+    if args.passes:
+        text = passes_sweep(args.nt, args.steps, gen, lgf)
         print(text)
         if args.out:
             with open(args.out, "w") as f:

@@ -63,7 +63,12 @@ enum { LGF_LAYOUT_AOS = 0, LGF_LAYOUT_AOS12 = 1 };
 
 /* lgf_set_option keys.  Options must be set before lgf_workspace_bytes / lgf_bind. */
 enum {
-    LGF_OPT_RECON = 1,          /* 18 (default) or 12 reals stored per link */
+    LGF_OPT_RECON = 1,          /* 18 (default) or 12 reals stored per link.  The links handed
+                                   to lgf_load_links must be SU(3) to working precision either way: with 12 reals
+                                   row 2 is never stored, and with 18 reals the fused link kernel (FUSION = 1)
+                                   stores row 2 of g U g^dagger as conj(row0 x row1) of the product instead of
+                                   multiplying it out (equal to rounding for special unitary links, DESIGN.md
+                                   reading R15); FUSION = 0 multiplies all three rows. */
     LGF_OPT_FFT_BATCH = 2,      /* 4 (default): Delta packed into 4 complex fields; 9: one FFT per
                                    element of the Delta matrix as in Alg. 1 line 3 */
     LGF_OPT_MAX_ITER = 3,       /* iteration cap of lgf_fix, default 100000 */
@@ -120,11 +125,20 @@ enum {
                                    of L2); a positive value must divide Nz (Nz = plain storage order).  Changes
                                    only the order of the FP64 partial sums of F and theta (1e-16 relative), not
                                    what is computed.  Before lgf_bind. */
-    LGF_OPT_ZT_PIPE = 13        /* middle pass of the tiled FFT ((z,t) forward, mask, (z,t) inverse; Alg. 1 lines 3-8,
+    LGF_OPT_ZT_PIPE = 13,       /* middle pass of the tiled FFT ((z,t) forward, mask, (z,t) inverse; Alg. 1 lines 3-8,
                                    PAPER.md:80-90).  1: persistent CTAs that keep their shared-memory tile and fetch
                                    the next tile with asynchronous copies (cp.async) while the current one is
                                    finished; 0: one tile per thread group, loaded straight into registers.  Same
                                    arithmetic in the same order: bitwise the same w.  Any time. */
+    LGF_OPT_FFT_PASSES = 14     /* pass structure of the tiled 4D FFT, the axis of the paper's comparison of 4 x 1D,
+                                   2D + 2D and 3D + 1D decompositions.  3 (default): (x,y) forward |
+                                   (z,t) forward, mask, (z,t) inverse in one tile visit | (x,y) inverse.  4: 2D + 2D
+                                   as the paper runs it, (x,y) forward | (z,t) forward and mask | (z,t) inverse |
+                                   (x,y) inverse (available for square and 32 x n (z,t) tiles).  8: 4 x 1D, one pass per
+                                   axis and direction with the same register lines (g is then rebuilt from w by the link
+                                   kernel; not with ACCUM_G).  Same w to rounding; timing comparison only
+                                   (bench_sweep.py --passes).  lgf_bind fails with LGF_ERR_INVALID_ARG where a structure
+                                   is not available.  Before lgf_bind. */
 };
 
 /* lgf_get_field / lgf_set_field selectors */

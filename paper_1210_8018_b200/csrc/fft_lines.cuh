@@ -218,4 +218,21 @@ template <int NA, int NB, int C, int SMIN> struct Tile {
 // CTA size: at least 128 threads, whole groups
 constexpr int cta_threads(int group) { return group >= 128 ? group : (128 / group) * group; }
 
+// p_max^2 / (p^2 V) for one mode (eq. 1.2; zero mode -> 0, reading R7): c = p_max^2 / V.
+// The reciprocal is the hardware seed (MUFU.RCP64H, about 20 bits) refined by two Newton steps, each
+// of which doubles the number of correct bits: p^2 is a sum of four numbers in [0, 4], so none of the
+// special cases of an IEEE division can occur and its slow path (a CALL per mode in SASS: 16 per thread
+// and tile, a sixth of the FP64 instructions of this pass) is dead weight.  Result within 2 ulp of c / p2.
+__device__ __forceinline__ double mask_factor(double c, double p2)
+{
+    double y;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(p2));
+    double e = fma(-p2, y, 1.0);
+    y = fma(y, e, y);
+    e = fma(-p2, y, 1.0);
+    y = fma(y, e, y);
+    return (p2 > 0.0) ? c * y : 0.0;
+}
+
+
 } // namespace lgf

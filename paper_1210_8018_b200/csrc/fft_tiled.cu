@@ -38,7 +38,9 @@ template <typename T, int NA, int NB> struct XYCfg {
     static constexpr size_t SMEM = (size_t)G * TL::ELEMS * sizeof(cx<T>);
 };
 
-template <typename T, int NA, int NB, int INVERSE>
+// AX = 0: both axes (the pass of the 3- and 4-pass structures).  AX = 1 / 2: the x-lines / y-lines alone, the
+// 1D passes of the 4 x 1D structure of the paper's comparison (LGF_OPT_FFT_PASSES = 8).
+template <typename T, int NA, int NB, int INVERSE, int AX = 0>
 __global__ void __launch_bounds__((XYCfg<T, NA, NB>::CTA))
 k_fft_xy(cx<T> *__restrict__ w, int64_t nplanes, const Ctrl *ctrl)
 {
@@ -61,6 +63,44 @@ k_fft_xy(cx<T> *__restrict__ w, int64_t nplanes, const Ctrl *ctrl)
     const bool on_y = ok && xa < NA && t < TL::SB * NA, on_x = ok && yb < NB && t < TL::SA * NB;
     const unsigned my = __ballot_sync(0xffffffffu, on_y), mx = __ballot_sync(0xffffffffu, on_x);
 
+    if (AX == 2) {                                        // y-lines only: global -> registers -> global, in place
+        if (on_y) {
+            cx<T> v[LB::NL];
+#pragma unroll
+            for (int i = 0; i < LB::NL; i++) v[i] = f[LB::nat(i, ha) * NA + xa];
+            LB::template dif<SIGN>(v, ha, my);
+#pragma unroll
+            for (int q = 0; q < LB::NL; q++) f[LB::slot(q, ha) * NA + xa] = v[q];
+        }
+        return;
+    }
+    if (AX == 1) {                                        // x-lines only: contiguous lines go through shared memory
+        if (ok) {
+#pragma unroll
+            for (int k = 0; k < (NA * NB + TP - 1) / TP; k++) {
+                const int e = t + k * TP;
+                if (e < NA * NB) sm[(e / NA) * TL::RS + (e % NA)] = f[e];
+            }
+        }
+        __syncthreads();
+        if (on_x) {
+            cx<T> v[LA::NL];
+#pragma unroll
+            for (int i = 0; i < LA::NL; i++) v[i] = sm[yb * TL::RS + LA::nat(i, hb)];
+            LA::template dif<SIGN>(v, hb, mx);
+#pragma unroll
+            for (int q = 0; q < LA::NL; q++) sm[yb * TL::RS + LA::slot(q, hb)] = v[q];
+        }
+        __syncthreads();
+        if (ok) {
+#pragma unroll
+            for (int k = 0; k < (NA * NB + TP - 1) / TP; k++) {
+                const int e = t + k * TP;
+                if (e < NA * NB) f[e] = sm[(e / NA) * TL::RS + (e % NA)];
+            }
+        }
+        return;
+    }
     if (!INVERSE) {
         if (on_y) {                                       // line along y at x = xa
             cx<T> v[LB::NL];
@@ -341,6 +381,57 @@ k_fft_xy_inv_g2(const cx<T> *__restrict__ w, cx<T> *__restrict__ gbuf, int64_t V
     cluster.sync();                                          // the peer may still be reading this CTA's fields
 }
 
+// ---------------------------------------------------------------- 1D passes along z or t
+// One line per thread (or pair of lanes), consecutive threads on consecutive x: the 1D passes of the
+// 4 x 1D structure (LGF_OPT_FFT_PASSES = 8).  Natural order in, natural order out, in place.  MASK: the
+// t-forward pass also applies p_max^2/(p^2 V), zero mode -> 0 (eq. 1.2).
+template <typename T, int N, int S, int SIGN, bool MASK>
+__global__ void __launch_bounds__(256)
+k_fft_axis(cx<T> *__restrict__ w, Geom geo, int axis, int64_t nlines, const double *__restrict__ ptab, double pmax2_over_V, const Ctrl *ctrl)
+{
+    if (*(volatile const int *)&ctrl->done) return;
+    typedef Line<T, N, S> LN;
+    int ll, h;
+    line_of_thread<S>((int)threadIdx.x, ll, h);
+    const int64_t line = (int64_t)blockIdx.x * (256 / S) + ll;
+    const bool on = line < nlines;
+    const unsigned m = __ballot_sync(0xffffffffu, on);
+    if (!on) return;
+    // line -> (x, y, the other of z / t, field); axis = 2: lines along z, axis = 3: lines along t
+    const int Nx = geo.N[0], Ny = geo.N[1], No = geo.N[axis == 2 ? 3 : 2];
+    unsigned u = (unsigned)line;
+    const int x = (int)(u % (unsigned)Nx); u /= (unsigned)Nx;
+    const int y = (int)(u % (unsigned)Ny); u /= (unsigned)Ny;
+    const int o = (int)(u % (unsigned)No); u /= (unsigned)No;
+    const int64_t so = geo.st[axis == 2 ? 3 : 2], sa = geo.st[axis];
+    cx<T> *f = w + (int64_t)u * geo.V + x + (int64_t)Nx * y + so * o;
+    cx<T> v[LN::NL];
+#pragma unroll
+    for (int i = 0; i < LN::NL; i++) v[i] = f[sa * LN::nat(i, h)];
+    LN::template dif<SIGN>(v, h, m);
+    if (MASK) {
+        const int z = axis == 2 ? 0 : o;                 // MASK runs on t-lines only (axis = 3): o is z
+        const double pxyz = ptab[x] + ptab[Nx + y] + ptab[Nx + Ny + z];
+        const double *pt = ptab + Nx + Ny + geo.N[2];
+#pragma unroll
+        for (int q = 0; q < LN::NL; q++) v[q] = cscale(v[q], (T)mask_factor(pmax2_over_V, pxyz + pt[LN::slot(q, h)]));
+    }
+#pragma unroll
+    for (int q = 0; q < LN::NL; q++) f[sa * LN::slot(q, h)] = v[q];
+}
+
+template <typename T, int N> static int launch_axis_n(const FftArgs &a, int axis, int sign, int mask, cudaStream_t st)
+{
+    constexpr int S = split_of(N, split_min<T>(N, N));
+    const int64_t nlines = (int64_t)a.nfields * a.geo.V / N;
+    const unsigned grid = (unsigned)((nlines + 256 / S - 1) / (256 / S));
+    const double c = a.pmax2 / (double)a.geo.V;
+    if (sign < 0 && mask) k_fft_axis<T, N, S, -1, true><<<grid, 256, 0, st>>>((cx<T> *)a.w, a.geo, axis, nlines, a.ptab, c, a.ctrl);
+    else if (sign < 0) k_fft_axis<T, N, S, -1, false><<<grid, 256, 0, st>>>((cx<T> *)a.w, a.geo, axis, nlines, a.ptab, c, a.ctrl);
+    else k_fft_axis<T, N, S, +1, false><<<grid, 256, 0, st>>>((cx<T> *)a.w, a.geo, axis, nlines, a.ptab, c, a.ctrl);
+    return 0;
+}
+
 // ---------------------------------------------------------------- dispatch
 template <typename T, int N> static int setup_xy_n()
 {
@@ -348,6 +439,10 @@ template <typename T, int N> static int setup_xy_n()
     e = cudaFuncSetAttribute(k_fft_xy<T, N, N, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)XYCfg<T, N, N>::SMEM);
     if (e != cudaSuccess) return 1;
     e = cudaFuncSetAttribute(k_fft_xy<T, N, N, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)XYCfg<T, N, N>::SMEM);
+    if (e != cudaSuccess) return 1;
+    e = cudaFuncSetAttribute(k_fft_xy<T, N, N, 0, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)XYCfg<T, N, N>::SMEM);
+    if (e != cudaSuccess) return 1;
+    e = cudaFuncSetAttribute(k_fft_xy<T, N, N, 1, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)XYCfg<T, N, N>::SMEM);
     if (e != cudaSuccess) return 1;
     if (XYGCfg<T, N, N>::FITS) {
         e = cudaFuncSetAttribute(k_fft_xy_inv_g<T, N, N, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)XYGCfg<T, N, N>::SMEM);
@@ -370,6 +465,18 @@ template <typename T, int N> static int launch_xy_n(const FftArgs &a, int which,
     const unsigned grid = (unsigned)((nplanes + X::G - 1) / X::G);
     if (which == 0) k_fft_xy<T, N, N, 0><<<grid, X::CTA, X::SMEM, st>>>((cx<T> *)a.w, nplanes, a.ctrl);
     else k_fft_xy<T, N, N, 1><<<grid, X::CTA, X::SMEM, st>>>((cx<T> *)a.w, nplanes, a.ctrl);
+    return 0;
+}
+// 1D passes along x (ax = 1) or y (ax = 2), forward (inverse = 0) or inverse
+template <typename T, int N> static int launch_xy1d_n(const FftArgs &a, int inverse, int ax, cudaStream_t st)
+{
+    typedef XYCfg<T, N, N> X;
+    const int64_t nplanes = (int64_t)a.nfields * a.geo.N[2] * a.geo.N[3];
+    const unsigned grid = (unsigned)((nplanes + X::G - 1) / X::G);
+    if (!inverse && ax == 1) k_fft_xy<T, N, N, 0, 1><<<grid, X::CTA, X::SMEM, st>>>((cx<T> *)a.w, nplanes, a.ctrl);
+    else if (!inverse) k_fft_xy<T, N, N, 0, 2><<<grid, X::CTA, X::SMEM, st>>>((cx<T> *)a.w, nplanes, a.ctrl);
+    else if (ax == 1) k_fft_xy<T, N, N, 1, 1><<<grid, X::CTA, X::SMEM, st>>>((cx<T> *)a.w, nplanes, a.ctrl);
+    else k_fft_xy<T, N, N, 1, 2><<<grid, X::CTA, X::SMEM, st>>>((cx<T> *)a.w, nplanes, a.ctrl);
     return 0;
 }
 
@@ -400,7 +507,9 @@ template <typename T, int N> static int gbuf_fits_n() { return (XYGCfg<T, N, N>:
 #define LGF_ZT_DECL(N)                                            \
     int zt_columns_na##N(int nt, int prec);                       \
     int zt_setup_na##N(int nt, int prec);                         \
-    int zt_launch_na##N(const FftArgs &a, cudaStream_t st);
+    int zt_launch_na##N(const FftArgs &a, cudaStream_t st);       \
+    int zt_has_half_na##N(int nt);                                \
+    int zt_launch_half_na##N(const FftArgs &a, int inverse, cudaStream_t st);
 LGF_ZT_DECL(8) LGF_ZT_DECL(12) LGF_ZT_DECL(16) LGF_ZT_DECL(24) LGF_ZT_DECL(32) LGF_ZT_DECL(48) LGF_ZT_DECL(64)
 #undef LGF_ZT_DECL
 #define LGF_NZ_SWITCH(FN, ...)                \
@@ -476,6 +585,56 @@ static int run_zt(const FftArgs &a, cudaStream_t st)
 void launch_fft_tiled(const FftArgs &a, int which, cudaStream_t st)
 {
     if (which == 1) run_zt(a, st); else run_xy(a, which, st);
+}
+
+// ---- the other pass structures of the paper's comparison (LGF_OPT_FFT_PASSES)
+static int run_xy1d(const FftArgs &a, int inverse, int ax, cudaStream_t st)
+{
+    const int n = a.geo.N[0], prec = a.prec;
+    LGF_FFT_SWITCH(launch_xy1d_n, a, inverse, ax, st)
+    return 1;
+}
+static int run_axis(const FftArgs &a, int axis, int sign, int mask, cudaStream_t st)
+{
+    const int n = a.geo.N[axis], prec = a.prec;
+    LGF_FFT_SWITCH(launch_axis_n, a, axis, sign, mask, st)
+    return 1;
+}
+static int run_zt_half(const FftArgs &a, int inverse, cudaStream_t st)
+{
+    const int nz = a.geo.N[2];
+    LGF_NZ_SWITCH(zt_launch_half_na, a, inverse, st)
+    return 1;
+}
+bool fft_tiled_passes_supported(const int N[4], int prec, int passes)
+{
+    if (!fft_tiled_supported(N, prec)) return false;
+    if (passes == 3 || passes == 8) return true;
+    if (passes == 4) { const int nz = N[2]; LGF_NZ_SWITCH(zt_has_half_na, N[3]) return false; }
+    return false;
+}
+// 2D + 2D as four passes (the paper's best): step 0 (x,y) forward, 1 (z,t) forward times the mask,
+// 2 (z,t) inverse, 3 (x,y) inverse (or launch_fft_tiled_inv_g in its place)
+void launch_fft_tiled_4pass(const FftArgs &a, int step, cudaStream_t st)
+{
+    if (step == 0) run_xy(a, 0, st);
+    else if (step == 1) run_zt_half(a, 0, st);
+    else if (step == 2) run_zt_half(a, 1, st);
+    else run_xy(a, 2, st);
+}
+// 4 x 1D as eight passes: steps 0..3 forward along y, x, z, t (the mask rides on the last), 4..7 inverse along t, z, x, y
+void launch_fft_tiled_8pass(const FftArgs &a, int step, cudaStream_t st)
+{
+    switch (step) {
+    case 0: run_xy1d(a, 0, 2, st); break;
+    case 1: run_xy1d(a, 0, 1, st); break;
+    case 2: run_axis(a, 2, -1, 0, st); break;
+    case 3: run_axis(a, 3, -1, 1, st); break;
+    case 4: run_axis(a, 3, +1, 0, st); break;
+    case 5: run_axis(a, 2, +1, 0, st); break;
+    case 6: run_xy1d(a, 1, 1, st); break;
+    default: run_xy1d(a, 1, 2, st); break;
+    }
 }
 
 // pass 2 fused with the g build: needs the 4 packed fields (nfields == 4)

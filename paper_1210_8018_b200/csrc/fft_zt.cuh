@@ -16,22 +16,6 @@ namespace lgf {
 #ifndef LGF_ZT_MAXB
 #define LGF_ZT_MAXB 2   /* 3 measured slower at 32^4 (47.6 vs 45.5 us: spills), equal at 48^4 */
 #endif
-// p_max^2 / (p^2 V) for one mode (eq. 1.2; zero mode -> 0, reading R7): c = p_max^2 / V.
-// The reciprocal is the hardware seed (MUFU.RCP64H, about 20 bits) refined by two Newton steps, each
-// of which doubles the number of correct bits: p^2 is a sum of four numbers in [0, 4], so none of the
-// special cases of an IEEE division can occur and its slow path (a CALL per mode in SASS: 16 per thread
-// and tile, a sixth of the FP64 instructions of this pass) is dead weight.  Result within 2 ulp of c / p2.
-__device__ __forceinline__ double mask_factor(double c, double p2)
-{
-    double y;
-    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(p2));
-    double e = fma(-p2, y, 1.0);
-    y = fma(y, e, y);
-    e = fma(-p2, y, 1.0);
-    y = fma(y, e, y);
-    return (p2 > 0.0) ? c * y : 0.0;
-}
-
 // 16- or 8-byte asynchronous copy global -> shared (LDGSTS): the data is in flight without holding registers
 template <typename V> __device__ __forceinline__ void cp_async_elem(V *smem_dst, const V *gsrc)
 {
@@ -232,6 +216,72 @@ k_fft_zt_pipe(cx<T> *__restrict__ w, Geom geo, const double *__restrict__ ptab, 
     cp_async_wait_all();
 }
 
+// ---------------------------------------------------------------- the (z,t) pass as two launches
+// 2D + 2D without the fusion of the middle (the structure the paper found best with CUFFT, PAPER.md:119:
+// "two 2D FFTs"; LGF_OPT_FFT_PASSES = 4): INVERSE = 0 transforms a tile forward along z and t and applies the
+// mask, INVERSE = 1 transforms it back; the field crosses HBM once more than in k_fft_zt.  z-lines
+// straight from global memory, through shared memory, t-lines stored straight to global memory;
+// natural order in global memory on both sides.
+template <typename T, int NA, int NB, int C, int INVERSE>
+__global__ void __launch_bounds__((ZTCfg<T, NA, NB, C>::CTA), (ZTCfg<T, NA, NB, C>::MINB))
+k_fft_zt_half(cx<T> *__restrict__ w, Geom geo, const double *__restrict__ ptab, double pmax2_over_V, int64_t ntiles, const Ctrl *ctrl)
+{
+    if (*(volatile const int *)&ctrl->done) return;
+    typedef ZTCfg<T, NA, NB, C> CF;
+    typedef typename CF::TL TL;
+    typedef Line<T, NA, TL::SA> LA;
+    typedef Line<T, NB, TL::SB> LB;
+    constexpr int TT = CF::TT, G = CF::G;
+    constexpr int SIGN = INVERSE ? +1 : -1;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    double *pt = (double *)smem_raw;
+    cx<T> *sm0 = (cx<T> *)(smem_raw + CF::PT);
+    const int grp = threadIdx.x / TT, t = threadIdx.x % TT;
+    cx<T> *sm = sm0 + (size_t)grp * TL::ELEMS;
+    const int64_t tile = (int64_t)blockIdx.x * G + grp;
+    const bool ok = tile < ntiles && grp < G;
+    const int Nx = geo.N[0], Ny = geo.N[1];
+    const int xchunks = Nx / C;
+    const int xc = (int)(tile % xchunks);
+    const int y = (int)((tile / xchunks) % Ny);
+    const int64_t fld = tile / ((int64_t)xchunks * Ny);
+    const int x0 = xc * C;
+    cx<T> *f = w + fld * geo.V + x0 + (int64_t)Nx * y;
+    const int64_t sz = geo.st[2], st = geo.st[3];
+    if (!INVERSE)
+        for (int i = threadIdx.x; i < NB; i += CF::CTA) pt[i] = ptab[Nx + Ny + NA + i];
+    int la, ha, lb, hb;
+    line_of_thread<TL::SA>(t, la, ha);
+    line_of_thread<TL::SB>(t, lb, hb);
+    const int ca = la % C, ta = la / C, cb = lb % C, zb = lb / C;
+    const bool on_z = ok && ta < NB && t < TL::SA * C * NB, on_t = ok && zb < NA && t < TL::SB * C * NA;
+    const unsigned mz = __ballot_sync(0xffffffffu, on_z), mt = __ballot_sync(0xffffffffu, on_t);
+    if (on_z) {
+        cx<T> v[LA::NL];
+        const cx<T> *g = f + ca + st * ta;
+#pragma unroll
+        for (int i = 0; i < LA::NL; i++) v[i] = g[sz * LA::nat(i, ha)];
+        LA::template dif<SIGN>(v, ha, mz);
+#pragma unroll
+        for (int q = 0; q < LA::NL; q++) sm[ta * TL::RS + LA::slot(q, ha) * C + ca] = v[q];
+    }
+    __syncthreads();
+    if (on_t) {
+        cx<T> v[LB::NL];
+#pragma unroll
+        for (int i = 0; i < LB::NL; i++) v[i] = sm[LB::nat(i, hb) * TL::RS + zb * C + cb];
+        LB::template dif<SIGN>(v, hb, mt);
+        if (!INVERSE) {
+            const double pxyz = ptab[x0 + cb] + ptab[Nx + y] + ptab[Nx + Ny + zb];
+#pragma unroll
+            for (int q = 0; q < LB::NL; q++) v[q] = cscale(v[q], (T)mask_factor(pmax2_over_V, pxyz + pt[LB::slot(q, hb)]));
+        }
+        cx<T> *g = f + cb + sz * zb;
+#pragma unroll
+        for (int q = 0; q < LB::NL; q++) g[st * LB::slot(q, hb)] = v[q];
+    }
+}
+
 // ---------------------------------------------------------------- launchers
 // x-columns per (z,t) tile: 64-byte runs in global memory (FP64), halved while the tile does not fit
 // in shared memory or does not divide Nz.  The columns must also divide Nx, which the caller checks
@@ -245,11 +295,12 @@ template <typename T, int NA, int NB> struct ZTC {
     static constexpr int C = tile_bytes(WANT) <= 200 * 1024 && NA % WANT == 0 ? WANT : (tile_bytes(WANT / 2) <= 200 * 1024 && NA % (WANT / 2) == 0 ? WANT / 2 : WANT / 4);
     static_assert(C >= 1 && tile_bytes(C) <= 220 * 1024, "(z,t) tile does not fit in shared memory");
 };
-// The persistent variant (LGF_OPT_ZT_PIPE) is instantiated for the square tiles and the 32 x n tiles of the
-// paper's lattices only (measured slower than the plain kernel on every lattice tried, profiles/r02*);
+// The persistent variant (LGF_OPT_ZT_PIPE) and the two-launch form (LGF_OPT_FFT_PASSES = 4) are instantiated
+// for the square tiles and the 32 x n tiles of the paper's lattices only (measured slower than the plain kernel on every lattice tried, profiles/r02*);
 // other pairs run the plain kernel whatever the option says.
 constexpr bool zt_pipe_pair(int na, int nb) { return na == nb || (na == 32 && (nb == 8 || nb == 16 || nb == 48 || nb == 64)); }
 
+template <typename T, int NA, int NB> int setup_zt_half_n();
 template <typename T, int NA, int NB> int setup_zt_n()
 {
     constexpr int C = ZTC<T, NA, NB>::C;
@@ -260,7 +311,31 @@ template <typename T, int NA, int NB> int setup_zt_n()
         e = cudaFuncSetAttribute(k_fft_zt_pipe<T, NA, NB, C>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Z::SMEM);
         if (e != cudaSuccess) return 1;
     }
+    return setup_zt_half_n<T, NA, NB>();
+}
+
+template <typename T, int NA, int NB> int setup_zt_half_n()
+{
+    if constexpr (zt_pipe_pair(NA, NB)) {
+        constexpr int C = ZTC<T, NA, NB>::C;
+        typedef ZTCfg<T, NA, NB, C> Z;
+        if (cudaFuncSetAttribute(k_fft_zt_half<T, NA, NB, C, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Z::SMEM) != cudaSuccess) return 1;
+        if (cudaFuncSetAttribute(k_fft_zt_half<T, NA, NB, C, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Z::SMEM) != cudaSuccess) return 1;
+    }
     return 0;
+}
+template <typename T, int NA, int NB> int launch_zt_half_n(const FftArgs &a, int inverse, cudaStream_t st)
+{
+    if constexpr (zt_pipe_pair(NA, NB)) {
+        constexpr int C = ZTC<T, NA, NB>::C;
+        typedef ZTCfg<T, NA, NB, C> Z;
+        const int64_t ntiles = (int64_t)a.nfields * a.geo.N[1] * (a.geo.N[0] / C);
+        const unsigned grid = (unsigned)((ntiles + Z::G - 1) / Z::G);
+        if (inverse) k_fft_zt_half<T, NA, NB, C, 1><<<grid, Z::CTA, Z::SMEM, st>>>((cx<T> *)a.w, a.geo, a.ptab, a.pmax2 / (double)a.geo.V, ntiles, a.ctrl);
+        else k_fft_zt_half<T, NA, NB, C, 0><<<grid, Z::CTA, Z::SMEM, st>>>((cx<T> *)a.w, a.geo, a.ptab, a.pmax2 / (double)a.geo.V, ntiles, a.ctrl);
+        return 0;
+    }
+    return 1;
 }
 
 inline int sm_count()

@@ -42,5 +42,18 @@ int LGF_ZT_FN(zt_launch_na)(const FftArgs &a, cudaStream_t st)
     LGF_NT_SWITCH((launch_zt_n<double, LGF_ZT_NA, NB>(a, st)), (launch_zt_n<float, LGF_ZT_NA, NB>(a, st)))
     return 1;
 }
+// the two-launch form (LGF_OPT_FFT_PASSES = 4): is it instantiated for this pair, and its launcher
+int LGF_ZT_FN(zt_has_half_na)(int nt)
+{
+    const int prec = 0;
+    LGF_NT_SWITCH((zt_pipe_pair(LGF_ZT_NA, NB) ? 1 : 0), 0)
+    return 0;
+}
+int LGF_ZT_FN(zt_launch_half_na)(const FftArgs &a, int inverse, cudaStream_t st)
+{
+    const int nt = a.geo.N[3], prec = a.prec;
+    LGF_NT_SWITCH((launch_zt_half_n<double, LGF_ZT_NA, NB>(a, inverse, st)), (launch_zt_half_n<float, LGF_ZT_NA, NB>(a, inverse, st)))
+    return 1;
+}
 
 } // namespace lgf

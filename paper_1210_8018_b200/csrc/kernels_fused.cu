@@ -33,20 +33,47 @@ static const int FUSED_THREADS = LGF_FUSED_THREADS;
 #endif
 
 // links are streamed: read (twice, the second time from L2) and written once per iteration
-template <typename V> __device__ __forceinline__ V ld_link(const V *p) { return __ldg(p); }
+// tuning macros for the cache behaviour of the loads (same-run A/B, profiles/r02_link_kernel.md):
+// LGF_LINK_LD: 0 ld.global.nc (default), 1 ld.global.nc.L1::no_allocate (the links are streamed; leave L1 to g)
+#ifndef LGF_LINK_LD
+#define LGF_LINK_LD 0
+#endif
+#ifndef LGF_FUSED_PREFETCH
+#define LGF_FUSED_PREFETCH 0
+#endif
+__device__ __forceinline__ double2 ld_na(const double2 *p)
+{
+    double2 v;
+    asm volatile("ld.global.nc.L1::no_allocate.v2.f64 {%0, %1}, [%2];" : "=d"(v.x), "=d"(v.y) : "l"(p));
+    return v;
+}
+__device__ __forceinline__ float2 ld_na(const float2 *p)
+{
+    float2 v;
+    asm volatile("ld.global.nc.L1::no_allocate.v2.f32 {%0, %1}, [%2];" : "=f"(v.x), "=f"(v.y) : "l"(p));
+    return v;
+}
+template <typename V> __device__ __forceinline__ V ld_link(const V *p)
+{
+#if LGF_LINK_LD == 1
+    return ld_na(p);
+#else
+    return __ldg(p);
+#endif
+}
+// Link stores as st.global.cs (evict first): the new links are not read again before the next iteration, and
+// written lines that linger in L2 push out the neighbour links and g that the kernel re-reads.  Same-run A/B on
+// B200 (profiles/r02_link_kernel.md): FP64 32^4 12-real 211.2 -> 198.7 us, 32^4 18-real 273.2 -> 270.6, 64^4 4320 -> 4300,
+// 16^4 23.6 -> 23.2; FP32 48^4 18-real 682.7 -> 708.6 (worse), 32^4 12-real 129.4 -> 127.8: on for FP64, off for FP32.
 #ifndef LGF_LINK_STCS
-#define LGF_LINK_STCS 0
+#define LGF_LINK_STCS(V) (sizeof(V) == 16)
 #endif
 #ifndef LGF_W_EVICT_LAST
 #define LGF_W_EVICT_LAST 0
 #endif
 template <typename V> __device__ __forceinline__ void st_link(V *p, V v)
 {
-#if LGF_LINK_STCS
-    __stcs(p, v);       // written once, not read again before the next iteration: evict first
-#else
-    *p = v;
-#endif
+    if (LGF_LINK_STCS(V)) __stcs(p, v); else *p = v;
 }
 // Delta is read back by the first FFT pass right after this kernel: ask L2 to keep it
 __device__ __forceinline__ void st_field(double2 *p, double2 v)
@@ -198,6 +225,12 @@ k_update_measure(const cx<T> *__restrict__ lin, cx<T> *__restrict__ lout, const 
             }
             th = store_delta<T, PACK>(di, E, wout, V, s);
         } else {
+#if LGF_FUSED_PREFETCH
+            // The thread's own links are first touched by the forward products at the end of its life (a DRAM
+            // round trip each); ask L2 for them now, behind the backward products.
+#pragma unroll
+            for (int k = 0; k < 4 * NE; k++) asm volatile("prefetch.global.L2 [%0];" ::"l"(lin + (int64_t)k * V + s));
+#endif
             // Backward links first: only their sum enters A'(x),
             //     sum_nu U'_nu(x-nu) = [sum_nu H_nu(x-nu)] g^dagger(x),   H_nu(y) = g(y) U_nu(y),
             // so rows 0, 1 of each H are one product, row 2 is conj(row0 x row1) (H is special

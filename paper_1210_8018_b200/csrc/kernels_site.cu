@@ -85,7 +85,7 @@ __global__ void k_ctrl_reset(Ctrl *ctrl, double2 *hist, double eps)
 // With 12-real storage only rows 0, 1 of g U g^dagger are computed and stored (reading R15).
 template <typename T, int NE, int PACK>
 __global__ void __launch_bounds__(SITE_THREADS)
-k_update(cx<T> *__restrict__ links, const cx<T> *__restrict__ w, Geom geo, T a, int gexp, const Ctrl *ctrl)
+k_update(cx<T> *links, const cx<T> *__restrict__ w, Geom geo, T a, int gexp, const Ctrl *ctrl)
 {
     if (*(volatile const int *)&ctrl->done) return;
     const int64_t V = geo.V;
@@ -101,7 +101,7 @@ k_update(cx<T> *__restrict__ links, const cx<T> *__restrict__ w, Geom geo, T a, 
         const int64_t sp = s + (c[mu] == geo.N[mu] - 1 ? -(int64_t)(geo.N[mu] - 1) : (int64_t)1) * geo.st[mu];
         cx<T> g1[9], u[9], t[9], r[9];
         build_g<T, PACK>(w, V, sp, a, gexp, g1);
-        load_link<T, NE>(links, V, mu, s, u);
+        load_link_rw<T, NE>(links, V, mu, s, u);
         mul_rows<R>(g0, u, t);
         mul_rows_dag<R>(t, g1, r);
         cx<T> *p = links + (int64_t)mu * NE * V + s;
@@ -117,7 +117,7 @@ k_update(cx<T> *__restrict__ links, const cx<T> *__restrict__ w, Geom geo, T a, 
 // four links and G is read-only here; k_g_identity resets it afterwards.
 template <typename T, int NE>
 __global__ void __launch_bounds__(SITE_THREADS)
-k_apply_g(cx<T> *__restrict__ links, const cx<T> *__restrict__ gacc, Geom geo)
+k_apply_g(cx<T> *links, const cx<T> *__restrict__ gacc, Geom geo)
 {
     const int64_t V = geo.V;
     const int64_t rr = (int64_t)blockIdx.x * SITE_THREADS + threadIdx.x;
@@ -134,7 +134,7 @@ k_apply_g(cx<T> *__restrict__ links, const cx<T> *__restrict__ gacc, Geom geo)
         cx<T> g1[9], u[9], t[9], r[9];
         load_g01<T, 4, true>(gacc, V, sp, (T)0, 0, g1);
         su3_row2(g1);
-        load_link<T, NE>(links, V, mu, s, u);
+        load_link_rw<T, NE>(links, V, mu, s, u);
         mul_rows<R>(g0, u, t);
         mul_rows_dag<R>(t, g1, r);
         cx<T> *p = links + (int64_t)mu * NE * V + s;

@@ -63,6 +63,12 @@ bool fft_tiled_supported(const int N[4], int prec);
 int fft_tiled_zt_columns(const int N[4], int prec);      // x-columns per (z,t) tile, 0 if the lattice is not tiled
 bool fft_tiled_gbuf_supported(const int N[4], int prec); // pass 2 with the g build fits in shared memory
 void launch_fft_tiled(const FftArgs &a, int which, cudaStream_t st);
+// the other pass structures of the paper's comparison (LGF_OPT_FFT_PASSES):
+// 4 = 2D + 2D as four launches (step 0..3; step 3 may be replaced by launch_fft_tiled_inv_g),
+// 8 = 4 x 1D as eight launches (step 0..7).  Same w as the three-pass default, to rounding.
+bool fft_tiled_passes_supported(const int N[4], int prec, int passes);
+void launch_fft_tiled_4pass(const FftArgs &a, int step, cudaStream_t st);
+void launch_fft_tiled_8pass(const FftArgs &a, int step, cudaStream_t st);
 // pass 2 of all 4 packed fields with g(x) = reunit(1 + (alpha/2) w(x)) as its epilogue: rows 0, 1 of g -> gbuf
 // accum = 1: gbuf holds the accumulated G and receives reunit(g G) instead (LGF_OPT_ACCUM_G)
 void launch_fft_tiled_inv_g(const FftArgs &a, void *gbuf, double alpha, int gexp, int accum, cudaStream_t st);

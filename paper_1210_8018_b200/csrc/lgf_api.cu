@@ -41,6 +41,7 @@ struct lgf_ctx {
     int graph = 1;           // LGF_OPT_GRAPH: replay captured iterations as a CUDA graph
     int zblock = 0;          // LGF_OPT_ZBLOCK: 0 = auto (resolved by lgf_bind into sa.geo.zb)
     int zt_pipe = 0;         // LGF_OPT_ZT_PIPE
+    int fft_passes = 3;      // LGF_OPT_FFT_PASSES: 3 (fused middle), 4 (2D + 2D), 8 (4 x 1D)
     cudaGraphExec_t gexec = nullptr;
     struct { double alpha, eps; int cur, wcur, gmap, unit; } gkey{};
     int64_t g_launches = 0, g_kcount[LGF_KERNEL_KINDS] = {0};
@@ -84,7 +85,7 @@ Layout make_layout(const lgf_ctx *c)
     // else the last FFT pass writes rows 0, 1 of g (6 complex per site) to gbuf
     // ACCUM_G: the links are not rewritten per iteration, so one buffer; the g buffer holds G
     const int nl = (c->fusion && !c->accum) ? 2 : 1;
-    const bool gb = c->fusion && c->pack == 4 && c->fft_path == 0 && fft_tiled_gbuf_supported(c->N, c->prec);
+    const bool gb = c->fusion && c->pack == 4 && c->fft_path == 0 && c->fft_passes != 8 && fft_tiled_gbuf_supported(c->N, c->prec);
     const int nw = (c->fusion && !gb) ? 2 : 1;
     for (int i = 0; i < 2; i++) { L.links[i] = off; if (i < nl) off = align_up(off + (size_t)4 * ne * c->V * e, 256); }
     for (int i = 0; i < 2; i++) { L.w[i] = off; if (i < nw) off = align_up(off + (size_t)c->pack * c->V * e, 256); }
@@ -172,11 +173,26 @@ void do_measure(lgf_ctx *c, double eps, int count_iter)
     c->wstate = 1;
 }
 
-void do_fourier(lgf_ctx *c)
+// the tiled FFT up to, but without, its last (x,y) inverse pass, in the pass structure LGF_OPT_FFT_PASSES asks for
+void do_fourier_head(lgf_ctx *c)
 {
-    if (c->tiled) {
+    if (c->fft_passes == 4) {
+        run_kernel(c, LGF_KERNEL_FFT_XY_FWD, 1, [&] { launch_fft_tiled_4pass(c->fa, 0, c->st); });
+        run_kernel(c, LGF_KERNEL_FFT_ZT, 2, [&] { launch_fft_tiled_4pass(c->fa, 1, c->st); launch_fft_tiled_4pass(c->fa, 2, c->st); });
+    } else {
         run_kernel(c, LGF_KERNEL_FFT_XY_FWD, 1, [&] { launch_fft_tiled(c->fa, 0, c->st); });
         run_kernel(c, LGF_KERNEL_FFT_ZT, 1, [&] { launch_fft_tiled(c->fa, 1, c->st); });
+    }
+}
+
+void do_fourier(lgf_ctx *c)
+{
+    if (c->tiled && c->fft_passes == 8) {
+        run_kernel(c, LGF_KERNEL_FFT_XY_FWD, 2, [&] { launch_fft_tiled_8pass(c->fa, 0, c->st); launch_fft_tiled_8pass(c->fa, 1, c->st); });
+        run_kernel(c, LGF_KERNEL_FFT_ZT, 4, [&] { for (int s = 2; s < 6; s++) launch_fft_tiled_8pass(c->fa, s, c->st); });
+        run_kernel(c, LGF_KERNEL_FFT_XY_INV, 2, [&] { launch_fft_tiled_8pass(c->fa, 6, c->st); launch_fft_tiled_8pass(c->fa, 7, c->st); });
+    } else if (c->tiled) {
+        do_fourier_head(c);
         run_kernel(c, LGF_KERNEL_FFT_XY_INV, 1, [&] { launch_fft_tiled(c->fa, 2, c->st); });
     } else {
         run_kernel(c, LGF_KERNEL_FFT_GENERIC, 8, [&] { launch_fft_generic(c->fa, c->st); });
@@ -207,8 +223,7 @@ void do_iteration(lgf_ctx *c, double alpha, double eps)
 {
     if (c->accum) {
         // w_buf[0] holds Delta of G U G^dagger; the last FFT pass turns it into g and G <- g G
-        run_kernel(c, LGF_KERNEL_FFT_XY_FWD, 1, [&] { launch_fft_tiled(c->fa, 0, c->st); });
-        run_kernel(c, LGF_KERNEL_FFT_ZT, 1, [&] { launch_fft_tiled(c->fa, 1, c->st); });
+        do_fourier_head(c);
         run_kernel(c, LGF_KERNEL_FFT_XY_INV_GACC, 1, [&] { launch_fft_tiled_inv_g(c->fa, c->gbuf, alpha, c->gmap, 1, c->st); });
         run_kernel(c, LGF_KERNEL_MEASURE_ACC, 1, [&] { launch_measure_acc(c->sa, c->gbuf, eps, c->st); });
         c->acc_dirty = true;
@@ -224,8 +239,7 @@ void do_iteration(lgf_ctx *c, double alpha, double eps)
     // w_buf[wcur] holds Delta of links_buf[cur]
     void *lin = c->links_buf[c->cur], *lout = c->links_buf[c->cur ^ 1];
     if (c->use_gbuf) {
-        run_kernel(c, LGF_KERNEL_FFT_XY_FWD, 1, [&] { launch_fft_tiled(c->fa, 0, c->st); });
-        run_kernel(c, LGF_KERNEL_FFT_ZT, 1, [&] { launch_fft_tiled(c->fa, 1, c->st); });
+        do_fourier_head(c);
         run_kernel(c, LGF_KERNEL_FFT_XY_INV_G, 1, [&] { launch_fft_tiled_inv_g(c->fa, c->gbuf, alpha, c->gmap, 0, c->st); });
         run_kernel(c, LGF_KERNEL_UPDATE_MEASURE, 1,
                    [&] { launch_update_measure(c->sa, lin, lout, c->gbuf, 1, c->w_buf[c->wcur], alpha, eps, c->st); });
@@ -438,7 +452,7 @@ int lgf_set_option(lgf_ctx *ctx, int key, int64_t value)
 {
     if (!ctx) return LGF_ERR_INVALID_ARG;
     const bool layout_key = (key == LGF_OPT_RECON || key == LGF_OPT_FFT_BATCH || key == LGF_OPT_FFT_PATH || key == LGF_OPT_FUSION ||
-                             key == LGF_OPT_L2_PERSIST || key == LGF_OPT_ACCUM_G || key == LGF_OPT_ZBLOCK);
+                             key == LGF_OPT_L2_PERSIST || key == LGF_OPT_ACCUM_G || key == LGF_OPT_ZBLOCK || key == LGF_OPT_FFT_PASSES);
     if (layout_key && ctx->bound) return fail(ctx, LGF_ERR_INVALID_ARG, "this option must be set before lgf_bind");
     switch (key) {
     case LGF_OPT_RECON:
@@ -474,6 +488,9 @@ int lgf_set_option(lgf_ctx *ctx, int key, int64_t value)
     case LGF_OPT_ZBLOCK:
         if (value < 0 || (value > 0 && ctx->N[2] % value != 0)) return fail(ctx, LGF_ERR_INVALID_ARG, "ZBLOCK must be 0 (auto) or a divisor of Nz");
         ctx->zblock = (int)value; break;
+    case LGF_OPT_FFT_PASSES:
+        if (value != 3 && value != 4 && value != 8) return fail(ctx, LGF_ERR_INVALID_ARG, "FFT_PASSES must be 3, 4 or 8");
+        ctx->fft_passes = (int)value; break;
     case LGF_OPT_ZT_PIPE:
         if (value != 0 && value != 1) return fail(ctx, LGF_ERR_INVALID_ARG, "ZT_PIPE must be 0 or 1");
         ctx->zt_pipe = (int)value; ctx->fa.zt_pipe = ctx->zt_pipe; graph_drop(ctx); break;
@@ -499,6 +516,10 @@ int lgf_bind(lgf_ctx *ctx, void *dev_workspace, size_t bytes, void *cuda_stream)
     if (((uintptr_t)dev_workspace) & 255) return fail(ctx, LGF_ERR_INVALID_ARG, "dev_workspace must be 256-byte aligned");
     if (ctx->accum && !(ctx->fusion && ctx->pack == 4 && ctx->fft_path == 0 && fft_tiled_gbuf_supported(ctx->N, ctx->prec)))
         return fail(ctx, LGF_ERR_INVALID_ARG, "ACCUM_G needs FUSION = 1, FFT_BATCH = 4 and a lattice the tiled FFT covers");
+    if (ctx->fft_passes != 3 && !(ctx->fft_path == 0 && fft_tiled_passes_supported(ctx->N, ctx->prec, ctx->fft_passes)))
+        return fail(ctx, LGF_ERR_INVALID_ARG, "FFT_PASSES = 4 / 8 need a lattice the tiled FFT covers (4: a square or 32 x n (z,t) tile)");
+    if (ctx->fft_passes == 8 && ctx->accum)
+        return fail(ctx, LGF_ERR_INVALID_ARG, "ACCUM_G builds g in the last 2D pass: not available with FFT_PASSES = 8");
     const Layout L = make_layout(ctx);
     if (bytes < L.total) return fail(ctx, LGF_ERR_WORKSPACE_TOO_SMALL, "workspace smaller than lgf_workspace_bytes()");
     ctx->lay = L;
@@ -547,7 +568,7 @@ int lgf_bind(lgf_ctx *ctx, void *dev_workspace, size_t bytes, void *cuda_stream)
         cudaError_t e = cudaGetLastError();
         return cuda_fail(ctx, e, "fft_tiled_setup");
     }
-    ctx->use_gbuf = ctx->fusion && ctx->tiled && ctx->pack == 4 && fft_tiled_gbuf_supported(ctx->N, ctx->prec);
+    ctx->use_gbuf = ctx->fusion && ctx->tiled && ctx->pack == 4 && ctx->fft_passes != 8 && fft_tiled_gbuf_supported(ctx->N, ctx->prec);
     l2_window_clear(ctx);
     if (ctx->use_gbuf) l2_window_set(ctx);   // one field buffer, used in place by every pass
     graph_drop(ctx);

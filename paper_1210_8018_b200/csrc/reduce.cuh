@@ -3,6 +3,10 @@
 #pragma once
 #include "common.cuh"
 
+#ifndef LGF_REDUCE_UNROLL
+#define LGF_REDUCE_UNROLL 8   /* 1: the plain loop (same sums; tuning A/B, profiles/r02_link_kernel.md) */
+#endif
+
 namespace lgf {
 
 __device__ __forceinline__ double warp_sum(double v)
@@ -51,10 +55,23 @@ __device__ __forceinline__ void finish_measure(double trF, double th, int64_t V,
     __syncthreads();
     if (!last) return;
     __threadfence();
+    // One CTA adds gridDim.x pairs while the rest of the GPU idles (8192 pairs at 32^4, 131072 at 64^4), so the
+    // loads are issued eight at a time per thread, as 16-byte pairs; the additions keep the index order
+    // i, i + THREADS, i + 2 THREADS, ... of each thread, i.e. the result is bitwise that of the plain loop.
     double f = 0, t = 0;
-    for (unsigned i = threadIdx.x; i < gridDim.x; i += THREADS) {
-        f += __ldcg(partials + 2 * (int64_t)i);
-        t += __ldcg(partials + 2 * (int64_t)i + 1);
+    const double2 *pp = (const double2 *)partials;
+    constexpr int UNR = LGF_REDUCE_UNROLL;
+    unsigned i = threadIdx.x;
+    for (; i + (UNR - 1) * THREADS < gridDim.x; i += UNR * THREADS) {
+        double2 v[UNR];
+#pragma unroll
+        for (int u = 0; u < UNR; u++) v[u] = __ldcg(pp + i + u * THREADS);
+#pragma unroll
+        for (int u = 0; u < UNR; u++) { f += v[u].x; t += v[u].y; }
+    }
+    for (; i < gridDim.x; i += THREADS) {
+        const double2 v = __ldcg(pp + i);
+        f += v.x; t += v.y;
     }
     block_sum2<THREADS>(f, t);
     if (threadIdx.x == 0) {

@@ -24,6 +24,18 @@ __device__ __forceinline__ void load_link(const cx<T> *__restrict__ links, int64
     if (NE == 6) su3_row2(u);
 }
 
+// The same through plain (coherent) loads, for the kernels that rewrite the link buffer in place (k_update,
+// k_apply_g): ld.global.nc promises that the data is read-only for the whole kernel, which an in-place
+// update does not honour even though every thread reads its own links before it writes them.
+template <typename T, int NE>
+__device__ __forceinline__ void load_link_rw(const cx<T> *links, int64_t V, int mu, int64_t s, cx<T> (&u)[9])
+{
+    const cx<T> *p = links + (int64_t)mu * NE * V + s;
+#pragma unroll
+    for (int k = 0; k < NE; k++) u[k] = p[(int64_t)k * V];
+    if (NE == 6) su3_row2(u);
+}
+
 template <typename T> __device__ __forceinline__ T rsqrt_t(T x);
 template <> __device__ __forceinline__ double rsqrt_t<double>(double x) { return rsqrt(x); }
 template <> __device__ __forceinline__ float rsqrt_t<float>(float x) { return rsqrtf(x); }

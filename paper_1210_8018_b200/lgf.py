@@ -20,7 +20,7 @@ ERR_WORKSPACE_TOO_SMALL, ERR_CUDA, ERR_NOT_CONVERGED, ERR_NUMERIC = -5, -6, -7, 
 PREC_FP64, PREC_FP32 = 0, 1
 LAYOUT_AOS, LAYOUT_AOS12 = 0, 1
 OPT_RECON, OPT_FFT_BATCH, OPT_MAX_ITER, OPT_CHECK_INTERVAL, OPT_FFT_PATH, OPT_PROFILE, OPT_FUSION, OPT_L2_PERSIST = 1, 2, 3, 4, 5, 6, 7, 8
-OPT_GMAP, OPT_ACCUM_G, OPT_GRAPH, OPT_ZBLOCK, OPT_ZT_PIPE = 9, 10, 11, 12, 13
+OPT_GMAP, OPT_ACCUM_G, OPT_GRAPH, OPT_ZBLOCK, OPT_ZT_PIPE, OPT_FFT_PASSES = 9, 10, 11, 12, 13, 14
 GMAP_FIRST_ORDER, GMAP_EXP = 0, 1
 FIELD_DELTA, FIELD_W, FIELD_G = 0, 1, 2
 STAGE_MEASURE, STAGE_FOURIER, STAGE_UPDATE = 0, 1, 2
@@ -115,7 +115,7 @@ class GaugeFixer:
 
     def __init__(self, N, precision="fp64", recon=18, fft_batch=4, fft_path=0, device="cuda:0",
                  stream=None, max_iter=None, check_interval=None, profile=False, fusion=None, l2_persist=None, gmap=None,
-                 accum_g=None, graph=None, zblock=None, zt_pipe=None):
+                 accum_g=None, graph=None, zblock=None, zt_pipe=None, fft_passes=None):
         import torch
 
         self.torch = torch
@@ -146,6 +146,8 @@ class GaugeFixer:
             self.set_option(OPT_ZBLOCK, zblock)
         if zt_pipe is not None:
             self.set_option(OPT_ZT_PIPE, zt_pipe)
+        if fft_passes is not None:
+            self.set_option(OPT_FFT_PASSES, fft_passes)
         if max_iter is not None:
             self.set_option(OPT_MAX_ITER, max_iter)
         if check_interval is not None:

@@ -417,3 +417,55 @@ def test_zt_pipe_full_size_32(lgf):
         res.append((r.F, r.theta, gf.get_links()))
         gf.close()
     assert res[0][0] == res[1][0] and res[0][1] == res[1][1] and np.array_equal(res[0][2], res[1][2])
+
+
+# ------------------------------------------------------------------ LGF_OPT_FFT_PASSES: 2D + 2D and 4 x 1D structures
+PASS_LATTICES = [((8, 8, 8, 8), 501), ((12, 12, 12, 12), 502), ((16, 16, 16, 16), 503), ((8, 8, 32, 16), 504),
+                 ((8, 8, 64, 64), 505), ((48, 48, 8, 8), 506), ((16, 16, 16, 32), 507), ((8, 8, 24, 48), 508)]
+
+
+@pytest.mark.parametrize("lat", PASS_LATTICES, ids=lambda v: "x".join(map(str, v[0])))
+@pytest.mark.parametrize("passes", [4, 8])
+def test_fft_pass_structures_match_oracle(lgf, lat, passes):
+    """The 2D + 2D four-pass and the 4 x 1D eight-pass structures give the oracle's w
+    (Alg. 1 lines 3-8) and the oracle's links after an iteration, FP64 and FP32, 4 and 9 fields."""
+    N, seed = lat
+    square_or_32xn = N[2] == N[3] or N[2] == 32
+    U = gen.gen_links(N, 0.5, seed)
+    D, _, _ = oracle.measure(N, U)
+    w = oracle.fourier_accelerate(N, D)
+    Uo = U.copy()
+    hist = oracle.iterate(N, Uo, ALPHA, 1)
+    if passes == 4 and not square_or_32xn:
+        with pytest.raises(lgf.LgfError):
+            lgf.GaugeFixer(N, fft_passes=4)          # the two-launch (z,t) pass is not instantiated for this tile
+        return
+    for prec, fb, tolw, tolu in (("fp64", 4, 2e-13, 1e-12), ("fp64", 9, 2e-13, 1e-12), ("fp32", 4, 2e-5, 1e-5)):
+        cdt = np.complex128 if prec == "fp64" else np.complex64
+        gf = lgf.GaugeFixer(N, precision=prec, fft_batch=fb, fft_passes=passes, recon=12 if fb == 4 else 18)
+        assert gf.uses_tiled_fft() and gf.uses_gbuf() == (passes == 4 and fb == 4)
+        gf.load_links(U.astype(cdt))
+        gf.set_field(lgf.FIELD_DELTA, D.astype(cdt))
+        gf.stage(lgf.STAGE_FOURIER)
+        w2 = gf.get_field(lgf.FIELD_W).astype(np.complex128)
+        assert np.abs(w2 - w).max() < tolw * np.abs(w).max()
+        gf.load_links(U.astype(cdt))
+        gf.reset_counters()
+        r = gf.iterate(ALPHA, 1)
+        kt = gf.kernel_times()
+        nfft = sum(v[1] for k, v in kt.items() if k.startswith("fft_"))
+        assert nfft == passes
+        assert np.abs(gf.get_links().astype(np.complex128) - Uo).max() < tolu
+        assert abs(r.theta - hist[1, 1]) <= (1e-10 if prec == "fp64" else 1e-4) * hist[1, 1]
+        gf.close()
+
+
+def test_fft_passes_validation(lgf):
+    with pytest.raises(lgf.LgfError):
+        lgf.GaugeFixer(8, fft_passes=5)
+    with pytest.raises(lgf.LgfError):
+        lgf.GaugeFixer((4, 6, 8, 12), fft_passes=8)            # not a tiled lattice
+    with pytest.raises(lgf.LgfError):
+        lgf.GaugeFixer(8, fft_passes=8, accum_g=1)
+    gf = lgf.GaugeFixer(8, fft_passes=4, accum_g=1)           # 2D + 2D keeps the g-building last pass
+    gf.close()
