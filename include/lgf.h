@@ -130,7 +130,7 @@ enum {
                                    the next tile with asynchronous copies (cp.async) while the current one is
                                    finished; 0: one tile per thread group, loaded straight into registers.  Same
                                    arithmetic in the same order: bitwise the same w.  Any time. */
-    LGF_OPT_FFT_PASSES = 14     /* pass structure of the tiled 4D FFT, the axis of the paper's comparison of 4 x 1D,
+    LGF_OPT_FFT_PASSES = 14,    /* pass structure of the tiled 4D FFT, the axis of the paper's comparison of 4 x 1D,
                                    2D + 2D and 3D + 1D decompositions.  3 (default): (x,y) forward |
                                    (z,t) forward, mask, (z,t) inverse in one tile visit | (x,y) inverse.  4: 2D + 2D
                                    as the paper runs it, (x,y) forward | (z,t) forward and mask | (z,t) inverse |
@@ -139,6 +139,47 @@ enum {
                                    kernel; not with ACCUM_G).  Same w to rounding; timing comparison only
                                    (bench_sweep.py --passes).  lgf_bind fails with LGF_ERR_INVALID_ARG where a structure
                                    is not available.  Before lgf_bind. */
+    LGF_OPT_SHARD_WORLD = 15,   /* R > 0: this context holds ONE t-slab of a lattice sharded over R GPUs (the B200
+                                   analogue of the paper's distributed CPU program):
+                                   lgf_create was given the extents of the WHOLE lattice, the context stores the
+                                   Nt / R time slices of rank SHARD_RANK between one halo slice below and one
+                                   above, and lgf_load_links / lgf_get_links move those Nt / R slices
+                                   ([Nx Ny Nz Nt/R] sites, same interchange layouts).  R must divide Nt and Ny.
+                                   The iteration is then driven step by step with lgf_shard_step, the exchanges
+                                   between the steps (all-to-all transposes of the packed field around the (z,t)
+                                   pass, one-slice halos of g and of the t-links, the all-reduce of F and theta)
+                                   being the caller's (paper_1210_8018_b200/sharded.py: torch.distributed over NCCL).
+                                   R = 1 is valid (the exchanges are with itself).  Default path only (FUSION = 1,
+                                   FFT_BATCH = 4, FFT_PASSES = 3, no ACCUM_G, tiled FFT).  0 (default): off.
+                                   Before lgf_bind. */
+    LGF_OPT_SHARD_RANK = 16     /* which slab, 0 <= rank < SHARD_WORLD: time slices [rank Nt/R, (rank+1) Nt/R).
+                                   Set after SHARD_WORLD, before lgf_bind. */
+};
+
+/* lgf_shard_step selectors: the kernels of one iteration of a sharded lattice, in the order of a step
+ * (exchanges the caller performs are in brackets):
+ *   start:      [halo of the t-links]  MEASURE  [all-reduce F, theta]  RESET
+ *   iteration:  XY_FWD  PACK  [all-to-all send -> recv]  ZT  [all-to-all recv -> send]  UNPACK  XY_INV_G
+ *               [halos of g]  LINK  [halo of the new t-links]  [all-reduce F, theta]  FINISH */
+enum {
+    LGF_SHARD_MEASURE = 0,   /* kernel (a) on the slab: Delta, and this rank's part of F and theta */
+    LGF_SHARD_RESET = 1,     /* after the all-reduce: iteration counter 0, history[0], done = (theta <= eps) */
+    LGF_SHARD_XY_FWD = 2,    /* (x,y) forward pass of the FFT on the slab */
+    LGF_SHARD_PACK = 3,      /* field -> send buffer, one contiguous block per destination rank */
+    LGF_SHARD_ZT = 4,        /* (z,t) forward, mask, (z,t) inverse on the receive buffer (all t, this rank's rows of y) */
+    LGF_SHARD_UNPACK = 5,    /* send buffer (after the return all-to-all) -> field */
+    LGF_SHARD_XY_INV_G = 6,  /* (x,y) inverse pass and g(x) (uses alpha) */
+    LGF_SHARD_LINK = 7,      /* fused link update + measure of the new links (uses alpha): this rank's part of F, theta */
+    LGF_SHARD_FINISH = 8     /* after the all-reduce: history entry, done = (theta <= eps) */
+};
+/* lgf_shard_region selectors: byte ranges of the bound workspace that the caller exchanges */
+enum {
+    LGF_REGION_CTRL = 0,     /* two doubles: F, theta (all-reduce, sum) */
+    LGF_REGION_XSEND = 1,    /* send buffer of the transposes: SHARD_WORLD equal contiguous blocks */
+    LGF_REGION_XRECV = 2,    /* receive buffer */
+    LGF_REGION_G = 3,        /* rows 0, 1 of g: 6 complex arrays of `stored sites` each, time slice t at t * slice sites */
+    LGF_REGION_LINKS = 4     /* the CURRENT link buffer (changes with every LINK step): 4 x NE complex arrays of
+                                `stored sites` each, array (mu * NE + k), own slices at t = 1..Nt/R, halos at 0 and Nt/R + 1 */
 };
 
 /* lgf_get_field / lgf_set_field selectors */
@@ -252,6 +293,18 @@ int lgf_zblock(const lgf_ctx *ctx);
  * (two launches on the bound stream, asynchronous; the calls that read the links do this
  * themselves).  No-op, LGF_OK, when nothing is pending or ACCUM_G is off.  Needs loaded links. */
 int lgf_sync_links(lgf_ctx *ctx);
+
+/* Sharded lattice (LGF_OPT_SHARD_WORLD): run one kernel step of the iteration on this rank's slab, asynchronously on the
+ * bound stream (alpha is used by XY_INV_G and LINK, eps by RESET and FINISH).  The exchanges between the steps are the
+ * caller's; see the LGF_SHARD_* list for the order.  LGF_ERR_INVALID_ARG on an unsharded context. */
+int lgf_shard_step(lgf_ctx *ctx, int step, double alpha, double eps);
+/* Byte range (offset from the bound workspace pointer, length) of an exchanged region; host out pointers. */
+int lgf_shard_region(const lgf_ctx *ctx, int region, size_t *offset, size_t *bytes);
+/* info[0..7] (host): stored sites per array, sites per time slice, own time slices, complex arrays per link direction,
+ * bytes per complex number, SHARD_WORLD, SHARD_RANK, sites of the interchange arrays of this rank.  n >= 8. */
+int lgf_shard_info(const lgf_ctx *ctx, int64_t *info, int n);
+/* (iterations, F, theta, converged) as the device holds them after the last RESET / FINISH.  Synchronises. */
+int lgf_shard_result(lgf_ctx *ctx, lgf_result *out);
 
 /* Debug entry point, not on the gauge-fixing path: the measured FP64 fused-multiply-add rate of the
  * current device (DFMA per second, best of 4 timed launches of a register-only FMA kernel on the given

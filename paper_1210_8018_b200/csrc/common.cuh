@@ -86,6 +86,12 @@ struct Geom {
     int64_t V;       // sites
     int64_t st[4];   // site-index stride of each direction: 1, Nx, Nx*Ny, Nx*Ny*Nz
     int zb;          // z-block of the site walk (divides Nz; Nz = plain lexicographic order), see walk_site
+    // One lattice sharded over several GPUs in t-slabs (LGF_OPT_SHARD_WORLD): the arrays of a
+    // rank hold its Ntw time slices between one halo slice below and one above, N[3] = Ntw + 2, t0 = 1, so the
+    // t-neighbours of a walked site never wrap; the per-site kernels walk the Vw interior sites only and
+    // normalise F and theta by the Vg sites of the whole lattice.  Unsharded: Vw = Vg = V, Ntw = N[3], t0 = 0.
+    int64_t Vw, Vg;
+    int Ntw, t0;
 };
 
 __device__ __forceinline__ void site_coords(const Geom &g, int64_t s, int c[4])
@@ -107,7 +113,7 @@ __device__ __forceinline__ void site_coords(const Geom &g, int64_t s, int c[4])
 // U_nu(x-nu), g(x-nu), g(x+mu) (Alg. 1 lines 12-16) are L2 hits even when one time
 // slice of links is larger than L2 (64^4: 151 MB per slice).  Only the first
 // plane of a z-block misses its -z neighbours (1/zb of the sites).  zb = Nz is the lexicographic order.
-// Returns the site index and fills c[0..3]; valid for r < V.
+// Returns the site index and fills c[0..3]; valid for r < Vw.
 __device__ __forceinline__ int64_t walk_site(const Geom &g, int64_t r, int c[4])
 {
     const unsigned P = (unsigned)(g.N[0] * g.N[1]);
@@ -115,9 +121,9 @@ __device__ __forceinline__ int64_t walk_site(const Geom &g, int64_t r, int c[4])
     const unsigned o = u % P, q = u / P;
     c[0] = (int)(o % (unsigned)g.N[0]);
     c[1] = (int)(o / (unsigned)g.N[0]);
-    const unsigned per = (unsigned)(g.zb * g.N[3]);
+    const unsigned per = (unsigned)(g.zb * g.Ntw);
     const unsigned zblk = q / per, rem = q % per;
-    c[3] = (int)(rem / (unsigned)g.zb);
+    c[3] = (int)(rem / (unsigned)g.zb) + g.t0;
     c[2] = (int)(zblk * (unsigned)g.zb + rem % (unsigned)g.zb);
     return (int64_t)o + (int64_t)P * (c[2] + g.N[2] * c[3]);
 }

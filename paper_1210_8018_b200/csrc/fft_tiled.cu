@@ -425,7 +425,7 @@ template <typename T, int N> static int launch_axis_n(const FftArgs &a, int axis
     constexpr int S = split_of(N, split_min<T>(N, N));
     const int64_t nlines = (int64_t)a.nfields * a.geo.V / N;
     const unsigned grid = (unsigned)((nlines + 256 / S - 1) / (256 / S));
-    const double c = a.pmax2 / (double)a.geo.V;
+    const double c = a.pmax2 / a.vnorm;
     if (sign < 0 && mask) k_fft_axis<T, N, S, -1, true><<<grid, 256, 0, st>>>((cx<T> *)a.w, a.geo, axis, nlines, a.ptab, c, a.ctrl);
     else if (sign < 0) k_fft_axis<T, N, S, -1, false><<<grid, 256, 0, st>>>((cx<T> *)a.w, a.geo, axis, nlines, a.ptab, c, a.ctrl);
     else k_fft_axis<T, N, S, +1, false><<<grid, 256, 0, st>>>((cx<T> *)a.w, a.geo, axis, nlines, a.ptab, c, a.ctrl);

@@ -331,8 +331,8 @@ template <typename T, int NA, int NB> int launch_zt_half_n(const FftArgs &a, int
         typedef ZTCfg<T, NA, NB, C> Z;
         const int64_t ntiles = (int64_t)a.nfields * a.geo.N[1] * (a.geo.N[0] / C);
         const unsigned grid = (unsigned)((ntiles + Z::G - 1) / Z::G);
-        if (inverse) k_fft_zt_half<T, NA, NB, C, 1><<<grid, Z::CTA, Z::SMEM, st>>>((cx<T> *)a.w, a.geo, a.ptab, a.pmax2 / (double)a.geo.V, ntiles, a.ctrl);
-        else k_fft_zt_half<T, NA, NB, C, 0><<<grid, Z::CTA, Z::SMEM, st>>>((cx<T> *)a.w, a.geo, a.ptab, a.pmax2 / (double)a.geo.V, ntiles, a.ctrl);
+        if (inverse) k_fft_zt_half<T, NA, NB, C, 1><<<grid, Z::CTA, Z::SMEM, st>>>((cx<T> *)a.w, a.geo, a.ptab, a.pmax2 / a.vnorm, ntiles, a.ctrl);
+        else k_fft_zt_half<T, NA, NB, C, 0><<<grid, Z::CTA, Z::SMEM, st>>>((cx<T> *)a.w, a.geo, a.ptab, a.pmax2 / a.vnorm, ntiles, a.ctrl);
         return 0;
     }
     return 1;
@@ -360,10 +360,10 @@ template <typename T, int NA, int NB> int launch_zt_n(const FftArgs &a, cudaStre
     if constexpr (zt_pipe_pair(NA, NB)) if (a.zt_pipe) {
         // persistent: as many CTAs as are resident at once, each walks tiles blockIdx, blockIdx + grid, ...
         const unsigned resident = (unsigned)(sm_count() * Z::MINB);
-        k_fft_zt_pipe<T, NA, NB, C><<<grid < resident ? grid : resident, Z::CTA, Z::SMEM, st>>>((cx<T> *)a.w, a.geo, a.ptab, a.pmax2 / (double)a.geo.V, ntiles, a.ctrl);
+        k_fft_zt_pipe<T, NA, NB, C><<<grid < resident ? grid : resident, Z::CTA, Z::SMEM, st>>>((cx<T> *)a.w, a.geo, a.ptab, a.pmax2 / a.vnorm, ntiles, a.ctrl);
         return 0;
     }
-    k_fft_zt<T, NA, NB, C><<<grid, Z::CTA, Z::SMEM, st>>>((cx<T> *)a.w, a.geo, a.ptab, a.pmax2 / (double)a.geo.V, ntiles, a.ctrl);
+    k_fft_zt<T, NA, NB, C><<<grid, Z::CTA, Z::SMEM, st>>>((cx<T> *)a.w, a.geo, a.ptab, a.pmax2 / a.vnorm, ntiles, a.ctrl);
     return 0;
 }
 

@@ -168,7 +168,7 @@ k_update_measure(const cx<T> *__restrict__ lin, cx<T> *__restrict__ lout, const 
     const int64_t V = geo.V;
     const int64_t rr = (int64_t)blockIdx.x * FUSED_THREADS + threadIdx.x;
     double trF = 0, th = 0;
-    if (rr < V) {
+    if (rr < geo.Vw) {
         int c[4];
         const int64_t s = walk_site(geo, rr, c);     // (z,t)-blocked walk: neighbour re-reads stay in L2
         if (!STORE && LGF_ACC_QSUM(NE)) {
@@ -285,7 +285,7 @@ k_update_measure(const cx<T> *__restrict__ lin, cx<T> *__restrict__ lout, const 
             th = store_delta<T, PACK>(di, E, wout, V, s);
         }
     }
-    finish_measure<FUSED_THREADS>(trF, th, V, ctrl, partials, hist, eps, 1);
+    finish_measure<FUSED_THREADS>(trF, th, geo.Vg, ctrl, partials, hist, eps, 1);
 }
 
 int fused_blocks(int64_t V) { return (int)((V + FUSED_THREADS - 1) / FUSED_THREADS); }
@@ -310,7 +310,7 @@ template <typename T, int NE, int PACK, bool GBUF, bool STORE> static void prefe
 void launch_update_measure(const SiteArgs &a, const void *lin, void *lout, const void *gsrc, int gbuf, void *wout,
                            double alpha, double eps, cudaStream_t st)
 {
-    const int nb = fused_blocks(a.geo.V);
+    const int nb = fused_blocks(a.geo.Vw);
 #define CALL(T, NE, PACK, GB) \
     do { prefer_l1<T, NE, PACK, GB, true>();   \
     k_update_measure<T, NE, PACK, GB, true><<<nb, FUSED_THREADS, 0, st>>>((const cx<T> *)lin, (cx<T> *)lout, (const cx<T> *)gsrc, \
@@ -329,7 +329,7 @@ void launch_update_measure(const SiteArgs &a, const void *lin, void *lout, const
 
 void launch_measure_acc(const SiteArgs &a, const void *gacc, double eps, cudaStream_t st)
 {
-    const int nb = fused_blocks(a.geo.V);
+    const int nb = fused_blocks(a.geo.Vw);
 #define CALL(T, NE) \
     do { prefer_l1<T, NE, 4, true, false>();  \
     k_update_measure<T, NE, 4, true, false><<<nb, FUSED_THREADS, 0, st>>>((const cx<T> *)a.links, (cx<T> *)nullptr, \

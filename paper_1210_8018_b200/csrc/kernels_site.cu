@@ -27,7 +27,7 @@ k_measure(const cx<T> *__restrict__ links, cx<T> *__restrict__ w, Geom geo, Ctrl
     const int64_t V = geo.V;
     const int64_t rr = (int64_t)blockIdx.x * SITE_THREADS + threadIdx.x;
     double trF = 0, th = 0;
-    if (rr < V) {
+    if (rr < geo.Vw) {
         int c[4];
         const int64_t s = walk_site(geo, rr, c);
         cx<T> A[9];
@@ -68,7 +68,7 @@ k_measure(const cx<T> *__restrict__ links, cx<T> *__restrict__ w, Geom geo, Ctrl
             w[8 * V + s] = mk<T>(0, d2);
         }
     }
-    finish_measure<SITE_THREADS>(trF, th, V, ctrl, partials, hist, eps, count_iter);
+    finish_measure<SITE_THREADS>(trF, th, geo.Vg, ctrl, partials, hist, eps, count_iter);
 }
 
 __global__ void k_ctrl_reset(Ctrl *ctrl, double2 *hist, double eps)
@@ -90,7 +90,7 @@ k_update(cx<T> *links, const cx<T> *__restrict__ w, Geom geo, T a, int gexp, con
     if (*(volatile const int *)&ctrl->done) return;
     const int64_t V = geo.V;
     const int64_t rr = (int64_t)blockIdx.x * SITE_THREADS + threadIdx.x;
-    if (rr >= V) return;
+    if (rr >= geo.Vw) return;
     int c[4];
     const int64_t s = walk_site(geo, rr, c);
     cx<T> g0[9];
@@ -121,7 +121,7 @@ k_apply_g(cx<T> *links, const cx<T> *__restrict__ gacc, Geom geo)
 {
     const int64_t V = geo.V;
     const int64_t rr = (int64_t)blockIdx.x * SITE_THREADS + threadIdx.x;
-    if (rr >= V) return;
+    if (rr >= geo.Vw) return;
     int c[4];
     const int64_t s = walk_site(geo, rr, c);
     cx<T> g0[9];
@@ -149,6 +149,43 @@ template <typename T> __global__ void k_g_identity(cx<T> *__restrict__ gacc, int
     if (s >= V) return;
 #pragma unroll
     for (int k = 0; k < 6; k++) gacc[(int64_t)k * V + s] = mk<T>((k == 0 || k == 4) ? (T)1 : (T)0, (T)0);
+}
+
+// ------------------------------------------------------------------ one lattice sharded in t-slabs
+// Transposes around the (z,t) pass (the all-to-all of a distributed FFT, as PFFT does for the paper's CPU
+// program).  A rank holds Ntl time slices of every field; for the (z,t) pass it needs
+// ALL time slices of the sites with y in its range of Ny/world rows.  Pack: the interior slices of the 4 packed
+// fields -> the send buffer, ordered [destination q][t_local][field][z][y - q Nyl][x], so that the block for q
+// is contiguous; after the all-to-all the receive buffer reads [source r][t_local][field][z][y_local][x] =
+// [t][field][z][y_local][x], which is the array the (z,t) kernel runs on (field stride Nx Nyl Nz, t stride 4 times
+// that).  Unpack is the same map backwards after the return all-to-all.  Consecutive threads: consecutive x.
+template <typename T, int UNPACK>
+__global__ void k_slab_pack(cx<T> *__restrict__ w, cx<T> *__restrict__ xbuf, Geom geo, int world)
+{
+    const int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (e >= 4 * geo.Vw) return;
+    const int Nx = geo.N[0], Ny = geo.N[1], Nz = geo.N[2], Ntl = geo.Ntw, Nyl = Ny / world;
+    unsigned u = (unsigned)e;
+    const int x = (int)(u % (unsigned)Nx); u /= (unsigned)Nx;
+    const int y = (int)(u % (unsigned)Ny); u /= (unsigned)Ny;
+    const int z = (int)(u % (unsigned)Nz); u /= (unsigned)Nz;
+    const int tl = (int)(u % (unsigned)Ntl); u /= (unsigned)Ntl;
+    const int f = (int)u;
+    const int q = y / Nyl, yl = y % Nyl;
+    const int64_t iw = (int64_t)f * geo.V + x + (int64_t)Nx * y + geo.st[2] * z + geo.st[3] * (tl + geo.t0);
+    const int64_t ix = ((((int64_t)q * Ntl + tl) * 4 + f) * Nz + z) * ((int64_t)Nyl * Nx) + (int64_t)yl * Nx + x;
+    if (UNPACK) w[iw] = xbuf[ix]; else xbuf[ix] = w[iw];
+}
+
+// (F, theta) in the control block are the sums over all ranks now: history entry of the current iteration
+// and the stop decision of Alg. 1 line 2, the same on every rank.
+__global__ void k_slab_finish(Ctrl *ctrl, double2 *hist, double eps)
+{
+    const double F = ctrl->F, theta = ctrl->theta;
+    const long long it = ctrl->iter;
+    if (it < LGF_HIST_CAP) hist[it] = make_double2(F, theta);
+    if (!(theta == theta) || theta > 1.0e300) ctrl->done = 2;
+    else if (theta <= eps) ctrl->done = 1;
 }
 
 // ------------------------------------------------------------------ layout conversions and taps
@@ -241,7 +278,7 @@ int measure_blocks(int64_t V) { return (int)((V + SITE_THREADS - 1) / SITE_THREA
 
 void launch_measure(const SiteArgs &a, double eps, int count_iter, cudaStream_t st)
 {
-    const int nb = measure_blocks(a.geo.V);
+    const int nb = measure_blocks(a.geo.Vw);
 #define CALL(T, NE, PACK) \
     k_measure<T, NE, PACK><<<nb, SITE_THREADS, 0, st>>>((const cx<T> *)a.links, (cx<T> *)a.w, a.geo, a.ctrl, a.partials, a.hist, eps, count_iter)
     LGF_DISPATCH(CALL);
@@ -250,7 +287,7 @@ void launch_measure(const SiteArgs &a, double eps, int count_iter, cudaStream_t 
 
 void launch_update(const SiteArgs &a, double alpha, cudaStream_t st)
 {
-    const int nb = measure_blocks(a.geo.V);
+    const int nb = measure_blocks(a.geo.Vw);
 #define CALL(T, NE, PACK) \
     k_update<T, NE, PACK><<<nb, SITE_THREADS, 0, st>>>((cx<T> *)a.links, (const cx<T> *)a.w, a.geo, (T)(alpha / 2.0), a.gexp, a.ctrl)
     LGF_DISPATCH(CALL);
@@ -259,7 +296,7 @@ void launch_update(const SiteArgs &a, double alpha, cudaStream_t st)
 
 void launch_apply_g(const SiteArgs &a, const void *gacc, cudaStream_t st)
 {
-    const int nb = measure_blocks(a.geo.V);
+    const int nb = measure_blocks(a.geo.Vw);
 #define CALL(T, NE, PACK) \
     k_apply_g<T, NE><<<nb, SITE_THREADS, 0, st>>>((cx<T> *)a.links, (const cx<T> *)gacc, a.geo)
     LGF_DISPATCH(CALL);
@@ -273,6 +310,23 @@ void launch_g_identity(const SiteArgs &a, void *gacc, cudaStream_t st)
     else k_g_identity<float><<<nb, 256, 0, st>>>((cx<float> *)gacc, a.geo.V);
 }
 
+void launch_slab_pack(const SiteArgs &a, void *xbuf, int world, int unpack, cudaStream_t st)
+{
+    const int nb = (int)((4 * a.geo.Vw + 255) / 256);
+    if (a.prec == 0) {
+        if (unpack) k_slab_pack<double, 1><<<nb, 256, 0, st>>>((cx<double> *)a.w, (cx<double> *)xbuf, a.geo, world);
+        else k_slab_pack<double, 0><<<nb, 256, 0, st>>>((cx<double> *)a.w, (cx<double> *)xbuf, a.geo, world);
+    } else {
+        if (unpack) k_slab_pack<float, 1><<<nb, 256, 0, st>>>((cx<float> *)a.w, (cx<float> *)xbuf, a.geo, world);
+        else k_slab_pack<float, 0><<<nb, 256, 0, st>>>((cx<float> *)a.w, (cx<float> *)xbuf, a.geo, world);
+    }
+}
+
+void launch_slab_finish(const SiteArgs &a, double eps, cudaStream_t st)
+{
+    k_slab_finish<<<1, 1, 0, st>>>(a.ctrl, a.hist, eps);
+}
+
 void launch_ctrl_reset(const SiteArgs &a, double eps, cudaStream_t st)
 {
     k_ctrl_reset<<<1, 1, 0, st>>>(a.ctrl, a.hist, eps);
@@ -280,6 +334,7 @@ void launch_ctrl_reset(const SiteArgs &a, double eps, cudaStream_t st)
 
 void launch_aos_to_soa(const SiteArgs &a, const void *aos, int per_link, int64_t s0, int64_t count, cudaStream_t st)
 {
+    s0 += a.geo.t0 * a.geo.st[3];     // sharded lattice: the interchange arrays hold the interior slices only
     const int nb = (int)((count * 4 + 255) / 256);
 #define CALL(T, NE, PACK) \
     do { if (per_link == 6) k_aos_to_soa<T, NE, 6><<<nb, 256, 0, st>>>((const cx<T> *)aos, (cx<T> *)a.links, a.geo.V, s0, count); \
@@ -290,6 +345,7 @@ void launch_aos_to_soa(const SiteArgs &a, const void *aos, int per_link, int64_t
 
 void launch_soa_to_aos(const SiteArgs &a, void *aos, int per_link, int64_t s0, int64_t count, cudaStream_t st)
 {
+    s0 += a.geo.t0 * a.geo.st[3];     // sharded lattice: the interchange arrays hold the interior slices only
     const int nb = (int)((count * 4 + 255) / 256);
 #define CALL(T, NE, PACK) \
     do { if (per_link == 6) k_soa_to_aos<T, NE, 6><<<nb, 256, 0, st>>>((cx<T> *)aos, (const cx<T> *)a.links, a.geo.V, s0, count); \
@@ -300,6 +356,7 @@ void launch_soa_to_aos(const SiteArgs &a, void *aos, int per_link, int64_t s0, i
 
 void launch_field_get(const SiteArgs &a, int which, double alpha, void *aos, int64_t s0, int64_t count, cudaStream_t st)
 {
+    s0 += a.geo.t0 * a.geo.st[3];
     const int nb = (int)((count + 255) / 256);
 #define CALL(T, NE, PACK) \
     k_field_get<T, PACK><<<nb, 256, 0, st>>>((const cx<T> *)a.w, a.geo.V, which, (T)(alpha / 2.0), a.gexp, (cx<T> *)aos, s0, count)
@@ -309,6 +366,7 @@ void launch_field_get(const SiteArgs &a, int which, double alpha, void *aos, int
 
 void launch_field_set(const SiteArgs &a, const void *aos, int64_t s0, int64_t count, cudaStream_t st)
 {
+    s0 += a.geo.t0 * a.geo.st[3];
     const int nb = (int)((count + 255) / 256);
 #define CALL(T, NE, PACK) \
     k_field_set<T, PACK><<<nb, 256, 0, st>>>((cx<T> *)a.w, a.geo.V, (const cx<T> *)aos, s0, count)

@@ -44,6 +44,12 @@ void launch_soa_to_aos(const SiteArgs &a, void *aos, int per_link, int64_t s0, i
 void launch_field_get(const SiteArgs &a, int which, double alpha, void *aos, int64_t s0, int64_t count, cudaStream_t st);
 void launch_field_set(const SiteArgs &a, const void *aos, int64_t s0, int64_t count, cudaStream_t st);
 
+// ---- one lattice sharded in t-slabs (LGF_OPT_SHARD_WORLD): transposes around the (z,t) pass and the global stop decision
+// field buffer (4 packed fields, interior slices of the slab) <-> exchange buffer [dest rank q][t_local][field][z][y in q's range][x]
+void launch_slab_pack(const SiteArgs &a, void *xbuf, int world, int unpack, cudaStream_t st);
+// after the all-reduce of (F, theta): history entry of the current iteration, done = (theta <= eps) or 2 on NaN/Inf
+void launch_slab_finish(const SiteArgs &a, double eps, cudaStream_t st);
+
 // ---- Fourier acceleration (Alg. 1 lines 3-8): w <- F^-1 [p_max^2/(p^2 V)] F w, zero mode -> 0
 struct FftArgs {
     Geom geo;
@@ -55,6 +61,7 @@ struct FftArgs {
     const void *tw;     // device: cx<T> forward twiddles exp(-2 pi i k/N_mu), four tables back to back
     const Ctrl *ctrl;
     int zt_pipe;        // LGF_OPT_ZT_PIPE: (z,t) pass as the persistent kernel with cp.async prefetch
+    double vnorm;       // sites of the whole lattice: the 1/V of the inverse transform (Alg. 1 line 7)
 };
 // generic per-axis transform: any extent, O(N^2) per line.  Returns launches issued.
 int launch_fft_generic(const FftArgs &a, cudaStream_t st);

@@ -27,7 +27,7 @@ struct EvPair { cudaEvent_t a, b; int kind; };
 size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 
 struct Layout {
-    size_t links[2], w[2], gbuf, partials, ctrl, hist, ptab, tw, staging, total;
+    size_t links[2], w[2], gbuf, partials, ctrl, hist, ptab, tw, staging, xbuf[2], ptab_zt, total;
     int64_t staging_sites;
 };
 
@@ -42,6 +42,12 @@ struct lgf_ctx {
     int zblock = 0;          // LGF_OPT_ZBLOCK: 0 = auto (resolved by lgf_bind into sa.geo.zb)
     int zt_pipe = 0;         // LGF_OPT_ZT_PIPE
     int fft_passes = 3;      // LGF_OPT_FFT_PASSES: 3 (fused middle), 4 (2D + 2D), 8 (4 x 1D)
+    // one lattice sharded in t-slabs over shard_world ranks (0 = off): V = sites of the interchange arrays (the
+    // rank's own time slices), Vp = stored sites (with the two halo slices), Vg = sites of the whole lattice
+    int shard_world = 0, shard_rank = 0;
+    int64_t Vp = 0, Vg = 0;
+    void *xbuf[2] = {nullptr, nullptr};   // exchange buffers of the transposes (send, receive)
+    FftArgs fa_zt{};                      // the (z,t) pass on the transposed field
     cudaGraphExec_t gexec = nullptr;
     struct { double alpha, eps; int cur, wcur, gmap, unit; } gkey{};
     int64_t g_launches = 0, g_kcount[LGF_KERNEL_KINDS] = {0};
@@ -80,6 +86,10 @@ Layout make_layout(const lgf_ctx *c)
     const size_t e = elem_bytes(c);
     const int ne = c->recon == 12 ? 6 : 9;
     size_t off = 0;
+    // sharded: the arrays hold the rank's Nt / world time slices plus one halo slice on either side
+    const int64_t plane3 = (int64_t)c->N[0] * c->N[1] * c->N[2];
+    const int64_t Vl = c->shard_world > 0 ? plane3 * (c->N[3] / c->shard_world) : (int64_t)plane3 * c->N[3];
+    const int64_t Vs = c->shard_world > 0 ? Vl + 2 * plane3 : Vl;
     // fusion: links are double-buffered (the fused kernel reads old neighbours while new links
     // are written); the fields are double-buffered when g is rebuilt from w inside that kernel,
     // else the last FFT pass writes rows 0, 1 of g (6 complex per site) to gbuf
@@ -87,17 +97,19 @@ Layout make_layout(const lgf_ctx *c)
     const int nl = (c->fusion && !c->accum) ? 2 : 1;
     const bool gb = c->fusion && c->pack == 4 && c->fft_path == 0 && c->fft_passes != 8 && fft_tiled_gbuf_supported(c->N, c->prec);
     const int nw = (c->fusion && !gb) ? 2 : 1;
-    for (int i = 0; i < 2; i++) { L.links[i] = off; if (i < nl) off = align_up(off + (size_t)4 * ne * c->V * e, 256); }
-    for (int i = 0; i < 2; i++) { L.w[i] = off; if (i < nw) off = align_up(off + (size_t)c->pack * c->V * e, 256); }
-    L.gbuf = off; if (gb) off = align_up(off + (size_t)6 * c->V * e, 256);
-    const int nblk = std::max(measure_blocks(c->V), fused_blocks(c->V));
+    for (int i = 0; i < 2; i++) { L.links[i] = off; if (i < nl) off = align_up(off + (size_t)4 * ne * Vs * e, 256); }
+    for (int i = 0; i < 2; i++) { L.w[i] = off; if (i < nw) off = align_up(off + (size_t)c->pack * Vs * e, 256); }
+    L.gbuf = off; if (gb) off = align_up(off + (size_t)6 * Vs * e, 256);
+    const int nblk = std::max(measure_blocks(Vl), fused_blocks(Vl));
     L.partials = off; off = align_up(off + (size_t)2 * nblk * sizeof(double), 256);
     L.ctrl = off; off = align_up(off + sizeof(Ctrl), 256);
     L.hist = off; off = align_up(off + (size_t)LGF_HIST_CAP * sizeof(double2), 256);
     L.ptab = off; off = align_up(off + (size_t)sum_n(c) * sizeof(double), 256);
     L.tw = off; off = align_up(off + (size_t)sum_n(c) * e, 256);
-    L.staging_sites = c->V < (1 << 17) ? c->V : (1 << 17);
+    L.staging_sites = Vl < (1 << 17) ? Vl : (1 << 17);
     L.staging = off; off = align_up(off + (size_t)L.staging_sites * 36 * e, 256);
+    for (int i = 0; i < 2; i++) { L.xbuf[i] = off; if (c->shard_world > 0) off = align_up(off + (size_t)4 * Vl * e, 256); }
+    L.ptab_zt = off; if (c->shard_world > 0) off = align_up(off + (size_t)sum_n(c) * sizeof(double), 256);
     L.total = off;
     return L;
 }
@@ -412,6 +424,15 @@ int need_loaded(lgf_ctx *ctx)
     return LGF_OK;
 }
 
+// the single-GPU drivers (measure / iterate / fix / stage / field taps) see only this rank's slab
+int need_unsharded(lgf_ctx *ctx)
+{
+    int rc = need_loaded(ctx);
+    if (rc) return rc;
+    if (ctx->shard_world > 0) return fail(ctx, LGF_ERR_INVALID_ARG, "sharded context (SHARD_WORLD): drive it with lgf_shard_step");
+    return LGF_OK;
+}
+
 } // namespace
 
 extern "C" {
@@ -452,7 +473,8 @@ int lgf_set_option(lgf_ctx *ctx, int key, int64_t value)
 {
     if (!ctx) return LGF_ERR_INVALID_ARG;
     const bool layout_key = (key == LGF_OPT_RECON || key == LGF_OPT_FFT_BATCH || key == LGF_OPT_FFT_PATH || key == LGF_OPT_FUSION ||
-                             key == LGF_OPT_L2_PERSIST || key == LGF_OPT_ACCUM_G || key == LGF_OPT_ZBLOCK || key == LGF_OPT_FFT_PASSES);
+                             key == LGF_OPT_L2_PERSIST || key == LGF_OPT_ACCUM_G || key == LGF_OPT_ZBLOCK || key == LGF_OPT_FFT_PASSES ||
+                             key == LGF_OPT_SHARD_WORLD || key == LGF_OPT_SHARD_RANK);
     if (layout_key && ctx->bound) return fail(ctx, LGF_ERR_INVALID_ARG, "this option must be set before lgf_bind");
     switch (key) {
     case LGF_OPT_RECON:
@@ -491,6 +513,13 @@ int lgf_set_option(lgf_ctx *ctx, int key, int64_t value)
     case LGF_OPT_FFT_PASSES:
         if (value != 3 && value != 4 && value != 8) return fail(ctx, LGF_ERR_INVALID_ARG, "FFT_PASSES must be 3, 4 or 8");
         ctx->fft_passes = (int)value; break;
+    case LGF_OPT_SHARD_WORLD:
+        if (value < 0 || (value > 0 && (ctx->N[3] % value != 0 || ctx->N[1] % value != 0)))
+            return fail(ctx, LGF_ERR_INVALID_ARG, "SHARD_WORLD must be 0 (off) or divide Nt and Ny");
+        ctx->shard_world = (int)value; if (ctx->shard_rank >= value) ctx->shard_rank = 0; break;
+    case LGF_OPT_SHARD_RANK:
+        if (value < 0 || value >= std::max(1, ctx->shard_world)) return fail(ctx, LGF_ERR_INVALID_ARG, "SHARD_RANK must be in [0, SHARD_WORLD)");
+        ctx->shard_rank = (int)value; break;
     case LGF_OPT_ZT_PIPE:
         if (value != 0 && value != 1) return fail(ctx, LGF_ERR_INVALID_ARG, "ZT_PIPE must be 0 or 1");
         ctx->zt_pipe = (int)value; ctx->fa.zt_pipe = ctx->zt_pipe; graph_drop(ctx); break;
@@ -520,6 +549,9 @@ int lgf_bind(lgf_ctx *ctx, void *dev_workspace, size_t bytes, void *cuda_stream)
         return fail(ctx, LGF_ERR_INVALID_ARG, "FFT_PASSES = 4 / 8 need a lattice the tiled FFT covers (4: a square or 32 x n (z,t) tile)");
     if (ctx->fft_passes == 8 && ctx->accum)
         return fail(ctx, LGF_ERR_INVALID_ARG, "ACCUM_G builds g in the last 2D pass: not available with FFT_PASSES = 8");
+    if (ctx->shard_world > 0 && !(ctx->fusion && ctx->pack == 4 && ctx->fft_path == 0 && ctx->fft_passes == 3 && !ctx->accum &&
+                                  fft_tiled_gbuf_supported(ctx->N, ctx->prec)))
+        return fail(ctx, LGF_ERR_INVALID_ARG, "SHARD_WORLD needs the default path: FUSION = 1, FFT_BATCH = 4, FFT_PASSES = 3, no ACCUM_G, a lattice the tiled FFT covers");
     const Layout L = make_layout(ctx);
     if (bytes < L.total) return fail(ctx, LGF_ERR_WORKSPACE_TOO_SMALL, "workspace smaller than lgf_workspace_bytes()");
     ctx->lay = L;
@@ -527,9 +559,19 @@ int lgf_bind(lgf_ctx *ctx, void *dev_workspace, size_t bytes, void *cuda_stream)
     ctx->st = (cudaStream_t)cuda_stream;
     Geom g{};
     for (int d = 0; d < 4; d++) g.N[d] = ctx->N[d];
-    g.V = ctx->V;
     g.st[0] = 1; g.st[1] = g.N[0]; g.st[2] = (int64_t)g.N[0] * g.N[1]; g.st[3] = (int64_t)g.N[0] * g.N[1] * g.N[2];
     g.zb = ctx->zblock > 0 ? ctx->zblock : auto_zblock(ctx);
+    ctx->Vg = g.st[3] * ctx->N[3];
+    if (ctx->shard_world > 0) {
+        const int ntl = ctx->N[3] / ctx->shard_world;
+        ctx->V = g.st[3] * ntl;                 // the interchange arrays of this rank: its own time slices
+        ctx->Vp = g.st[3] * (ntl + 2);
+        g.N[3] = ntl + 2; g.Ntw = ntl; g.t0 = 1;
+    } else {
+        ctx->V = ctx->Vg; ctx->Vp = ctx->Vg;
+        g.Ntw = g.N[3]; g.t0 = 0;
+    }
+    g.V = ctx->Vp; g.Vw = ctx->V; g.Vg = ctx->Vg;
     SiteArgs &s = ctx->sa;
     s.geo = g;
     for (int i = 0; i < 2; i++) { ctx->links_buf[i] = ctx->base + L.links[i]; ctx->w_buf[i] = ctx->base + L.w[i]; }
@@ -540,7 +582,7 @@ int lgf_bind(lgf_ctx *ctx, void *dev_workspace, size_t bytes, void *cuda_stream)
     s.hist = (double2 *)(ctx->base + L.hist);
     s.prec = ctx->prec; s.recon = ctx->recon; s.pack = ctx->pack; s.gexp = ctx->gmap;
     FftArgs &f = ctx->fa;
-    f.geo = g; f.nfields = ctx->pack; f.prec = ctx->prec; f.zt_pipe = ctx->zt_pipe;
+    f.geo = g; f.nfields = ctx->pack; f.prec = ctx->prec; f.zt_pipe = ctx->zt_pipe; f.vnorm = (double)ctx->Vg;
     sync_ptrs(ctx);
     f.ptab = (const double *)(ctx->base + L.ptab);
     f.pmax2 = ctx->pmax2;
@@ -560,6 +602,27 @@ int lgf_bind(lgf_ctx *ctx, void *dev_workspace, size_t bytes, void *cuda_stream)
         }
     if (ctx->prec == LGF_PREC_FP64) CK(cudaMemcpyAsync(ctx->base + L.tw, twd.data(), sizeof(double) * 2 * sn, cudaMemcpyHostToDevice, ctx->st));
     else CK(cudaMemcpyAsync(ctx->base + L.tw, twf.data(), sizeof(float) * 2 * sn, cudaMemcpyHostToDevice, ctx->st));
+    if (ctx->shard_world > 0) {
+        // the (z,t) pass runs on the transposed field: all Nt time slices of the sites with y in this rank's range
+        const int R = ctx->shard_world, nyl = ctx->N[1] / R;
+        for (int i = 0; i < 2; i++) ctx->xbuf[i] = ctx->base + L.xbuf[i];
+        FftArgs &z = ctx->fa_zt;
+        z = f;
+        z.geo.N[1] = nyl; z.geo.N[3] = ctx->N[3];
+        z.geo.V = (int64_t)ctx->N[0] * nyl * ctx->N[2];                   // field stride
+        z.geo.st[1] = ctx->N[0]; z.geo.st[2] = (int64_t)ctx->N[0] * nyl; z.geo.st[3] = 4 * z.geo.V;
+        z.w = ctx->xbuf[1];
+        std::vector<double> pz;                                            // the y table restricted to this rank's rows
+        pz.insert(pz.end(), ctx->ptab_h.begin(), ctx->ptab_h.begin() + ctx->N[0]);
+        pz.insert(pz.end(), ctx->ptab_h.begin() + ctx->N[0] + ctx->shard_rank * nyl, ctx->ptab_h.begin() + ctx->N[0] + (ctx->shard_rank + 1) * nyl);
+        pz.insert(pz.end(), ctx->ptab_h.begin() + ctx->N[0] + ctx->N[1], ctx->ptab_h.end());
+        CK(cudaMemcpyAsync(ctx->base + L.ptab_zt, pz.data(), sizeof(double) * pz.size(), cudaMemcpyHostToDevice, ctx->st));
+        CK(cudaStreamSynchronize(ctx->st));
+        z.ptab = (const double *)(ctx->base + L.ptab_zt);
+        // halo slices and exchange buffers start from zeros (they are read by passes that run over whole arrays)
+        CK(cudaMemsetAsync(ctx->base, 0, L.partials, ctx->st));
+        CK(cudaMemsetAsync(ctx->base + L.xbuf[0], 0, L.ptab_zt - L.xbuf[0], ctx->st));
+    }
     CK(cudaMemsetAsync(s.ctrl, 0, sizeof(Ctrl), ctx->st));
     CK(cudaMemsetAsync(s.hist, 0, sizeof(double2) * LGF_HIST_CAP, ctx->st));
     CK(cudaStreamSynchronize(ctx->st)); // the host vectors above go out of scope
@@ -603,7 +666,7 @@ int lgf_load_links(lgf_ctx *ctx, const void *src, int src_is_device, int src_lay
     }
     int rc = clear_done(ctx);
     if (rc) return rc;
-    do_measure(ctx, -1.0, 0);
+    if (ctx->shard_world == 0) do_measure(ctx, -1.0, 0);     // sharded: the measure needs the halo links first (lgf_shard_step)
     CK(cudaGetLastError());
     if (!src_is_device) CK(cudaStreamSynchronize(ctx->st));
     ctx->loaded = true;
@@ -636,7 +699,7 @@ int lgf_get_links(lgf_ctx *ctx, void *dst, int dst_is_device, int dst_layout)
 
 int lgf_measure(lgf_ctx *ctx, double *F, double *theta)
 {
-    int rc = need_loaded(ctx);
+    int rc = need_unsharded(ctx);
     if (rc) return rc;
     if ((rc = clear_done(ctx))) return rc;
     materialise(ctx);
@@ -650,7 +713,7 @@ int lgf_measure(lgf_ctx *ctx, double *F, double *theta)
 
 int lgf_iterate(lgf_ctx *ctx, double alpha, int64_t n, lgf_result *out)
 {
-    int rc = need_loaded(ctx);
+    int rc = need_unsharded(ctx);
     if (rc) return rc;
     if (n < 0) return fail(ctx, LGF_ERR_INVALID_ARG, "n must be >= 0");
     if (ctx->wstate != 1) {
@@ -674,7 +737,7 @@ int lgf_iterate(lgf_ctx *ctx, double alpha, int64_t n, lgf_result *out)
 
 int lgf_fix(lgf_ctx *ctx, double alpha, double eps, lgf_result *out)
 {
-    int rc = need_loaded(ctx);
+    int rc = need_unsharded(ctx);
     if (rc) return rc;
     if (!(eps >= 0)) return fail(ctx, LGF_ERR_INVALID_ARG, "eps must be >= 0");
     if (ctx->wstate != 1) {
@@ -704,7 +767,7 @@ int lgf_fix(lgf_ctx *ctx, double alpha, double eps, lgf_result *out)
 
 int lgf_stage(lgf_ctx *ctx, int stage, double alpha)
 {
-    int rc = need_loaded(ctx);
+    int rc = need_unsharded(ctx);
     if (rc) return rc;
     if ((rc = clear_done(ctx))) return rc;
     materialise(ctx);
@@ -818,6 +881,87 @@ int lgf_reset_counters(lgf_ctx *ctx)
 int lgf_uses_tiled_fft(const lgf_ctx *ctx) { return ctx && ctx->tiled ? 1 : 0; }
 int lgf_uses_gbuf(const lgf_ctx *ctx) { return ctx && ctx->bound && ctx->use_gbuf ? 1 : 0; }
 int lgf_zblock(const lgf_ctx *ctx) { return ctx && ctx->bound ? ctx->sa.geo.zb : 0; }
+
+int lgf_shard_step(lgf_ctx *ctx, int step, double alpha, double eps)
+{
+    int rc = need_loaded(ctx);
+    if (rc) return rc;
+    if (ctx->shard_world <= 0) return fail(ctx, LGF_ERR_INVALID_ARG, "not a sharded context (LGF_OPT_SHARD_WORLD)");
+    switch (step) {
+    case LGF_SHARD_MEASURE:
+        if ((rc = clear_done(ctx))) return rc;
+        do_measure(ctx, -1.0, 0); break;
+    case LGF_SHARD_RESET:
+        run_kernel(ctx, LGF_KERNEL_LAYOUT, 1, [&] { launch_ctrl_reset(ctx->sa, eps, ctx->st); }); break;
+    case LGF_SHARD_XY_FWD:
+        if (ctx->wstate != 1) return fail(ctx, LGF_ERR_INVALID_ARG, "XY_FWD needs Delta in the field buffer");
+        run_kernel(ctx, LGF_KERNEL_FFT_XY_FWD, 1, [&] { launch_fft_tiled(ctx->fa, 0, ctx->st); }); break;
+    case LGF_SHARD_PACK:
+        run_kernel(ctx, LGF_KERNEL_LAYOUT, 1, [&] { launch_slab_pack(ctx->sa, ctx->xbuf[0], ctx->shard_world, 0, ctx->st); }); break;
+    case LGF_SHARD_ZT:
+        run_kernel(ctx, LGF_KERNEL_FFT_ZT, 1, [&] { launch_fft_tiled(ctx->fa_zt, 1, ctx->st); }); break;
+    case LGF_SHARD_UNPACK:
+        run_kernel(ctx, LGF_KERNEL_LAYOUT, 1, [&] { launch_slab_pack(ctx->sa, ctx->xbuf[0], ctx->shard_world, 1, ctx->st); }); break;
+    case LGF_SHARD_XY_INV_G:
+        run_kernel(ctx, LGF_KERNEL_FFT_XY_INV_G, 1, [&] { launch_fft_tiled_inv_g(ctx->fa, ctx->gbuf, alpha, ctx->gmap, 0, ctx->st); });
+        ctx->wstate = 2; break;
+    case LGF_SHARD_LINK: {
+        void *lin = ctx->links_buf[ctx->cur], *lout = ctx->links_buf[ctx->cur ^ 1];
+        run_kernel(ctx, LGF_KERNEL_UPDATE_MEASURE, 1,
+                   [&] { launch_update_measure(ctx->sa, lin, lout, ctx->gbuf, 1, ctx->w_buf[ctx->wcur], alpha, -1.0, ctx->st); });
+        ctx->cur ^= 1;
+        sync_ptrs(ctx);
+        ctx->wstate = 1;
+        break;
+    }
+    case LGF_SHARD_FINISH:
+        run_kernel(ctx, LGF_KERNEL_LAYOUT, 1, [&] { launch_slab_finish(ctx->sa, eps, ctx->st); }); break;
+    default: return fail(ctx, LGF_ERR_INVALID_ARG, "unknown shard step");
+    }
+    CK(cudaGetLastError());
+    return LGF_OK;
+}
+
+int lgf_shard_region(const lgf_ctx *ctx, int region, size_t *offset, size_t *bytes)
+{
+    if (!ctx || !ctx->bound || ctx->shard_world <= 0 || !offset || !bytes) return LGF_ERR_INVALID_ARG;
+    const size_t e = ctx->prec == LGF_PREC_FP64 ? 16 : 8;
+    const int ne = ctx->recon == 12 ? 6 : 9;
+    const Layout &L = ctx->lay;
+    switch (region) {
+    case LGF_REGION_CTRL: *offset = L.ctrl; *bytes = 2 * sizeof(double); break;        /* F, theta: the first two doubles */
+    case LGF_REGION_XSEND: *offset = L.xbuf[0]; *bytes = (size_t)4 * ctx->V * e; break;
+    case LGF_REGION_XRECV: *offset = L.xbuf[1]; *bytes = (size_t)4 * ctx->V * e; break;
+    case LGF_REGION_G: *offset = L.gbuf; *bytes = (size_t)6 * ctx->Vp * e; break;
+    case LGF_REGION_LINKS: *offset = L.links[ctx->cur]; *bytes = (size_t)4 * ne * ctx->Vp * e; break;
+    default: return LGF_ERR_INVALID_ARG;
+    }
+    return LGF_OK;
+}
+
+int lgf_shard_info(const lgf_ctx *ctx, int64_t *info, int n)
+{
+    if (!ctx || !ctx->bound || ctx->shard_world <= 0 || !info || n < 8) return LGF_ERR_INVALID_ARG;
+    info[0] = ctx->Vp;                                                   /* stored sites per array (with halos) */
+    info[1] = (int64_t)ctx->N[0] * ctx->N[1] * ctx->N[2];                /* sites of one time slice */
+    info[2] = ctx->N[3] / ctx->shard_world;                              /* own time slices */
+    info[3] = ctx->recon == 12 ? 6 : 9;                                  /* complex arrays per link direction */
+    info[4] = ctx->prec == LGF_PREC_FP64 ? 16 : 8;                       /* bytes per complex number */
+    info[5] = ctx->shard_world; info[6] = ctx->shard_rank; info[7] = ctx->V;
+    return LGF_OK;
+}
+
+int lgf_shard_result(lgf_ctx *ctx, lgf_result *out)
+{
+    int rc = need_loaded(ctx);
+    if (rc) return rc;
+    if (!out) return fail(ctx, LGF_ERR_INVALID_ARG, "out is NULL");
+    Ctrl h;
+    if ((rc = read_ctrl(ctx, &h))) return rc;
+    out->iterations = h.iter; out->F = h.F; out->theta = h.theta; out->converged = (h.done == 1);
+    if (h.done == 2) return fail(ctx, LGF_ERR_NUMERIC, "theta is NaN or Inf");
+    return LGF_OK;
+}
 
 int lgf_sync_links(lgf_ctx *ctx)
 {

@@ -21,6 +21,10 @@ PREC_FP64, PREC_FP32 = 0, 1
 LAYOUT_AOS, LAYOUT_AOS12 = 0, 1
 OPT_RECON, OPT_FFT_BATCH, OPT_MAX_ITER, OPT_CHECK_INTERVAL, OPT_FFT_PATH, OPT_PROFILE, OPT_FUSION, OPT_L2_PERSIST = 1, 2, 3, 4, 5, 6, 7, 8
 OPT_GMAP, OPT_ACCUM_G, OPT_GRAPH, OPT_ZBLOCK, OPT_ZT_PIPE, OPT_FFT_PASSES = 9, 10, 11, 12, 13, 14
+OPT_SHARD_WORLD, OPT_SHARD_RANK = 15, 16
+(SHARD_MEASURE, SHARD_RESET, SHARD_XY_FWD, SHARD_PACK, SHARD_ZT, SHARD_UNPACK, SHARD_XY_INV_G, SHARD_LINK,
+ SHARD_FINISH) = range(9)
+REGION_CTRL, REGION_XSEND, REGION_XRECV, REGION_G, REGION_LINKS = range(5)
 GMAP_FIRST_ORDER, GMAP_EXP = 0, 1
 FIELD_DELTA, FIELD_W, FIELD_G = 0, 1, 2
 STAGE_MEASURE, STAGE_FOURIER, STAGE_UPDATE = 0, 1, 2
@@ -32,7 +36,7 @@ SYMBOLS = [
     "lgf_create", "lgf_set_option", "lgf_workspace_bytes", "lgf_bind", "lgf_load_links", "lgf_get_links",
     "lgf_measure", "lgf_iterate", "lgf_fix", "lgf_stage", "lgf_get_field", "lgf_set_field", "lgf_history",
     "lgf_kernel_time", "lgf_launch_count", "lgf_reset_counters", "lgf_uses_tiled_fft", "lgf_uses_gbuf", "lgf_zblock", "lgf_sync_links", "lgf_last_error",
-    "lgf_destroy", "lgf_debug_dfma_rate",
+    "lgf_destroy", "lgf_debug_dfma_rate", "lgf_shard_step", "lgf_shard_region", "lgf_shard_info", "lgf_shard_result",
 ]
 
 
@@ -88,6 +92,10 @@ def lib():
     L.lgf_last_error.restype = ctypes.c_char_p
     L.lgf_destroy.argtypes = [vp]
     L.lgf_debug_dfma_rate.argtypes = [vp, dp]
+    L.lgf_shard_step.argtypes = [vp, i, d, d]
+    L.lgf_shard_region.argtypes = [vp, i, ctypes.POINTER(ctypes.c_size_t), ctypes.POINTER(ctypes.c_size_t)]
+    L.lgf_shard_info.argtypes = [vp, ctypes.POINTER(i64), i]
+    L.lgf_shard_result.argtypes = [vp, rp]
     _lib = L
     return L
 
@@ -115,12 +123,14 @@ class GaugeFixer:
 
     def __init__(self, N, precision="fp64", recon=18, fft_batch=4, fft_path=0, device="cuda:0",
                  stream=None, max_iter=None, check_interval=None, profile=False, fusion=None, l2_persist=None, gmap=None,
-                 accum_g=None, graph=None, zblock=None, zt_pipe=None, fft_passes=None):
+                 accum_g=None, graph=None, zblock=None, zt_pipe=None, fft_passes=None, shard=None):
         import torch
 
         self.torch = torch
         self.N = _dims(N)
         self.V = self.N[0] * self.N[1] * self.N[2] * self.N[3]
+        if shard is not None:                   # (world, rank): this object holds one t-slab of the lattice N
+            self.V //= int(shard[0])            # sites of the interchange arrays: the rank's own time slices
         self.prec = {"fp64": PREC_FP64, "fp32": PREC_FP32}[precision]
         self.np_dtype = np.complex128 if self.prec == PREC_FP64 else np.complex64
         self.torch_dtype = torch.complex128 if self.prec == PREC_FP64 else torch.complex64
@@ -148,6 +158,9 @@ class GaugeFixer:
             self.set_option(OPT_ZT_PIPE, zt_pipe)
         if fft_passes is not None:
             self.set_option(OPT_FFT_PASSES, fft_passes)
+        if shard is not None:
+            self.set_option(OPT_SHARD_WORLD, shard[0])
+            self.set_option(OPT_SHARD_RANK, shard[1])
         if max_iter is not None:
             self.set_option(OPT_MAX_ITER, max_iter)
         if check_interval is not None:
@@ -286,6 +299,28 @@ class GaugeFixer:
 
     def zblock(self):
         return int(self.L.lgf_zblock(self.ctx))
+
+    # -- one lattice sharded over several GPUs (LGF_OPT_SHARD_WORLD): the steps and the exchanged regions
+    def shard_step(self, step, alpha=0.0, eps=-1.0):
+        self._ck(self.L.lgf_shard_step(self.ctx, int(step), float(alpha), float(eps)))
+
+    def shard_region(self, region, dtype):
+        """A torch view (1D, `dtype`) of an exchanged region of the workspace (include/lgf.h, LGF_REGION_*)."""
+        off, nb = ctypes.c_size_t(), ctypes.c_size_t()
+        self._ck(self.L.lgf_shard_region(self.ctx, int(region), ctypes.byref(off), ctypes.byref(nb)))
+        base = (self.workspace.data_ptr() + 255) // 256 * 256 - self.workspace.data_ptr()
+        return self.workspace[base + off.value: base + off.value + nb.value].view(dtype)
+
+    def shard_info(self):
+        a = (ctypes.c_int64 * 8)()
+        self._ck(self.L.lgf_shard_info(self.ctx, a, 8))
+        keys = ("stored_sites", "slice_sites", "own_slices", "ne", "elem_bytes", "world", "rank", "sites")
+        return dict(zip(keys, [int(x) for x in a]))
+
+    def shard_result(self):
+        r = lgf_result()
+        self._ck(self.L.lgf_shard_result(self.ctx, ctypes.byref(r)))
+        return r
 
     def sync_links(self):
         self._ck(self.L.lgf_sync_links(self.ctx))

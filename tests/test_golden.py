@@ -59,7 +59,10 @@ def test_all_golden_trajectories_satisfy_the_invariants():
         it, F, th, hist = read_golden(f)
         assert hist.shape[0] == it + 1
         assert th <= 1e-15 < hist[-2, 1]                       # stopped at the first theta <= eps
-        assert np.all(np.diff(hist[:, 0]) >= 0)                # F never decreases (P12)
+        # F never decreases (P12), up to the rounding of the stored double once the increments fall below one
+        # unit in the last place at convergence (1.1e-16 for F in [0.5, 1): the 48^4 trajectory ends ...703, ...702)
+        assert np.all(np.diff(hist[:, 0]) >= -2.3e-16)
+        assert np.all(np.diff(hist[: it - 5, 0]) > 0)
         assert hist[-1, 0] == F and hist[-1, 1] == th
         tail = hist[-1, 1] / hist[-2, 1]
         assert 0.1 < tail < 0.5                                # tail ratio ~0.26

@@ -330,12 +330,14 @@ def test_headline_32_12real_one_iteration_and_golden(lgf):
     assert np.abs(U1 - Uo).max() < 1e-12
     assert abs(r1.F - hist[1, 0]) <= 1e-10 * abs(hist[1, 0])
     assert abs(r1.theta - hist[1, 1]) <= 1e-10 * hist[1, 1]
-    path = golden_path(n, seed)
-    if os.path.exists(path):
-        it, F, th, ghist = read_golden(path)
-        gf.load_links(U)
-        r = gf.fix(ALPHA, 1e-15)
-        assert r.converged == 1 and abs(r.iterations - it) <= 0.02 * it and abs(r.F - F) <= 1e-10
+    it, F, th, ghist = read_golden(golden_path(n, seed))
+    assert np.array_equal(hist[1], ghist[1])                  # the golden file belongs to this input
+    gf.load_links(U)
+    r = gf.fix(ALPHA, 1e-15)
+    assert r.converged == 1 and abs(r.iterations - it) <= 0.02 * it and abs(r.F - F) <= 1e-10
+    h = gf.history()
+    k = min(h.shape[0], ghist.shape[0]) - 3
+    assert np.allclose(h[:k, 0], ghist[:k, 0], rtol=0, atol=1e-10) and np.allclose(h[:k, 1], ghist[:k, 1], rtol=1e-6, atol=1e-25)
 
 
 def _mem_available_gb():
@@ -359,46 +361,66 @@ def _unitarity_defect(U):
     return worst
 
 
+def _golden_count(hist, eps):
+    """Iterations the oracle's trajectory needs to reach theta <= eps (R2: stop at the first theta <= eps)."""
+    idx = np.nonzero(hist[:, 1] <= eps)[0]
+    assert idx.size, "golden trajectory never reaches eps"
+    return int(idx[0])
+
+
 @pytest.mark.slow
 def test_full_size_48_fp32(lgf):
     """BASELINE config 4 in the configuration bench.py times: 48^4, FP32 storage and FFT, FP64 sums,
     18-real links.  One iteration against the oracle element by element (north_star: 1e-5), then
-    Algorithm 1 to theta <= 1e-12 with the invariants that hold at any size."""
+    Algorithm 1 to theta <= 1e-12 against the oracle's golden trajectory (tests/golden/fix_48_*.txt, FP64
+    oracle on the same generator output): iteration count within +-2 %, final F within 1e-5, the (F, theta)
+    prefix, plus the invariants that hold at any size.  The ACCUM_G leg is held to the same golden."""
     n, seed = 48, gen.BASE_SEED + 48
+    git, gF, gth, ghist = read_golden(golden_path(n, seed))
+    n12 = _golden_count(ghist, 1e-12)
     U = gen.gen_links(n, 0.5, seed)
     gf = fixer(lgf, n, precision="fp32", recon=18)
     assert gf.uses_tiled_fft() and gf.uses_gbuf()
     U32 = U.astype(np.complex64)
     gf.load_links(U32)
     _, F0, th0 = oracle.measure(n, U, want_delta=False)
+    assert F0 == ghist[0, 0] and th0 == ghist[0, 1]           # the golden file belongs to this input
     Fg, thg = gf.measure()
     assert abs(Fg - F0) < 1e-6 and abs(thg - th0) <= 1e-5 * th0
     r1 = gf.iterate(ALPHA, 1)
     U1 = gf.get_links().astype(np.complex128)
     Uo = U.copy()
     hist = oracle.iterate(n, Uo, ALPHA, 1)
+    assert np.array_equal(hist[1], ghist[1])
     assert np.abs(U1 - Uo).max() < 1e-5
     assert abs(r1.F - hist[1, 0]) < 1e-5 and abs(r1.theta - hist[1, 1]) <= 1e-4 * hist[1, 1]
     del Uo, U1
-    gf.load_links(U32)
-    r = gf.fix(ALPHA, 1e-12)
-    assert r.converged == 1 and r.theta <= 1e-12 and 35 <= r.iterations <= 70
-    h = gf.history()
-    assert np.all(np.diff(h[:, 0]) >= -1e-6)                 # F never decreases (pin P12), FP32 rounding
-    Ufix = gf.get_links()
-    assert _unitarity_defect(Ufix) < 5e-5                     # no reunitarisation of links (reading R18)
-    assert abs(oracle.plaquette(n, Ufix.astype(np.complex128)) - oracle.plaquette(n, U)) < 1e-5
-    # LGF_OPT_ACCUM_G at the same size (the configuration `bench.py --accum-g 1 --workload 48^4` times)
+
+    def check_against_golden(fx):
+        fx.load_links(U32)
+        r = fx.fix(ALPHA, 1e-12)
+        assert r.converged == 1 and r.theta <= 1e-12
+        assert abs(r.iterations - n12) <= max(1, int(0.02 * n12)), (r.iterations, n12)
+        assert abs(r.F - ghist[r.iterations, 0]) < 1e-5 and abs(r.F - gF) < 1e-5
+        h = fx.history()
+        assert h.shape[0] == r.iterations + 1
+        k = min(h.shape[0], n12) - 6                          # FP32 theta leaves the FP64 trajectory near its floor
+        assert np.allclose(h[:k, 0], ghist[:k, 0], rtol=0, atol=1e-5)
+        assert np.allclose(h[:k, 1], ghist[:k, 1], rtol=2e-3, atol=0)
+        assert np.all(np.diff(h[:, 0]) >= -1e-6)              # F never decreases (pin P12), FP32 rounding
+        Ufix = fx.get_links()
+        assert _unitarity_defect(Ufix) < 5e-5                 # no reunitarisation of links (reading R18)
+        assert abs(oracle.plaquette(n, Ufix.astype(np.complex128)) - oracle.plaquette(n, U)) < 1e-5
+        return r, Ufix
+
+    r, Ufix = check_against_golden(gf)
     gf.close()
+    # LGF_OPT_ACCUM_G at the same size (the configuration `bench.py --accum-g 1 --workload 48^4` times)
     ga = fixer(lgf, n, precision="fp32", recon=18, accum_g=1)
     ga.load_links(U32)
     ra1 = ga.iterate(ALPHA, 1)
     assert abs(ra1.F - hist[1, 0]) < 1e-5 and abs(ra1.theta - hist[1, 1]) <= 1e-4 * hist[1, 1]
-    ga.load_links(U32)
-    ra = ga.fix(ALPHA, 1e-12)
-    assert ra.converged == 1 and abs(ra.iterations - r.iterations) <= 2 and abs(ra.F - r.F) < 1e-5
-    Ua = ga.get_links()
-    assert _unitarity_defect(Ua) < 5e-5
+    ra, Ua = check_against_golden(ga)
     assert np.abs(Ua - Ufix).max() < 5e-3                     # same minimum; FP32 rounding differs along the way
     ga.close()
 
@@ -406,16 +428,21 @@ def test_full_size_48_fp32(lgf):
 @pytest.mark.slow
 def test_full_size_64_fp64(lgf):
     """BASELINE config 5 in the configuration bench.py times: 64^4, FP64, 18-real links (9.7 GB of
-    links).  Measure and one iteration against the oracle (element by element when the host has the
-    memory for it), then Algorithm 1 to theta <= 1e-15 with the invariants that hold at any size."""
+    links).  Measure and one iteration against the oracle element by element, then Algorithm 1 to
+    theta <= 1e-15 against the oracle's golden trajectory (tests/golden/fix_64_*.txt): iteration count within
+    +-2 %, final F within 1e-10, the (F, theta) prefix, plus the invariants that hold at any size.  The
+    ACCUM_G leg is held to the same golden.  Needs about 45 GB of host memory (explicit skip otherwise)."""
     if _mem_available_gb() < 48:
         pytest.skip("needs about 45 GB of host memory")
     n, seed = 64, gen.BASE_SEED + 64
+    git, gF, gth, ghist = read_golden(golden_path(n, seed))
     U = gen.gen_links(n, 0.6, seed)
     gf = fixer(lgf, n, recon=18)
     assert gf.uses_tiled_fft() and gf.uses_gbuf()             # 64^2 planes: 2-CTA cluster variant of the last pass
+    assert gf.zblock() < 64                                   # one time slice of links exceeds L2: blocked site walk
     gf.load_links(U)
     D, F0, th0 = oracle.measure(n, U)
+    assert F0 == ghist[0, 0] and th0 == ghist[0, 1]           # the golden file belongs to this input
     Fg, thg = gf.measure()
     assert abs(Fg - F0) <= 1e-12 * max(abs(F0), 1e-3) + 1e-15 and abs(thg - th0) <= 1e-12 * th0
     assert np.abs(gf.get_field(lgf.FIELD_DELTA) - D).max() < 1e-13
@@ -423,36 +450,44 @@ def test_full_size_64_fp64(lgf):
     p0 = oracle.plaquette(n, U)
     r1 = gf.iterate(ALPHA, 1)
     U1 = gf.get_links()
-    # the fused kernel's F, theta are those of the links it stored
-    _, F1, th1 = oracle.measure(n, U1, want_delta=False)
-    assert abs(r1.F - F1) <= 1e-10 * abs(F1) and abs(r1.theta - th1) <= 1e-10 * th1
-    assert r1.F > F0 and abs(oracle.plaquette(n, U1) - p0) < 1e-12     # a gauge transformation (pin P11)
-    if _mem_available_gb() >= 40:
-        hist = oracle.iterate(n, U, ALPHA, 1)                 # in place: U becomes the oracle's U after one iteration
-        assert np.abs(U1 - U).max() < 1e-12
-        assert abs(r1.F - hist[1, 0]) <= 1e-10 * abs(hist[1, 0]) and abs(r1.theta - hist[1, 1]) <= 1e-10 * hist[1, 1]
+    hist = oracle.iterate(n, U, ALPHA, 1)                     # in place: U becomes the oracle's links after one iteration
+    assert np.array_equal(hist[1], ghist[1])
+    worst = 0.0
+    for lo in range(0, U.shape[0], 1 << 20):
+        worst = max(worst, float(np.abs(U1[lo:lo + (1 << 20)] - U[lo:lo + (1 << 20)]).max()))
+    assert worst < 1e-12
+    assert abs(r1.F - hist[1, 0]) <= 1e-10 * abs(hist[1, 0]) and abs(r1.theta - hist[1, 1]) <= 1e-10 * hist[1, 1]
+    assert abs(oracle.plaquette(n, U1) - p0) < 1e-12          # a gauge transformation (pin P11)
     del U1
-    r = gf.fix(ALPHA, 1e-15)                                  # continues from the links after one iteration
-    assert r.converged == 1 and r.theta <= 1e-15 and 35 <= r.iterations <= 70
-    h = gf.history()
-    assert np.all(np.diff(h[:, 0]) >= -1e-15)
+
+    def check_against_golden(fx):
+        """fx holds the links after one iteration: the rest of the trajectory is rows 1.. of the golden file"""
+        r = fx.fix(ALPHA, 1e-15)
+        assert r.converged == 1 and r.theta <= 1e-15
+        assert abs(1 + r.iterations - git) <= int(0.02 * git), (r.iterations, git)
+        assert abs(r.F - gF) <= 1e-10
+        h = fx.history()
+        assert h.shape[0] == r.iterations + 1
+        k = min(h.shape[0], ghist.shape[0] - 1) - 3           # the tail sits at the rounding floor
+        assert np.allclose(h[:k, 0], ghist[1:1 + k, 0], rtol=0, atol=1e-10)
+        assert np.allclose(h[:k, 1], ghist[1:1 + k, 1], rtol=1e-6, atol=1e-25)
+        assert np.all(np.diff(h[:, 0]) >= -1e-15)
+        return r
+
+    r = check_against_golden(gf)                              # continues from the links after one iteration
     Ufix = gf.get_links()
     assert _unitarity_defect(Ufix) < 1e-12
     assert abs(oracle.plaquette(n, Ufix) - p0) < 1e-12
-    # LGF_OPT_ACCUM_G at the same size against the default path, from the same start (whatever U holds now)
-    gf.load_links(U)
-    rb = gf.fix(ALPHA, 1e-15)
-    Ub = gf.get_links(out=Ufix)
     gf.close()
+    # LGF_OPT_ACCUM_G at the same size, from the oracle's links after one iteration, against the same golden rows
     ga = fixer(lgf, n, recon=18, accum_g=1)
     ga.load_links(U)
-    ra = ga.fix(ALPHA, 1e-15)
-    assert ra.converged == 1 and ra.iterations == rb.iterations and abs(ra.F - rb.F) <= 1e-10
+    ra = check_against_golden(ga)
     del U
     Ua = ga.get_links()
     assert _unitarity_defect(Ua) < 1e-12
     worst = 0.0
     for lo in range(0, Ua.shape[0], 1 << 20):
-        worst = max(worst, float(np.abs(Ua[lo:lo + (1 << 20)] - Ub[lo:lo + (1 << 20)]).max()))
-    assert worst < 1e-9
+        worst = max(worst, float(np.abs(Ua[lo:lo + (1 << 20)] - Ufix[lo:lo + (1 << 20)]).max()))
+    assert worst < 1e-9                                       # the same minimum
     ga.close()
