@@ -422,8 +422,9 @@ def run_ours(args):
                          f"{os.cpu_count()} cores on the box)"}
 
     traffic, traffic_src = ncu_traffic(f"{args.workload}-{prec}-recon{recon}-fields{args.fft_batch}", dom)
-    # FP64 instruction counts per site of the two link kernels (cuobjdump -sass of this build, profiles/r02_sass.md)
-    fp64_per_site = {"update_measure": 1722, "measure_acc": 1500}
+    # FP64 instructions (DFMA + DMUL + DADD) per site of the link kernels, counted in the SASS of this build up to the block
+    # reduction (cuobjdump -sass, profiles/r02_sass.md): 12-real 1182 + 289 + 176, 18-real 1038 + 241 + 188 (ACCUM_G 18-real: sum form)
+    fp64_per_site = {"update_measure": 1647 if recon == 12 else 1467, "measure_acc": 1647 if recon == 12 else 1316}
     alu = None
     if dfma_rate:
         nominal = 148 * 64 * 1.965e9

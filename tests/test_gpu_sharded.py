@@ -72,7 +72,7 @@ def test_sharded_fix_matches_golden(mods, R):
     Ufix = _gather(sg.get_links())
     assert abs(oracle.plaquette(n, Ufix) - oracle.plaquette(n, U)) < 1e-12      # a gauge transformation (pin P11)
     r2 = sg.fix(ALPHA, 1e-15)
-    assert r2.iterations == it and r2.converged == 1                              # already converged: no further step
+    assert r2.iterations == 0 and r2.converged == 1 and r2.F == r.F               # already converged: no further step
     sg.close()
 
 
