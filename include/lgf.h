@@ -152,8 +152,16 @@ enum {
                                    R = 1 is valid (the exchanges are with itself).  Default path only (FUSION = 1,
                                    FFT_BATCH = 4, FFT_PASSES = 3, no ACCUM_G, tiled FFT).  0 (default): off.
                                    Before lgf_bind. */
-    LGF_OPT_SHARD_RANK = 16     /* which slab, 0 <= rank < SHARD_WORLD: time slices [rank Nt/R, (rank+1) Nt/R).
+    LGF_OPT_SHARD_RANK = 16,    /* which slab, 0 <= rank < SHARD_WORLD: time slices [rank Nt/R, (rank+1) Nt/R).
                                    Set after SHARD_WORLD, before lgf_bind. */
+    LGF_OPT_TMARCH = 17         /* 0 (default: 4 for FP32 contexts without ACCUM_G, else 1, as measured), 1, 2 or 4:
+                                   consecutive time slices a thread of the fused link kernel walks.  From its
+                                   second site on the -t neighbour is the thread's own previous site, whose product
+                                   g(x) U_t(x) it has just formed (Alg. 1 lines 12-16), so 12 of the
+                                   102 loads and one of the nine 3x3 products per site are saved.  Falls back to 1
+                                   when it does not divide the number of time slices the context walks.  Same
+                                   arithmetic per link; the order of the F, theta partial sums changes (1e-16).
+                                   Before lgf_bind. */
 };
 
 /* lgf_shard_step selectors: the kernels of one iteration of a sharded lattice, in the order of a step

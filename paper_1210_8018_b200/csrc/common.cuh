@@ -114,16 +114,18 @@ __device__ __forceinline__ void site_coords(const Geom &g, int64_t s, int c[4])
 // slice of links is larger than L2 (64^4: 151 MB per slice).  Only the first
 // plane of a z-block misses its -z neighbours (1/zb of the sites).  zb = Nz is the lexicographic order.
 // Returns the site index and fills c[0..3]; valid for r < Vw.
-__device__ __forceinline__ int64_t walk_site(const Geom &g, int64_t r, int c[4])
+// tk > 1 (the link kernel's LGF_OPT_TMARCH): a thread handles tk consecutive time slices; r then runs over Vw / tk
+// threads and the site returned is the first of the tk.
+__device__ __forceinline__ int64_t walk_site(const Geom &g, int64_t r, int c[4], int tk = 1)
 {
     const unsigned P = (unsigned)(g.N[0] * g.N[1]);
     const unsigned u = (unsigned)r;          // V <= 64^4 = 2^24
     const unsigned o = u % P, q = u / P;
     c[0] = (int)(o % (unsigned)g.N[0]);
     c[1] = (int)(o / (unsigned)g.N[0]);
-    const unsigned per = (unsigned)(g.zb * g.Ntw);
+    const unsigned per = (unsigned)(g.zb * (g.Ntw / tk));
     const unsigned zblk = q / per, rem = q % per;
-    c[3] = (int)(rem / (unsigned)g.zb) + g.t0;
+    c[3] = (int)(rem / (unsigned)g.zb) * tk + g.t0;
     c[2] = (int)(zblk * (unsigned)g.zb + rem % (unsigned)g.zb);
     return (int64_t)o + (int64_t)P * (c[2] + g.N[2] * c[3]);
 }

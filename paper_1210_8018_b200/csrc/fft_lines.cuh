@@ -185,24 +185,114 @@ template <typename T, int N> struct Line<T, N, 2> {
     }
 };
 
-// thread t of a group -> (line, half).  S = 2 keeps the two halves of a line 16 lanes apart, so
-// that the 8 lanes of a shared-memory wavefront still belong to 8 consecutive lines.
+// S = 4: the line is shared by the four lanes l, l^8, l^16, l^24 of a warp, quarter h = 2 a + b (a: lane bit 4,
+// b: lane bit 3), N/4 elements each: the two-lane scheme applied twice.  Lane h starts with the positions
+// [h N/8, (h+1) N/8) and the same plus N/2; the first radix-2 stage and an exchange across bit a leave y
+// (even frequencies) in the lanes a = 0 and z (odd) in a = 1, each N/2-point sequence shared by the two lanes b = 0, 1
+// exactly as a two-lane line is; the second stage and an exchange across bit b leave every lane with an
+// N/4-point sequence of its own.  Slot s of lane (a, b) ends up holding frequency 4 slot_freq<N/4>(s) + a + 2 b.
+// Same number of shuffles and selects per thread as the two-lane form of a line of half the length, half the
+// registers per thread and twice the threads per line: for kernels that are bound by latency at 16 warps per
+// SM (profiles/r02_fft_passes.md).
+template <typename V> __device__ __forceinline__ V shfl8(unsigned mask, V v)
+{
+    v.x = __shfl_xor_sync(mask, v.x, 8);
+    v.y = __shfl_xor_sync(mask, v.y, 8);
+    return v;
+}
+template <typename T, int N> struct Line<T, N, 4> {
+    static_assert(N % 8 == 0, "four-lane lines need N divisible by 8");
+    static constexpr int NL = N / 4, Q = N / 8, M = N / 2;
+    static __device__ __forceinline__ int nat(int i, int h) { return h * Q + (i >= Q ? i - Q + M : i); }
+    static __device__ __forceinline__ int slot(int s, int h) { return 4 * slot_freq<NL>(s) + (h >> 1) + 2 * (h & 1); }
+    // exp(SIGN 2 pi i h / 8): the part of the first-stage twiddle exp(SIGN 2 pi i (h Q + i) / N) that depends on the lane
+    template <int SIGN> static __device__ __forceinline__ cx<T> lane_tw(int h)
+    {
+        const T r = (T)0.70710678118654752440;
+        const T re = h == 0 ? (T)1 : (h == 1 ? r : (h == 2 ? (T)0 : -r));
+        const T im = h == 0 ? (T)0 : (h == 2 ? (T)1 : r);
+        return mk<T>(re, SIGN > 0 ? im : -im);
+    }
+    template <int SIGN> static __device__ __forceinline__ void dif(cx<T> (&v)[NL], int h, unsigned mask)
+    {
+        const int a = h >> 1, b = h & 1;
+        const cx<T> lt = lane_tw<SIGN>(h);
+#pragma unroll
+        for (int i = 0; i < Q; i++) {                        // stage 1 on N points, exchange across bit a
+            const cx<T> p = v[i], q = v[Q + i];
+            const cx<T> y = p + q;
+            const cx<T> z = cmul(mul_tw<T, N, SIGN>(p - q, i), lt);
+            const cx<T> got = shfl16(mask, a ? y : z);
+            v[i] = a ? got : y;
+            v[Q + i] = a ? z : got;
+        }
+#pragma unroll
+        for (int i = 0; i < Q; i++) {                        // stage 2 on N/2 points, exchange across bit b
+            const cx<T> p = v[i], q = v[Q + i];
+            const cx<T> y = p + q;
+            cx<T> z = mul_tw<T, M, SIGN>(p - q, i);
+            if (b) z = rot90<SIGN>(z);
+            const cx<T> got = shfl8(mask, b ? y : z);
+            v[i] = b ? got : y;
+            v[Q + i] = b ? z : got;
+        }
+        Dif<T, NL, NL, SIGN>::run(v);
+    }
+    template <int SIGN> static __device__ __forceinline__ void dit(cx<T> (&v)[NL], int h, unsigned mask)
+    {
+        const int a = h >> 1, b = h & 1;
+        const cx<T> lt = lane_tw<SIGN>(h);
+        Dit<T, NL, NL, SIGN>::run(v);
+#pragma unroll
+        for (int i = 0; i < Q; i++) {
+            const cx<T> got = shfl8(mask, b ? v[i] : v[Q + i]);
+            const cx<T> y = b ? got : v[i];
+            cx<T> z = b ? v[Q + i] : got;
+            z = mul_tw<T, M, SIGN>(z, i);
+            if (b) z = rot90<SIGN>(z);
+            v[i] = y + z;
+            v[Q + i] = y - z;
+        }
+#pragma unroll
+        for (int i = 0; i < Q; i++) {
+            const cx<T> got = shfl16(mask, a ? v[i] : v[Q + i]);
+            const cx<T> y = a ? got : v[i];
+            cx<T> z = a ? v[Q + i] : got;
+            z = cmul(mul_tw<T, N, SIGN>(z, i), lt);
+            v[i] = y + z;
+            v[Q + i] = y - z;
+        }
+    }
+};
+
+// thread t of a group -> (line, part).  S = 2 keeps the two halves of a line 16 lanes apart (S = 4: the four
+// quarters 8 lanes apart), so that the 8 lanes of a shared-memory wavefront still belong to 8 consecutive lines.
 template <int S> __device__ __forceinline__ void line_of_thread(int t, int &line, int &h)
 {
     if (S == 1) { line = t; h = 0; }
-    else { h = (t >> 4) & 1; line = (t & 15) | ((t >> 5) << 4); }
+    else if (S == 2) { h = (t >> 4) & 1; line = (t & 15) | ((t >> 5) << 4); }
+    else { h = (t >> 3) & 3; line = (t & 7) | ((t >> 5) << 3); }
 }
 // Lines of at least SMIN points are shared by two lanes.  48 and 64 must be (registers).  32-point
 // lines are split for FP64 tiles with NA == NB only: a same-run A/B at 32^4 FP64 gave 0.3164 against
 // 0.3279 ms per iteration (twice the warps per tile at 84-128 instead of 146-196 registers), while FP32
 // tiles and the (32, 48) / (32, 64) (z,t) tiles of 32^3 x n lattices got 5-15 % slower
 // (profiles/r01e_final.md).  LGF_SPLIT_MIN overrides the rule for tuning sweeps.
-#ifdef LGF_SPLIT_MIN
-template <typename T> constexpr int split_min(int, int) { return LGF_SPLIT_MIN; }
-#else
-template <typename T> constexpr int split_min(int na, int nb) { return (sizeof(T) == 8 && na == nb) ? 32 : 48; }
+// LGF_SPLIT4_MIN: lines of at least that many points are shared by four lanes (FP64 tiles with NA == NB only; 0 = never).
+#ifndef LGF_SPLIT4_MIN
+#define LGF_SPLIT4_MIN 0
 #endif
-constexpr int split_of(int n, int smin) { return n >= smin ? 2 : 1; }
+#ifdef LGF_SPLIT_MIN
+template <typename T> constexpr int split_min2(int, int) { return LGF_SPLIT_MIN; }
+#else
+template <typename T> constexpr int split_min2(int na, int nb) { return (sizeof(T) == 8 && na == nb) ? 32 : 48; }
+#endif
+// the two thresholds packed into one template argument: (four-lane threshold << 8) | two-lane threshold
+template <typename T> constexpr int split_min(int na, int nb)
+{
+    return ((sizeof(T) == 8 && na == nb && LGF_SPLIT4_MIN > 0 ? LGF_SPLIT4_MIN : 255) << 8) | split_min2<T>(na, nb);
+}
+constexpr int split_of(int n, int smin) { return n >= (smin >> 8) ? 4 : (n >= (smin & 255) ? 2 : 1); }
 
 // ---------------------------------------------------------------- tile geometry
 // Shared tile of a group: element (c, a, b) at (b*RS + a*C + c), RS = NA*C + C (one padding

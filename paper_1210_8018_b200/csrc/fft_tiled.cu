@@ -40,8 +40,11 @@ template <typename T, int NA, int NB> struct XYCfg {
 
 // AX = 0: both axes (the pass of the 3- and 4-pass structures).  AX = 1 / 2: the x-lines / y-lines alone, the
 // 1D passes of the 4 x 1D structure of the paper's comparison (LGF_OPT_FFT_PASSES = 8).
+#ifndef LGF_XY_MINB
+#define LGF_XY_MINB 1   /* minimum CTAs per SM asked of the (x,y) passes (register cap); tuning macro */
+#endif
 template <typename T, int NA, int NB, int INVERSE, int AX = 0>
-__global__ void __launch_bounds__((XYCfg<T, NA, NB>::CTA))
+__global__ void __launch_bounds__((XYCfg<T, NA, NB>::CTA), LGF_XY_MINB)
 k_fft_xy(cx<T> *__restrict__ w, int64_t nplanes, const Ctrl *ctrl)
 {
     if (*(volatile const int *)&ctrl->done) return;

@@ -159,18 +159,21 @@ __device__ __forceinline__ double store_delta(const T (&di)[3], const cx<T> (&E)
 #ifndef LGF_ACC_MINB
 #define LGF_ACC_MINB(NE, T) ((NE) == 9 && sizeof(T) == 8 ? 3 : 4)
 #endif
-template <typename T, int NE, int PACK, bool GBUF, bool STORE>
+// MARCH (LGF_OPT_TMARCH > 1): the thread walks tk consecutive time slices; a separate instantiation, so that the
+// one-site form keeps its registers.
+template <typename T, int NE, int PACK, bool GBUF, bool STORE, bool MARCH = false>
 __global__ void __launch_bounds__(FUSED_THREADS, (STORE ? LGF_FUSED_MINB : LGF_ACC_MINB(NE, T)))
 k_update_measure(const cx<T> *__restrict__ lin, cx<T> *__restrict__ lout, const cx<T> *__restrict__ gsrc,
-                 cx<T> *__restrict__ wout, Geom geo, T a, int gexp, Ctrl *ctrl, double *partials, double2 *hist, double eps)
+                 cx<T> *__restrict__ wout, Geom geo, T a, int gexp, Ctrl *ctrl, double *partials, double2 *hist, double eps, int tk_arg)
 {
+    const int tk = MARCH ? tk_arg : 1;
     if (*(volatile int *)&ctrl->done) return;
     const int64_t V = geo.V;
     const int64_t rr = (int64_t)blockIdx.x * FUSED_THREADS + threadIdx.x;
     double trF = 0, th = 0;
-    if (rr < geo.Vw) {
+    if (rr < geo.Vw / tk) {
         int c[4];
-        const int64_t s = walk_site(geo, rr, c);     // (z,t)-blocked walk: neighbour re-reads stay in L2
+        int64_t s = walk_site(geo, rr, c, tk);       // (z,t)-blocked walk: neighbour re-reads stay in L2
         if (!STORE && LGF_ACC_QSUM(NE)) {
             // ACCUM_G: nothing is stored, so the forward links enter only through their sum as well,
             //     sum_mu U'_mu(x) = G(x) [sum_mu U_mu(x) G^dagger(x+mu)]:
@@ -231,6 +234,11 @@ k_update_measure(const cx<T> *__restrict__ lin, cx<T> *__restrict__ lout, const 
 #pragma unroll
             for (int k = 0; k < 4 * NE; k++) asm volatile("prefetch.global.L2 [%0];" ::"l"(lin + (int64_t)k * V + s));
 #endif
+            // LGF_OPT_TMARCH: the thread walks tk consecutive time slices.  The -t neighbour of its second, third ...
+            // site is its own previous site, whose H_t = g U_t it has just formed for the forward product
+            // (Tc below): 12 loads and one product less per site after the first.
+            cx<T> Tc[6];
+          for (int kk = 0; kk < tk; kk++) {
             // Backward links first: only their sum enters A'(x),
             //     sum_nu U'_nu(x-nu) = [sum_nu H_nu(x-nu)] g^dagger(x),   H_nu(y) = g(y) U_nu(y),
             // so rows 0, 1 of each H are one product, row 2 is conj(row0 x row1) (H is special
@@ -242,10 +250,16 @@ k_update_measure(const cx<T> *__restrict__ lin, cx<T> *__restrict__ lout, const 
             for (int q = 0; q < 4; q++) {
                 const int nu = LGF_FUSED_BWD_REV ? 3 - q : q;
                 const int64_t sb = s + (c[nu] == 0 ? (int64_t)(geo.N[nu] - 1) : (int64_t)-1) * geo.st[nu];
-                cx<T> gb[9], u[9], h[9];
-                load_g01<T, PACK, GBUF>(gsrc, V, sb, a, gexp, gb);
-                load_link_in<T, NE>(lin, V, nu, sb, u);
-                mul_rows<2>(gb, u, h);
+                cx<T> h[9];
+                if (MARCH && nu == 3 && kk > 0) {
+#pragma unroll
+                    for (int k = 0; k < 6; k++) h[k] = Tc[k];
+                } else {
+                    cx<T> gb[9], u[9];
+                    load_g01<T, PACK, GBUF>(gsrc, V, sb, a, gexp, gb);
+                    load_link_in<T, NE>(lin, V, nu, sb, u);
+                    mul_rows<2>(gb, u, h);
+                }
                 su3_row2(h);
 #pragma unroll
                 for (int k = 0; k < 9; k++) X[k] = X[k] + h[k];
@@ -271,6 +285,10 @@ k_update_measure(const cx<T> *__restrict__ lin, cx<T> *__restrict__ lout, const 
                 su3_row2(g1);
                 load_link_in<T, NE>(lin, V, mu, s, u);
                 mul_rows<2>(g0, u, t);
+                if (MARCH && mu == 3) {
+#pragma unroll
+                    for (int k = 0; k < 6; k++) Tc[k] = t[k];
+                }
                 mul_rows_dag<2>(t, g1, r);
                 su3_row2(r);
                 if (STORE) {
@@ -281,8 +299,11 @@ k_update_measure(const cx<T> *__restrict__ lin, cx<T> *__restrict__ lout, const 
                 tr += r[0].x + r[4].x + r[8].x;
                 acc_ah<T>(r, (T)-1, di, E);
             }
-            trF = (double)tr;
-            th = store_delta<T, PACK>(di, E, wout, V, s);
+            trF += (double)tr;
+            th += store_delta<T, PACK>(di, E, wout, V, s);
+            s += geo.st[3];
+            c[3] += 1;
+          }
         }
     }
     finish_measure<FUSED_THREADS>(trF, th, geo.Vg, ctrl, partials, hist, eps, 1);
@@ -301,7 +322,10 @@ template <typename T, int NE, int PACK, bool GBUF, bool STORE> static void prefe
     static bool done = false;
     if (done) return;
     done = true;
-    if (cudaFuncSetAttribute(k_update_measure<T, NE, PACK, GBUF, STORE>, cudaFuncAttributePreferredSharedMemoryCarveout,
+    if (cudaFuncSetAttribute(k_update_measure<T, NE, PACK, GBUF, STORE, false>, cudaFuncAttributePreferredSharedMemoryCarveout,
+                             (int)cudaSharedmemCarveoutMaxL1) != cudaSuccess)
+        cudaGetLastError();
+    if (cudaFuncSetAttribute(k_update_measure<T, NE, PACK, GBUF, STORE, true>, cudaFuncAttributePreferredSharedMemoryCarveout,
                              (int)cudaSharedmemCarveoutMaxL1) != cudaSuccess)
         cudaGetLastError();
 #endif
@@ -310,11 +334,14 @@ template <typename T, int NE, int PACK, bool GBUF, bool STORE> static void prefe
 void launch_update_measure(const SiteArgs &a, const void *lin, void *lout, const void *gsrc, int gbuf, void *wout,
                            double alpha, double eps, cudaStream_t st)
 {
-    const int nb = fused_blocks(a.geo.Vw);
+    const int tk = a.tmarch > 0 ? a.tmarch : 1;
+    const int nb = fused_blocks(a.geo.Vw / tk);
 #define CALL(T, NE, PACK, GB) \
     do { prefer_l1<T, NE, PACK, GB, true>();   \
-    k_update_measure<T, NE, PACK, GB, true><<<nb, FUSED_THREADS, 0, st>>>((const cx<T> *)lin, (cx<T> *)lout, (const cx<T> *)gsrc, \
-        (cx<T> *)wout, a.geo, (T)(alpha / 2.0), a.gexp, a.ctrl, a.partials, a.hist, eps); } while (0)
+    if (tk > 1) k_update_measure<T, NE, PACK, GB, true, true><<<nb, FUSED_THREADS, 0, st>>>((const cx<T> *)lin, (cx<T> *)lout, (const cx<T> *)gsrc, \
+        (cx<T> *)wout, a.geo, (T)(alpha / 2.0), a.gexp, a.ctrl, a.partials, a.hist, eps, tk); \
+    else k_update_measure<T, NE, PACK, GB, true, false><<<nb, FUSED_THREADS, 0, st>>>((const cx<T> *)lin, (cx<T> *)lout, (const cx<T> *)gsrc, \
+        (cx<T> *)wout, a.geo, (T)(alpha / 2.0), a.gexp, a.ctrl, a.partials, a.hist, eps, 1); } while (0)
 #define CALL_NE(T, NE)                                           \
     do {                                                         \
         if (gbuf) { CALL(T, NE, 4, true); }                      \
@@ -329,11 +356,15 @@ void launch_update_measure(const SiteArgs &a, const void *lin, void *lout, const
 
 void launch_measure_acc(const SiteArgs &a, const void *gacc, double eps, cudaStream_t st)
 {
-    const int nb = fused_blocks(a.geo.Vw);
+    // the 18-real form sums the forward links first (LGF_ACC_QSUM) and walks one site per thread
+    const int tk = (a.tmarch > 0 && !(LGF_ACC_QSUM(a.recon == 12 ? 6 : 9))) ? a.tmarch : 1;
+    const int nb = fused_blocks(a.geo.Vw / tk);
 #define CALL(T, NE) \
     do { prefer_l1<T, NE, 4, true, false>();  \
-    k_update_measure<T, NE, 4, true, false><<<nb, FUSED_THREADS, 0, st>>>((const cx<T> *)a.links, (cx<T> *)nullptr, \
-        (const cx<T> *)gacc, (cx<T> *)a.w, a.geo, (T)0, 0, a.ctrl, a.partials, a.hist, eps); } while (0)
+    if (tk > 1) k_update_measure<T, NE, 4, true, false, true><<<nb, FUSED_THREADS, 0, st>>>((const cx<T> *)a.links, (cx<T> *)nullptr, \
+        (const cx<T> *)gacc, (cx<T> *)a.w, a.geo, (T)0, 0, a.ctrl, a.partials, a.hist, eps, tk); \
+    else k_update_measure<T, NE, 4, true, false, false><<<nb, FUSED_THREADS, 0, st>>>((const cx<T> *)a.links, (cx<T> *)nullptr, \
+        (const cx<T> *)gacc, (cx<T> *)a.w, a.geo, (T)0, 0, a.ctrl, a.partials, a.hist, eps, 1); } while (0)
     if (a.prec == 0) { if (a.recon == 12) CALL(double, 6); else CALL(double, 9); }
     else             { if (a.recon == 12) CALL(float, 6); else CALL(float, 9); }
 #undef CALL

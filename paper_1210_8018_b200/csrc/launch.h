@@ -15,6 +15,7 @@ struct SiteArgs {
     int recon;          // 18 or 12
     int pack;           // 4 or 9
     int gexp;           // LGF_OPT_GMAP: 0 first order + reunitarisation, 1 exact exponential
+    int tmarch;         // LGF_OPT_TMARCH: consecutive time slices per thread of the link kernel (1, 2 or 4; divides Ntw)
 };
 
 // kernel (a): Delta, F, theta (eq. 1.5, 1.1, 1.4).  eps < 0: never raise `done`.

@@ -42,6 +42,7 @@ struct lgf_ctx {
     int zblock = 0;          // LGF_OPT_ZBLOCK: 0 = auto (resolved by lgf_bind into sa.geo.zb)
     int zt_pipe = 0;         // LGF_OPT_ZT_PIPE
     int fft_passes = 3;      // LGF_OPT_FFT_PASSES: 3 (fused middle), 4 (2D + 2D), 8 (4 x 1D)
+    int tmarch = 0;          // LGF_OPT_TMARCH: time slices per thread of the link kernel (0 = auto)
     // one lattice sharded in t-slabs over shard_world ranks (0 = off): V = sites of the interchange arrays (the
     // rank's own time slices), Vp = stored sites (with the two halo slices), Vg = sites of the whole lattice
     int shard_world = 0, shard_rank = 0;
@@ -474,7 +475,7 @@ int lgf_set_option(lgf_ctx *ctx, int key, int64_t value)
     if (!ctx) return LGF_ERR_INVALID_ARG;
     const bool layout_key = (key == LGF_OPT_RECON || key == LGF_OPT_FFT_BATCH || key == LGF_OPT_FFT_PATH || key == LGF_OPT_FUSION ||
                              key == LGF_OPT_L2_PERSIST || key == LGF_OPT_ACCUM_G || key == LGF_OPT_ZBLOCK || key == LGF_OPT_FFT_PASSES ||
-                             key == LGF_OPT_SHARD_WORLD || key == LGF_OPT_SHARD_RANK);
+                             key == LGF_OPT_SHARD_WORLD || key == LGF_OPT_SHARD_RANK || key == LGF_OPT_TMARCH);
     if (layout_key && ctx->bound) return fail(ctx, LGF_ERR_INVALID_ARG, "this option must be set before lgf_bind");
     switch (key) {
     case LGF_OPT_RECON:
@@ -513,6 +514,9 @@ int lgf_set_option(lgf_ctx *ctx, int key, int64_t value)
     case LGF_OPT_FFT_PASSES:
         if (value != 3 && value != 4 && value != 8) return fail(ctx, LGF_ERR_INVALID_ARG, "FFT_PASSES must be 3, 4 or 8");
         ctx->fft_passes = (int)value; break;
+    case LGF_OPT_TMARCH:
+        if (value != 0 && value != 1 && value != 2 && value != 4) return fail(ctx, LGF_ERR_INVALID_ARG, "TMARCH must be 0 (auto), 1, 2 or 4");
+        ctx->tmarch = (int)value; break;
     case LGF_OPT_SHARD_WORLD:
         if (value < 0 || (value > 0 && (ctx->N[3] % value != 0 || ctx->N[1] % value != 0)))
             return fail(ctx, LGF_ERR_INVALID_ARG, "SHARD_WORLD must be 0 (off) or divide Nt and Ny");
@@ -574,6 +578,10 @@ int lgf_bind(lgf_ctx *ctx, void *dev_workspace, size_t bytes, void *cuda_stream)
     g.V = ctx->Vp; g.Vw = ctx->V; g.Vg = ctx->Vg;
     SiteArgs &s = ctx->sa;
     s.geo = g;
+    // auto: measured on B200 (profiles/r02_link_kernel.md) FP32 gains 3 % with 4 slices per thread, FP64 loses 15 % (the
+    // carried product costs registers the FP64 kernel does not have: 364 B of spills); the walked slices must split into whole groups
+    const int want = ctx->tmarch > 0 ? ctx->tmarch : ((ctx->prec == LGF_PREC_FP32 && !ctx->accum) ? 4 : 1);
+    s.tmarch = (g.Ntw % want == 0) ? want : 1;
     for (int i = 0; i < 2; i++) { ctx->links_buf[i] = ctx->base + L.links[i]; ctx->w_buf[i] = ctx->base + L.w[i]; }
     ctx->gbuf = ctx->base + L.gbuf;
     ctx->cur = 0; ctx->wcur = 0;

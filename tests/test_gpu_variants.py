@@ -469,3 +469,69 @@ def test_fft_passes_validation(lgf):
         lgf.GaugeFixer(8, fft_passes=8, accum_g=1)
     gf = lgf.GaugeFixer(8, fft_passes=4, accum_g=1)           # 2D + 2D keeps the g-building last pass
     gf.close()
+
+
+# ------------------------------------------------------------------ 18-real storage and links that are not exactly SU(3)
+def test_18_real_fused_path_projects_row_2_as_documented(lgf):
+    """include/lgf.h (LGF_OPT_RECON) and DESIGN.md reading R15: links must be SU(3) to working precision.  With a
+    deliberately non-unitary third row, FUSION = 0 multiplies all three rows like the oracle, while the fused kernel
+    stores row 2 of g U g^dagger as conj(row0 x row1) of the product: rows 0, 1 agree with the oracle either way, row 2
+    of the fused path differs by the size of the defect.  For exactly special unitary links both agree (other tests)."""
+    N = (8, 8, 8, 8)
+    U = gen.gen_links(N, 0.3, 31)
+    U[:, :, 2, :] *= 1.0 + 1e-6                      # row 2 no longer conj(row0 x row1): defect 1e-6
+    Uo = U.copy()
+    oracle.iterate(N, Uo, ALPHA, 1)
+    unf = lgf.GaugeFixer(N, recon=18, fusion=0)
+    unf.load_links(U)
+    unf.iterate(ALPHA, 1)
+    assert np.abs(unf.get_links() - Uo).max() < 1e-12
+    fus = lgf.GaugeFixer(N, recon=18)
+    fus.load_links(U)
+    fus.iterate(ALPHA, 1)
+    Uf = fus.get_links()
+    # rows 0, 1 of g U g^dagger only need rows 0, 1 of g and all of U ... whose row 2 enters through U g^dagger: first order in the defect
+    assert np.abs(Uf[:, :, :2, :] - Uo[:, :, :2, :]).max() < 5e-6
+    d2 = np.abs(Uf[:, :, 2, :] - Uo[:, :, 2, :]).max()
+    assert 1e-7 < d2 < 5e-6                         # the projection is visible and of the size of the defect
+
+
+# ------------------------------------------------------------------ LGF_OPT_TMARCH: several time slices per thread
+@pytest.mark.parametrize("var", [dict(recon=12), dict(recon=18), dict(recon=18, precision="fp32"), dict(recon=12, accum_g=1),
+                                 dict(recon=18, fft_batch=9), dict(recon=12, zblock=2)], ids=vid)
+@pytest.mark.parametrize("tk", [2, 4])
+def test_tmarch_gives_the_same_links(lgf, var, tk):
+    """A thread of the link kernel that walks tk time slices takes the -t neighbour of its later sites from its own
+    previous site: same products, so the links after 3 iterations are bitwise those of one site per thread, F and theta
+    agree to the rounding of the partial sums, and the first iteration matches the oracle."""
+    N = (8, 8, 8, 12) if tk == 4 else (8, 8, 8, 6)
+    if var.get("accum_g") and N[3] == 6:
+        N = (8, 8, 8, 8)
+    fp32 = var.get("precision") == "fp32"
+    U = gen.gen_links(N, 0.5, 606)
+    Uo = U.copy()
+    hist = oracle.iterate(N, Uo, ALPHA, 1)
+    Uin = U.astype(np.complex64) if fp32 else U
+    res = []
+    for t in (1, tk):
+        gf = lgf.GaugeFixer(N, tmarch=t, **var)
+        gf.load_links(Uin)
+        r1 = gf.iterate(ALPHA, 1)
+        assert np.abs(gf.get_links().astype(np.complex128) - Uo).max() < (1e-5 if fp32 else 1e-12)
+        assert abs(r1.theta - hist[1, 1]) <= (1e-4 if fp32 else 1e-10) * hist[1, 1]
+        r3 = gf.iterate(ALPHA, 2)
+        res.append((gf.get_links(), r3.F, r3.theta))
+        gf.close()
+    assert np.array_equal(res[0][0], res[1][0])
+    assert abs(res[0][1] - res[1][1]) <= (1e-7 if fp32 else 1e-14) and abs(res[0][2] - res[1][2]) <= (1e-6 if fp32 else 1e-13) * res[0][2]
+
+
+def test_tmarch_falls_back_when_it_does_not_divide(lgf):
+    with pytest.raises(lgf.LgfError):
+        lgf.GaugeFixer(8, tmarch=3)
+    N = (8, 8, 8, 6)                                  # 4 does not divide Nt = 6: one site per thread
+    U = gen.gen_links(N, 0.5, 607)
+    a, b = lgf.GaugeFixer(N, tmarch=4), lgf.GaugeFixer(N, tmarch=1)
+    a.load_links(U); b.load_links(U)
+    ra, rb = a.iterate(ALPHA, 2), b.iterate(ALPHA, 2)
+    assert ra.F == rb.F and ra.theta == rb.theta and np.array_equal(a.get_links(), b.get_links())
