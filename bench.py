@@ -149,6 +149,13 @@ def ncu_traffic(workload_key, kernel):
                                            capture_output=True, text=True, timeout=10).stdout.strip() or None
         except (OSError, subprocess.SubprocessError):
             src["commit"] = None
+        if not src["commit"]:           # no git history here (GPU boxes): the "commit:" line of the .md beside the csv
+            try:
+                for line in open(os.path.join(ROOT, src["file"][:-4] + ".md")):
+                    if line.startswith("commit:"):
+                        src["commit"] = line.split()[1]
+            except OSError:
+                pass
     return best, src
 
 
@@ -329,6 +336,32 @@ def run_ours(args):
     gf.get_links(out=host_out.numpy())
     torch.cuda.synchronize()
     fix_e2e_s = time.perf_counter() - tf2
+    # the same steps for a STREAM of lattices (ensembles are the use case): three contexts, streams and host
+    # threads, so that the upload of one lattice, the kernels of another and the download of a third overlap (ensemble.py)
+    pipe_s = pipe_fix_s = None
+    if args.pipeline and world == 1 and V <= 48 ** 4:          # 64^4 would pin another 30 GB of host memory for the three slots
+        try:
+            from paper_1210_8018_b200 import ensemble
+
+            ens = ensemble.EnsembleFixer(N, slots=3, precision=prec, recon=recon, fft_batch=args.fft_batch, device=f"cuda:{local}")
+            pouts = [torch.empty_like(host).pin_memory() for _ in range(3)]
+            ens.run([host.numpy()] * 3, [p.numpy() for p in pouts], ALPHA, iterations=1)          # warm-up
+            torch.cuda.synchronize()
+            tp = time.perf_counter()
+            ens.run([host.numpy()] * e2e_steps, [pouts[k % 3].numpy() for k in range(e2e_steps)], ALPHA, iterations=1)
+            torch.cuda.synchronize()
+            pipe_s = time.perf_counter() - tp
+            # and the time to solution for a stream of lattices: load, lgf_fix, get per lattice, three in flight
+            nfix = 12
+            tq = time.perf_counter()
+            rq = ens.run([host.numpy()] * nfix, [pouts[k % 3].numpy() for k in range(nfix)], ALPHA, fix_eps)
+            torch.cuda.synchronize()
+            pipe_fix_s = (time.perf_counter() - tq, nfix, int(rq[0].iterations))
+            ens.close()
+            del pouts
+        except Exception as e:                                  # noqa: BLE001
+            pipe_s = None
+            sys.stderr.write(f"bench.py: pipelined e2e leg skipped: {e}\n")
     clocks = sampler.stop(t0, t1) if sampler else None
     try:
         dfma_rate = lgf.debug_dfma_rate(stream.cuda_stream)     # measured FP64 FMA rate: the "alu" denominator
@@ -452,10 +485,18 @@ def run_ours(args):
                 "ms_per_step": 1e3 * e2e_all / e2e_steps,
                 "what": "every step: lgf_load_links(pinned host, " + ("12-real rows 0-1 layout" if per_link == 6 else "18-real layout")
                         + ") + lgf_iterate(1) with its (iterations, F, theta) readback + lgf_get_links(pinned host, same layout)",
+                "pipelined": (None if pipe_s is None else
+                              {"what": "the same step (load, one iteration, get) for a stream of lattices through ensemble.EnsembleFixer: 3 contexts, "
+                                       "streams and host threads on this GPU, transfers of different lattices overlapped",
+                               "value": V * e2e_steps / pipe_s, "unit": UNIT, "ms_per_step": 1e3 * pipe_s / e2e_steps}),
                 "fix": {"what": "time to solution through the same calls: lgf_load_links(host) + lgf_fix(alpha, eps) + lgf_get_links(host)",
                         "eps": fix_eps, "iterations": int(r_fix2.iterations), "converged": int(r_fix2.converged),
                         "ms": 1e3 * fix_e2e_all, "value": world * V * int(r_fix2.iterations) / fix_e2e_all, "unit": UNIT,
-                        "h2d_bytes": h2d, "d2h_bytes": h2d + 32}},
+                        "h2d_bytes": h2d, "d2h_bytes": h2d + 32,
+                        "pipelined": (None if pipe_fix_s is None else
+                                      {"what": f"{pipe_fix_s[1]} lattices through ensemble.EnsembleFixer (3 in flight), each load + lgf_fix + get",
+                                       "ms_per_lattice": 1e3 * pipe_fix_s[0] / pipe_fix_s[1], "iterations": pipe_fix_s[2],
+                                       "value": V * pipe_fix_s[2] * pipe_fix_s[1] / pipe_fix_s[0], "unit": UNIT})}},
         "gpu_launches": int(launches),
         "roofline": {"bound": "hbm", "kernel": dom, "achieved": kern[dom]["GBps"], "peak": peak, "unit": "GB/s",
                      "frac": kern[dom]["GBps"] / peak,
@@ -547,6 +588,7 @@ def main():
     ap.add_argument("--gmap", type=int, default=0, choices=[0, 1], help="LGF_OPT_GMAP: 1 = exact exponential")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cufft-reference", type=int, default=1, choices=[0, 1])
+    ap.add_argument("--pipeline", type=int, default=1, choices=[0, 1], help="also time the e2e step for a stream of lattices (ensemble.py)")
     ap.add_argument("--zblock", type=int, default=None, help="LGF_OPT_ZBLOCK (default: chosen from the L2 size)")
     ap.add_argument("--zt-pipe", type=int, default=None, choices=[0, 1], help="LGF_OPT_ZT_PIPE")
     ap.add_argument("--launch-selftest", action="store_true", help="start the ranks, reduce one timing, print the rank count")

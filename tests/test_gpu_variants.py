@@ -535,3 +535,29 @@ def test_tmarch_falls_back_when_it_does_not_divide(lgf):
     a.load_links(U); b.load_links(U)
     ra, rb = a.iterate(ALPHA, 2), b.iterate(ALPHA, 2)
     assert ra.F == rb.F and ra.theta == rb.theta and np.array_equal(a.get_links(), b.get_links())
+
+
+# ------------------------------------------------------------------ ensemble.py: lattices pipelined through one GPU
+def test_ensemble_pipeline_equals_one_lattice_at_a_time(lgf):
+    """Seven different lattices through three slots (three contexts, streams and host threads): results and links
+    are those of one context fixing them one after another, bitwise, and the first one matches the golden count."""
+    import torch
+
+    from paper_1210_8018_b200 import ensemble
+
+    n = 8
+    seeds = [gen.BASE_SEED + 8] + list(range(700, 706))
+    ins = [torch.from_numpy(gen.gen_links(n, 0.3, s)).pin_memory() for s in seeds]
+    outs = [torch.empty_like(t).pin_memory() for t in ins]
+    ens = ensemble.EnsembleFixer(n, slots=3, recon=12)
+    res = ens.run([t.numpy() for t in ins], [t.numpy() for t in outs], ALPHA, 1e-15)
+    ens.close()
+    it, F, th, hist = read_golden(golden_path(n, seeds[0]))
+    assert res[0].iterations == it and abs(res[0].F - F) <= 1e-10
+    gf = lgf.GaugeFixer(n, recon=12)
+    for t, o, r in zip(ins, outs, res):
+        gf.load_links(t.numpy())
+        r1 = gf.fix(ALPHA, 1e-15)
+        assert (r1.iterations, r1.F, r1.theta, r1.converged) == (r.iterations, r.F, r.theta, r.converged)
+        assert np.array_equal(gf.get_links(), o.numpy())
+    gf.close()
