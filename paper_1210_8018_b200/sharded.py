@@ -74,8 +74,15 @@ class TorchDistComm:
         self.rank = dist.get_rank(group)
         self.local_ranks = [self.rank]
 
+    @staticmethod
+    def _bytes(t):
+        """Transport view: collectives move bytes, whatever the element type (complex tensors are not supported by every backend)."""
+        import torch
+
+        return t.view(torch.uint8) if t.is_complex() else t
+
     def all_to_all(self, dst, src):
-        self.dist.all_to_all_single(dst[0], src[0], group=self.group)
+        self.dist.all_to_all_single(self._bytes(dst[0]), self._bytes(src[0]), group=self.group)
 
     def halo(self, to_lower, to_upper, from_upper, from_lower):
         dist, R, r = self.dist, self.world, self.rank
@@ -83,14 +90,15 @@ class TorchDistComm:
         ops = []
         # per peer, sends and receives are matched in the order they are posted; with R = 2 both neighbours
         # are the same rank, and its first message (its to_lower) is this rank's from_upper
+        B = self._bytes
         if to_lower is not None:
-            ops.append(dist.P2POp(dist.isend, to_lower[0], lo, group=self.group))
+            ops.append(dist.P2POp(dist.isend, B(to_lower[0]), lo, group=self.group))
         if to_upper is not None:
-            ops.append(dist.P2POp(dist.isend, to_upper[0], up, group=self.group))
+            ops.append(dist.P2POp(dist.isend, B(to_upper[0]), up, group=self.group))
         if to_lower is not None:
-            ops.append(dist.P2POp(dist.irecv, from_upper[0], up, group=self.group))
+            ops.append(dist.P2POp(dist.irecv, B(from_upper[0]), up, group=self.group))
         if to_upper is not None:
-            ops.append(dist.P2POp(dist.irecv, from_lower[0], lo, group=self.group))
+            ops.append(dist.P2POp(dist.irecv, B(from_lower[0]), lo, group=self.group))
         for w in dist.batch_isend_irecv(ops):
             w.wait()
 
@@ -251,6 +259,6 @@ def exchange_selftest(comm, world, rank_data):
     fu = [torch.empty_like(x) for x in lo]
     fl = [torch.empty_like(x) for x in up]
     comm.halo(lo, up, fu, fl)
-    tot = [d[0].sum().reshape(1).clone() for d in rank_data]
+    tot = [d[0].real.sum().reshape(1).clone() if d[0].is_complex() else d[0].sum().reshape(1).clone() for d in rank_data]
     comm.all_reduce_sum(tot)
     return [(r.view(world, -1), a, b, t) for r, a, b, t in zip(recv, fu, fl, tot)]

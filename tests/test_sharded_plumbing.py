@@ -24,7 +24,8 @@ def _rank_data(world, r, n=6, h=5):
     blocks = torch.arange(world * n, dtype=torch.float64).view(world, n) + 1000.0 * r
     to_lower = torch.arange(h, dtype=torch.float64) + 100.0 * r + 0.25
     to_upper = torch.arange(h, dtype=torch.float64) + 100.0 * r + 0.75
-    return blocks, to_lower, to_upper
+    # complex, as the fields and links are: the transport must not depend on the element type
+    return torch.complex(blocks, -blocks), torch.complex(to_lower, to_upper), torch.complex(to_upper, to_lower)
 
 
 def _worker(rank, world, port, out):
@@ -63,7 +64,7 @@ def test_in_process_reference_is_what_the_layout_needs():
         for q in range(world):
             assert torch.equal(recv[q], data[q][0][r])
         assert torch.equal(fu, data[(r + 1) % world][1]) and torch.equal(fl, data[(r - 1) % world][2])
-        assert tot.item() == sum(d[0].sum().item() for d in data)
+        assert tot.item() == sum(d[0].real.sum().item() for d in data)
 
 
 def test_slab_of_takes_whole_time_slices():
