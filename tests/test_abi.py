@@ -109,3 +109,56 @@ def test_product_path_does_not_touch_the_oracle():
                 src = open(os.path.join(dirpath, f)).read()
                 assert not re.search(r"^\s*(import|from)\s+(oracle|gen)\b", src, flags=re.M), f
                 assert "lgf_oracle" not in src and "orc_" not in src, f
+
+
+def header_enums():
+    """NAME = value pairs of every enum of include/lgf.h."""
+    src = open(os.path.join(ROOT, "include", "lgf.h")).read()
+    src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
+    return {m.group(1): int(m.group(2)) for m in re.finditer(r"\b(LGF_[A-Z0-9_]+)\s*=\s*(-?\d+)", src)}
+
+
+def test_binding_constants_equal_the_header_enums():
+    from paper_1210_8018_b200 import lgf
+
+    enums = header_enums()
+    assert len(enums) >= 60
+    checked = 0
+    for name, value in enums.items():
+        short = name[len("LGF_"):]
+        if hasattr(lgf, short):
+            assert getattr(lgf, short) == value, name
+            checked += 1
+    # every option, shard step and region the binding offers is one the header declares, with the same value
+    assert checked >= 45
+    for short in dir(lgf):
+        if short.startswith(("OPT_", "SHARD_", "REGION_", "ERR_", "STAGE_", "FIELD_", "LAYOUT_", "PREC_")):
+            assert "LGF_" + short in enums, short
+    assert len(lgf.KERNEL_NAMES) == enums["LGF_KERNEL_KINDS"]
+
+
+def test_round_2_options_validate_on_the_host(L):
+    from paper_1210_8018_b200 import lgf
+
+    ctx = ctypes.c_void_p()
+    assert L.lgf_create(16, 16, 12, 24, lgf.PREC_FP64, ctypes.byref(ctx)) == lgf.OK
+    for key, good, bad in [(lgf.OPT_ZBLOCK, [0, 1, 3, 12], [-1, 5, 24]), (lgf.OPT_ZT_PIPE, [0, 1], [2]),
+                           (lgf.OPT_FFT_PASSES, [3, 4, 8], [0, 2, 5]), (lgf.OPT_TMARCH, [0, 1, 2, 4], [3, 8]),
+                           (lgf.OPT_SHARD_WORLD, [0, 1, 2, 4, 8], [5, 3, 16])]:
+        for v in bad:
+            assert L.lgf_set_option(ctx, key, v) == lgf.ERR_INVALID_ARG, (key, v)
+        for v in good:
+            assert L.lgf_set_option(ctx, key, v) == lgf.OK, (key, v)
+    assert L.lgf_set_option(ctx, lgf.OPT_SHARD_WORLD, 4) == lgf.OK
+    assert L.lgf_set_option(ctx, lgf.OPT_SHARD_RANK, 4) == lgf.ERR_INVALID_ARG
+    assert L.lgf_set_option(ctx, lgf.OPT_SHARD_RANK, 3) == lgf.OK
+    # a sharded context stores Nt / R + 2 time slices of every array plus the two exchange buffers
+    sharded = L.lgf_workspace_bytes(ctx)
+    assert L.lgf_set_option(ctx, lgf.OPT_SHARD_WORLD, 0) == lgf.OK
+    whole = L.lgf_workspace_bytes(ctx)
+    assert whole / 4 < sharded < whole / 2
+    # the shard calls refuse a context that is not bound / not sharded, without touching a GPU
+    off, nb = ctypes.c_size_t(), ctypes.c_size_t()
+    assert L.lgf_shard_region(ctx, lgf.REGION_G, ctypes.byref(off), ctypes.byref(nb)) == lgf.ERR_INVALID_ARG
+    assert L.lgf_shard_step(ctx, lgf.SHARD_ZT, 0.0, 0.0) == lgf.ERR_NOT_BOUND
+    assert L.lgf_destroy(ctx) == lgf.OK
