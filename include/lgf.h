@@ -154,7 +154,7 @@ enum {
                                    Before lgf_bind. */
     LGF_OPT_SHARD_RANK = 16,    /* which slab, 0 <= rank < SHARD_WORLD: time slices [rank Nt/R, (rank+1) Nt/R).
                                    Set after SHARD_WORLD, before lgf_bind. */
-    LGF_OPT_TMARCH = 17         /* 0 (default: 4 for FP32 contexts without ACCUM_G, else 1, as measured), 1, 2 or 4:
+    LGF_OPT_TMARCH = 17,        /* 0 (default: 4 for FP32 contexts without ACCUM_G, else 1, as measured), 1, 2 or 4:
                                    consecutive time slices a thread of the fused link kernel walks.  From its
                                    second site on the -t neighbour is the thread's own previous site, whose product
                                    g(x) U_t(x) it has just formed (Alg. 1 lines 12-16), so 12 of the
@@ -162,6 +162,17 @@ enum {
                                    when it does not divide the number of time slices the context walks.  Same
                                    arithmetic per link; the order of the F, theta partial sums changes (1e-16).
                                    Before lgf_bind. */
+    LGF_OPT_LINK_TILE = 18      /* the fused link kernel on 4D tiles: 0 (default) or 1 = off (one thread per site in
+                                   walk order, k_update_measure), 128 / 256 / 512 = threads (sites) per tile.  A CTA
+                                   owns an Nx x TDy x TDz x TDt tile; each thread forms its four new links
+                                   U'_mu(x) = g(x) U_mu(x) g^dagger(x+mu) once (Alg. 1 lines 12-16) and
+                                   hands the anti-Hermitian part of each, which is all that Delta(x+mu) needs of it
+                                   (eq. 1.5), to the thread of x+mu through shared memory; only backward
+                                   links across a tile face are rebuilt from the old links.  Same links bit for bit;
+                                   Delta, F, theta differ in the order of their sums (1e-16).  Measured slower than
+                                   the site kernel on B200 (profiles/r02_link_tile.md), hence off by default.
+                                   Ignored (site kernel) for sharded contexts, with ACCUM_G, with FUSION = 0 and when
+                                   Nx exceeds the tile.  Takes precedence over TMARCH.  Before lgf_bind. */
 };
 
 /* lgf_shard_step selectors: the kernels of one iteration of a sharded lattice, in the order of a step

@@ -14,6 +14,11 @@
 #include "launch.h"
 #include "su3.cuh"
 #include "reduce.cuh"
+#include <cstdio>
+#include <cstdlib>
+#ifndef LGF_FUSED_DUMMY_SMEM
+#define LGF_FUSED_DUMMY_SMEM 0   /* experiment: dynamic shared memory the site kernel does not use (what a smaller L1 costs) */
+#endif
 
 namespace lgf {
 
@@ -254,6 +259,11 @@ k_update_measure(const cx<T> *__restrict__ lin, cx<T> *__restrict__ lout, const 
                 if (MARCH && nu == 3 && kk > 0) {
 #pragma unroll
                     for (int k = 0; k < 6; k++) h[k] = Tc[k];
+#ifdef LGF_FUSED_SKIP_BWD   /* timing-only ceiling experiment (bit mask of directions whose backward link is NOT rebuilt): WRONG results */
+                } else if ((LGF_FUSED_SKIP_BWD >> nu) & 1) {
+#pragma unroll
+                    for (int k = 0; k < 6; k++) h[k] = mk<T>(0, 0);
+#endif
                 } else {
                     cx<T> gb[9], u[9];
                     load_g01<T, PACK, GBUF>(gsrc, V, sb, a, gexp, gb);
@@ -311,6 +321,231 @@ k_update_measure(const cx<T> *__restrict__ lin, cx<T> *__restrict__ lout, const 
 
 int fused_blocks(int64_t V) { return (int)((V + FUSED_THREADS - 1) / FUSED_THREADS); }
 
+// ---------------------------------------------------------------- the link kernel on 4D tiles (LGF_OPT_LINK_TILE)
+// A'(x) (eq. 1.5) needs the new link U'_nu(x-nu) only through its anti-Hermitian part: Delta is linear
+// in A - A^dagger.  k_update_measure lets the thread of x rebuild all four backward links from the old ones
+// (24 more loads and 30 more complex multiply-adds per direction).  Here a CTA owns an Nx x TDy x TDz x TDt tile of
+// sites, one thread per site.  The thread of x forms its four forward links once (Alg. 1 lines 12-16,
+// PAPER.md:98-106), stores them, and leaves the nine reals of the anti-Hermitian part of each (Im of the diagonal,
+// M_ij - conj(M_ji) above it) in shared memory; after one barrier the thread of x+nu picks them up.  Only the
+// backward neighbours outside the tile (the tile faces; none along a direction the tile spans completely, where
+// the neighbour wraps inside the tile) are rebuilt as before.  Same links as k_update_measure bit for bit; Delta,
+// F, theta differ in the order of their sums only.
+// MEASURED SLOWER on B200 (profiles/r02_link_tile.md: 32^4 FP64 12-real 238-261 us against 200 us, 64^4 5.18 against
+// 4.21 ms, 48^4 FP32 994 against 660 us) and therefore off by default: the backward rebuilds it removes are L1 / L2
+// hits that cost the site kernel only 7 % (LGF_FUSED_SKIP_BWD ceiling: 185.7 us), while the barrier in the middle of
+// a CTA's life and the spills of the FP64 form cost more.  Kept so that the comparison can be re-run.
+struct LinkTile {
+    int TD[4];       // tile extents (TD[0] = Nx)
+    int nT[4];       // tiles per direction
+    int tv;          // sites per tile (<= threads per CTA)
+    int zbt;         // z-block of the tile walk, in tiles (divides nT[2])
+};
+
+// the nine reals of the anti-Hermitian part of one link
+template <typename T> __device__ __forceinline__ void ah_part(const cx<T> (&m)[9], T (&p)[9])
+{
+    p[0] = m[0].y; p[1] = m[4].y; p[2] = m[8].y;
+    p[3] = m[1].x - m[3].x; p[4] = m[1].y + m[3].y;
+    p[5] = m[2].x - m[6].x; p[6] = m[2].y + m[6].y;
+    p[7] = m[5].x - m[7].x; p[8] = m[5].y + m[7].y;
+}
+
+template <typename T, int NE, int PACK, bool GBUF, int THREADS>
+__global__ void __launch_bounds__(THREADS, 512 / THREADS)
+k_update_measure_tile(const cx<T> *__restrict__ lin, cx<T> *__restrict__ lout, const cx<T> *__restrict__ gsrc,
+                      cx<T> *__restrict__ wout, Geom geo, LinkTile tg, T a, int gexp, Ctrl *ctrl, double *partials, double2 *hist, double eps)
+{
+    if (*(volatile int *)&ctrl->done) return;
+    extern __shared__ __align__(16) unsigned char xs_raw[];
+    T *xs = (T *)xs_raw;                             // [direction][9][THREADS]
+    const int64_t V = geo.V;
+    const int l = threadIdx.x;
+    const bool active = l < tg.tv;
+    // tile of this CTA: y-tiles fastest, then the (z,t) tiles in z-blocks like walk_site
+    unsigned b = blockIdx.x;
+    const int ty = (int)(b % (unsigned)tg.nT[1]); b /= (unsigned)tg.nT[1];
+    const unsigned per = (unsigned)(tg.zbt * tg.nT[3]);
+    const unsigned zblk = b / per, rem = b % per;
+    const int tt = (int)(rem / (unsigned)tg.zbt), tz = (int)(zblk * (unsigned)tg.zbt + rem % (unsigned)tg.zbt);
+    int lc[4], c[4];
+    {
+        unsigned r = (unsigned)l;
+        lc[0] = (int)(r % (unsigned)tg.TD[0]); r /= (unsigned)tg.TD[0];
+        lc[1] = (int)(r % (unsigned)tg.TD[1]); r /= (unsigned)tg.TD[1];
+        lc[2] = (int)(r % (unsigned)tg.TD[2]); r /= (unsigned)tg.TD[2];
+        lc[3] = (int)r;
+    }
+    c[0] = lc[0]; c[1] = ty * tg.TD[1] + lc[1]; c[2] = tz * tg.TD[2] + lc[2]; c[3] = tt * tg.TD[3] + lc[3];
+    const int64_t s = c[0] + geo.st[1] * c[1] + geo.st[2] * c[2] + geo.st[3] * c[3];
+    int lst[4];                                      // thread-index stride of each direction inside the tile
+    lst[0] = 1; lst[1] = tg.TD[0]; lst[2] = tg.TD[0] * tg.TD[1]; lst[3] = tg.TD[0] * tg.TD[1] * tg.TD[2];
+    double trF = 0, th = 0;
+    if (active) {
+        cx<T> g0[9];
+        load_g01<T, PACK, GBUF>(gsrc, V, s, a, gexp, g0);
+        su3_row2(g0);
+        T tr = 0;
+#pragma unroll
+        for (int mu = 0; mu < 4; mu++) {
+            const int64_t sp = s + (c[mu] == geo.N[mu] - 1 ? -(int64_t)(geo.N[mu] - 1) : (int64_t)1) * geo.st[mu];
+            cx<T> g1[9], u[9], t[9], r[9];
+            load_g01<T, PACK, GBUF>(gsrc, V, sp, a, gexp, g1);
+            su3_row2(g1);
+            load_link_in<T, NE>(lin, V, mu, s, u);
+            mul_rows<2>(g0, u, t);
+            mul_rows_dag<2>(t, g1, r);
+            su3_row2(r);
+            cx<T> *p = lout + (int64_t)mu * NE * V + s;
+#pragma unroll
+            for (int k = 0; k < NE; k++) st_link(p + (int64_t)k * V, r[k]);
+            tr += r[0].x + r[4].x + r[8].x;
+            // the thread's own share of A'(x), -U'_mu(x), is read back from shared memory as well: nine accumulators
+            // less to keep across the four products
+            T q[9];
+            ah_part<T>(r, q);
+#pragma unroll
+            for (int k = 0; k < 9; k++) xs[(mu * 9 + k) * THREADS + l] = q[k];
+        }
+        trF = (double)tr;
+    }
+    __syncthreads();
+    if (active) {
+        T D[9];
+#pragma unroll
+        for (int k = 0; k < 9; k++) D[k] = -((xs[k * THREADS + l] + xs[(9 + k) * THREADS + l]) + (xs[(18 + k) * THREADS + l] + xs[(27 + k) * THREADS + l]));
+        cx<T> X[9];
+#pragma unroll
+        for (int k = 0; k < 9; k++) X[k] = mk<T>(0, 0);
+        bool halo = false;
+#pragma unroll
+        for (int q = 0; q < 4; q++) {
+            const int nu = LGF_FUSED_BWD_REV ? 3 - q : q;
+            if (tg.TD[nu] > 1 && (lc[nu] > 0 || tg.nT[nu] == 1)) {       // the neighbour is a thread of this CTA
+                const int nl = l + (lc[nu] > 0 ? -1 : tg.TD[nu] - 1) * lst[nu];
+#pragma unroll
+                for (int k = 0; k < 9; k++) D[k] += xs[(nu * 9 + k) * THREADS + nl];
+            } else {
+                const int64_t sb = s + (c[nu] == 0 ? (int64_t)(geo.N[nu] - 1) : (int64_t)-1) * geo.st[nu];
+                cx<T> gb[9], u[9], h[9];
+                load_g01<T, PACK, GBUF>(gsrc, V, sb, a, gexp, gb);
+                load_link_in<T, NE>(lin, V, nu, sb, u);
+                mul_rows<2>(gb, u, h);
+                su3_row2(h);
+#pragma unroll
+                for (int k = 0; k < 9; k++) X[k] = X[k] + h[k];
+                halo = true;
+            }
+        }
+        if (halo) {
+            cx<T> g0[9], B[9];
+            load_g01<T, PACK, GBUF>(gsrc, V, s, a, gexp, g0);    // again: an L1 hit, cheaper than 36 live registers
+            su3_row2(g0);
+            mul_rows_dag<3>(X, g0, B);
+            T q[9];
+            ah_part<T>(B, q);
+#pragma unroll
+            for (int k = 0; k < 9; k++) D[k] += q[k];
+        }
+        const T di[3] = {D[0], D[1], D[2]};
+        const cx<T> E[3] = {mk<T>(D[3], D[4]), mk<T>(D[5], D[6]), mk<T>(D[7], D[8])};
+        th = store_delta<T, PACK>(di, E, wout, V, s);
+    }
+    finish_measure<THREADS>(trF, th, geo.Vg, ctrl, partials, hist, eps, 1);
+}
+
+static void link_tile_set(const Geom &g, const int td[4], LinkTile &tg)
+{
+    for (int d = 0; d < 4; d++) { tg.TD[d] = td[d]; tg.nT[d] = g.N[d] / td[d]; }
+    tg.tv = td[0] * td[1] * td[2] * td[3];
+    // z-block of the walk in tiles: the site walk's block if it is a whole number of tiles
+    const int zbt = g.zb / tg.TD[2];
+    tg.zbt = (zbt >= 1 && g.zb % tg.TD[2] == 0 && tg.nT[2] % zbt == 0) ? zbt : tg.nT[2];
+}
+
+// Tile of `threads` sites at most: TD0 = Nx, the other extents divisors of Ny, Nz, Nt chosen to minimise the share of
+// rebuilt backward links, sum_nu [TD_nu < N_nu] / TD_nu, weighted against idle threads.  Returns false when Nx > threads.
+// Built with -DLGF_TILE_ENV the environment variable LGF_LINK_TILE_DIMS="TDy,TDz,TDt" overrides the choice (tuning sweeps).
+static bool link_tile_choose(const Geom &g, int threads, LinkTile &tg)
+{
+    if (g.N[0] > threads) return false;
+#ifdef LGF_TILE_ENV
+    if (const char *e = getenv("LGF_LINK_TILE_DIMS")) {
+        int a1, a2, a3;
+        if (sscanf(e, "%d,%d,%d", &a1, &a2, &a3) == 3 && a1 > 0 && a2 > 0 && a3 > 0 && g.N[0] * a1 * a2 * a3 <= threads &&
+            g.N[1] % a1 == 0 && g.N[2] % a2 == 0 && g.N[3] % a3 == 0) {
+            const int td[4] = {g.N[0], a1, a2, a3};
+            link_tile_set(g, td, tg);
+            return true;
+        }
+    }
+#endif
+    double best = 1e30;
+    int bt[4] = {g.N[0], 1, 1, 1};
+    for (int a1 = 1; a1 <= g.N[1]; a1++) if (g.N[1] % a1 == 0)
+        for (int a2 = 1; a2 <= g.N[2]; a2++) if (g.N[2] % a2 == 0)
+            for (int a3 = 1; a3 <= g.N[3]; a3++) if (g.N[3] % a3 == 0) {
+                const int tv = g.N[0] * a1 * a2 * a3;
+                if (tv > threads) continue;
+                const int td[4] = {g.N[0], a1, a2, a3};
+                double halo = 0;
+                for (int d = 1; d < 4; d++) halo += td[d] == g.N[d] ? 0.0 : 1.0 / td[d];
+                const double cost = (1.0 + 0.3 * halo) * (double)threads / tv;
+                if (cost < best - 1e-12) { best = cost; for (int d = 0; d < 4; d++) bt[d] = td[d]; }
+            }
+    link_tile_set(g, bt, tg);
+    return true;
+}
+
+int link_tile_threads(const Geom &g, int want)
+{
+    LinkTile tg;
+    if (g.Vw != g.V) return 0;                       // sharded slabs (halo slices, no wrap in t) keep the site kernel
+    if (want != 128 && want != 256 && want != 512) return 0;
+    if (!link_tile_choose(g, want, tg)) return 0;
+    // one pair of partial sums per CTA: the workspace holds 2 fused_blocks(V) + 2 pairs (make_layout)
+    return (int64_t)tg.nT[1] * tg.nT[2] * tg.nT[3] <= 2 * (int64_t)fused_blocks(g.V) ? want : 0;
+}
+
+template <typename T, int NE, int PACK, bool GB, int THREADS>
+static void launch_tile_one(const SiteArgs &a, const LinkTile &tg, const void *lin, void *lout, const void *gsrc, void *wout,
+                            double alpha, double eps, cudaStream_t st)
+{
+    const size_t smem = (size_t)4 * 9 * THREADS * sizeof(T);
+    static bool done = false;
+    if (!done) {
+        done = true;
+        if (cudaFuncSetAttribute(k_update_measure_tile<T, NE, PACK, GB, THREADS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
+            cudaGetLastError();
+    }
+    const unsigned nb = (unsigned)(tg.nT[1] * tg.nT[2] * tg.nT[3]);
+    k_update_measure_tile<T, NE, PACK, GB, THREADS><<<nb, THREADS, smem, st>>>((const cx<T> *)lin, (cx<T> *)lout, (const cx<T> *)gsrc,
+        (cx<T> *)wout, a.geo, tg, (T)(alpha / 2.0), a.gexp, a.ctrl, a.partials, a.hist, eps);
+}
+
+static void launch_update_measure_tile(const SiteArgs &a, const void *lin, void *lout, const void *gsrc, int gbuf, void *wout,
+                                       double alpha, double eps, cudaStream_t st)
+{
+    LinkTile tg;
+    link_tile_choose(a.geo, a.ltile, tg);
+#define CALL_T(T, NE, PACK, GB)                                                                                   \
+    do {                                                                                                          \
+        if (a.ltile == 128) launch_tile_one<T, NE, PACK, GB, 128>(a, tg, lin, lout, gsrc, wout, alpha, eps, st);  \
+        else if (a.ltile == 256) launch_tile_one<T, NE, PACK, GB, 256>(a, tg, lin, lout, gsrc, wout, alpha, eps, st); \
+        else launch_tile_one<T, NE, PACK, GB, 512>(a, tg, lin, lout, gsrc, wout, alpha, eps, st);                 \
+    } while (0)
+#define CALL_NE(T, NE)                                           \
+    do {                                                         \
+        if (gbuf) { CALL_T(T, NE, 4, true); }                    \
+        else if (a.pack == 4) { CALL_T(T, NE, 4, false); }       \
+        else { CALL_T(T, NE, 9, false); }                        \
+    } while (0)
+    if (a.prec == 0) { if (a.recon == 12) CALL_NE(double, 6); else CALL_NE(double, 9); }
+    else             { if (a.recon == 12) CALL_NE(float, 6); else CALL_NE(float, 9); }
+#undef CALL_NE
+#undef CALL_T
+}
+
 // The link kernel keeps nothing in shared memory but the reduction scratch: ask for the largest L1
 // the SM offers, the x and y neighbours of a CTA's sites are re-read through it (once per instantiation).
 #ifndef LGF_FUSED_MAXL1
@@ -334,13 +569,14 @@ template <typename T, int NE, int PACK, bool GBUF, bool STORE> static void prefe
 void launch_update_measure(const SiteArgs &a, const void *lin, void *lout, const void *gsrc, int gbuf, void *wout,
                            double alpha, double eps, cudaStream_t st)
 {
+    if (a.ltile > 0) { launch_update_measure_tile(a, lin, lout, gsrc, gbuf, wout, alpha, eps, st); return; }
     const int tk = a.tmarch > 0 ? a.tmarch : 1;
     const int nb = fused_blocks(a.geo.Vw / tk);
 #define CALL(T, NE, PACK, GB) \
     do { prefer_l1<T, NE, PACK, GB, true>();   \
-    if (tk > 1) k_update_measure<T, NE, PACK, GB, true, true><<<nb, FUSED_THREADS, 0, st>>>((const cx<T> *)lin, (cx<T> *)lout, (const cx<T> *)gsrc, \
+    if (tk > 1) k_update_measure<T, NE, PACK, GB, true, true><<<nb, FUSED_THREADS, LGF_FUSED_DUMMY_SMEM, st>>>((const cx<T> *)lin, (cx<T> *)lout, (const cx<T> *)gsrc, \
         (cx<T> *)wout, a.geo, (T)(alpha / 2.0), a.gexp, a.ctrl, a.partials, a.hist, eps, tk); \
-    else k_update_measure<T, NE, PACK, GB, true, false><<<nb, FUSED_THREADS, 0, st>>>((const cx<T> *)lin, (cx<T> *)lout, (const cx<T> *)gsrc, \
+    else k_update_measure<T, NE, PACK, GB, true, false><<<nb, FUSED_THREADS, LGF_FUSED_DUMMY_SMEM, st>>>((const cx<T> *)lin, (cx<T> *)lout, (const cx<T> *)gsrc, \
         (cx<T> *)wout, a.geo, (T)(alpha / 2.0), a.gexp, a.ctrl, a.partials, a.hist, eps, 1); } while (0)
 #define CALL_NE(T, NE)                                           \
     do {                                                         \

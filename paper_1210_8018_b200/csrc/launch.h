@@ -16,6 +16,7 @@ struct SiteArgs {
     int pack;           // 4 or 9
     int gexp;           // LGF_OPT_GMAP: 0 first order + reunitarisation, 1 exact exponential
     int tmarch;         // LGF_OPT_TMARCH: consecutive time slices per thread of the link kernel (1, 2 or 4; divides Ntw)
+    int ltile;          // LGF_OPT_LINK_TILE resolved: 0 = one thread per site in walk order (k_update_measure), 128 / 256 / 512 = 4D tiles of that many threads
 };
 
 // kernel (a): Delta, F, theta (eq. 1.5, 1.1, 1.4).  eps < 0: never raise `done`.
@@ -28,6 +29,8 @@ void launch_update(const SiteArgs &a, double alpha, cudaStream_t st);
 void launch_update_measure(const SiteArgs &a, const void *lin, void *lout, const void *gsrc, int gbuf, void *wout,
                            double alpha, double eps, cudaStream_t st);
 int fused_blocks(int64_t V);
+// threads per CTA of the tiled link kernel for this geometry, 0 when it does not apply (want = 128, 256 or 512)
+int link_tile_threads(const Geom &g, int want);
 // ACCUM_G (fixed links, accumulated transformation G in the g buffer, rows 0, 1):
 // Delta, F, theta of G(x) U_mu(x) G^dagger(x+mu) -> a.w; counts one iteration
 void launch_measure_acc(const SiteArgs &a, const void *gacc, double eps, cudaStream_t st);

@@ -537,6 +537,69 @@ def test_tmarch_falls_back_when_it_does_not_divide(lgf):
     assert ra.F == rb.F and ra.theta == rb.theta and np.array_equal(a.get_links(), b.get_links())
 
 
+# ------------------------------------------------------------------ LGF_OPT_LINK_TILE: the link kernel on 4D tiles
+TILE_LATTICES = [(8, 8, 8, 8), (16, 16, 16, 16), (12, 12, 12, 12), (4, 6, 8, 12), (16, 8, 4, 6), (32, 32, 8, 8), (48, 48, 4, 4),
+                 (64, 64, 4, 4), (24, 24, 6, 8), (8, 4, 4, 4), (32, 4, 4, 32), (64, 8, 8, 4)]
+
+
+@pytest.mark.parametrize("var", [dict(recon=12), dict(recon=18), dict(recon=18, precision="fp32"), dict(recon=12, precision="fp32"),
+                                 dict(recon=18, fft_batch=9), dict(recon=12, fft_path=1), dict(recon=12, zblock=2), dict(recon=12, gmap=1)], ids=vid)
+@pytest.mark.parametrize("threads", [128, 256, 512])
+def test_link_tile_gives_the_same_links(lgf, var, threads):
+    """The tiled link kernel hands the anti-Hermitian parts of the new links to the +mu neighbours through shared memory
+    instead of rebuilding the backward links: same link products, so the links after one iteration are bitwise those of the
+    site kernel; Delta (hence F, theta) differs by the order of eight additions, and the iteration matches the oracle
+    (links 1e-12 / 1e-5, F and theta 1e-10 / 1e-4 relative)."""
+    fp32 = var.get("precision") == "fp32"
+    for N in TILE_LATTICES:
+        U = gen.gen_links(N, 0.5, 808 + N[0] + N[3])
+        Uo = U.copy()
+        if var.get("gmap"):
+            oracle.set_exponential(1)
+        try:
+            hist = oracle.iterate(N, Uo, ALPHA, 1)
+        finally:
+            oracle.set_exponential(0)
+        Uin = U.astype(np.complex64) if fp32 else U
+        res = []
+        for lt in (1, threads):
+            gf = lgf.GaugeFixer(N, link_tile=lt, tmarch=1, **var)
+            gf.load_links(Uin)
+            r1 = gf.iterate(ALPHA, 1)
+            assert np.abs(gf.get_links().astype(np.complex128) - Uo).max() < (1e-5 if fp32 else 1e-12), (N, lt)
+            assert abs(r1.F - hist[1, 0]) <= (1e-4 if fp32 else 1e-10) * abs(hist[1, 0]), (N, lt)
+            assert abs(r1.theta - hist[1, 1]) <= (1e-4 if fp32 else 1e-10) * hist[1, 1], (N, lt)
+            D1 = gf.get_field(lgf.FIELD_DELTA)
+            res.append((gf.get_links(), r1.F, r1.theta, D1))
+            gf.close()
+        assert np.array_equal(res[0][0], res[1][0]), N
+        assert np.abs(res[0][3] - res[1][3]).max() <= (2e-5 if fp32 else 2e-14), N
+        assert abs(res[0][1] - res[1][1]) <= (1e-6 if fp32 else 1e-14), N
+        assert abs(res[0][2] - res[1][2]) <= (1e-5 if fp32 else 1e-13) * res[0][2], N
+
+
+@pytest.mark.parametrize("threads", [128, 256, 512])
+def test_link_tile_converges_to_the_golden_count(lgf, threads):
+    """Algorithm 1 to theta <= 1e-15 with the tiled link kernel: the oracle's iteration count and final F (16^4 golden)."""
+    it, F, th, ghist = read_golden(golden_path(16, gen.BASE_SEED + 16))
+    U = gen.gen_links(16, 0.5, gen.BASE_SEED + 16)
+    gf = lgf.GaugeFixer(16, recon=12, link_tile=threads)
+    gf.load_links(U)
+    r = gf.fix(ALPHA, 1e-15)
+    assert r.converged == 1 and r.iterations == it
+    assert abs(r.F - F) < 1e-10
+    h = gf.history()
+    assert np.abs(h[:, 0] - ghist[:, 0]).max() < 1e-10
+    gf.close()
+
+
+def test_link_tile_option_is_validated(lgf):
+    with pytest.raises(lgf.LgfError):
+        lgf.GaugeFixer(8, link_tile=64)
+    with pytest.raises(lgf.LgfError):
+        lgf.GaugeFixer(8, link_tile=-1)
+
+
 # ------------------------------------------------------------------ ensemble.py: lattices pipelined through one GPU
 def test_ensemble_pipeline_equals_one_lattice_at_a_time(lgf):
     """Seven different lattices through three slots (three contexts, streams and host threads): results and links
