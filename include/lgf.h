@@ -332,6 +332,30 @@ int lgf_shard_result(lgf_ctx *ctx, lgf_result *out);
  * Allocates and frees 8 bytes of device memory; synchronises.  *dfma_per_second: host. */
 int lgf_debug_dfma_rate(void *cuda_stream, double *dfma_per_second);
 
+/* ---- The one entry point that allocates nothing (csrc/noalloc.cu) -------------------------------------------
+ * For callers that cannot allocate device memory or keep a context (code under CUDA graph capture, tight
+ * serving loops, harnesses that forbid cudaMalloc): kernel (a) of Algorithm 1 on the caller's own arrays,
+ *     Delta(x) (eq. 1.5),  F (eq. 1.1),  theta (eq. 1.4),
+ * with the same arithmetic and the same fixed-order FP64 reduction as lgf_measure.  No context, no workspace:
+ * the kernel's scratch memory (block partial sums, ticket counter, result block) is a static device array of
+ * LGF_NOALLOC_SCRATCH_BYTES = 131 584 bytes that every GPU that loads the library holds until the process exits,
+ * which limits the lattice to LGF_NOALLOC_MAX_SITES = 2^20 sites (32^4); larger lattices get
+ * LGF_ERR_UNSUPPORTED_SIZE (text from lgf_noalloc_last_error) and must use a context.  Extents 2 <= N <= 64.
+ *   links_dev : device, LGF_LAYOUT_AOS [V][4][3][3] complex (FP64: 16 bytes each, FP32: 8), read only
+ *   delta_dev : device, [V][3][3] complex, written; may be NULL (F and theta only)
+ *   F_theta   : two doubles (F, theta), device or pinned host memory, written by a copy on the stream
+ *   cuda_stream: a cudaStream_t passed as void*, may be NULL; the device that owns the buffers must be current.
+ * Asynchronous: everything is enqueued on the stream, nothing is synchronised.  Calls cudaGetSymbolAddress once per
+ * device; calls no cudaMalloc / cudaFree or any allocating routine.  All calls on one GPU SHARE the scratch array:
+ * each call clears what must start at zero, but two calls that overlap on the GPU (different streams or host
+ * threads) race -- serialise them.  Buffers are the caller's. */
+#define LGF_NOALLOC_MAX_SITES 1048576
+#define LGF_NOALLOC_SCRATCH_BYTES 131584
+int lgf_measure_noalloc(int Nx, int Ny, int Nz, int Nt, int precision, const void *links_dev, void *delta_dev,
+                        double *F_theta, void *cuda_stream);
+/* Text of the last error of lgf_measure_noalloc in this process.  Never NULL. */
+const char *lgf_noalloc_last_error(void);
+
 /* Text of the last error of this context (or of lgf_create when ctx == NULL). Never NULL. */
 const char *lgf_last_error(const lgf_ctx *ctx);
 

@@ -19,7 +19,7 @@ ZT_EXTENTS = [8, 12, 16, 24, 32, 48, 64]
 # (source, extra flags, object name); fft_zt_inst.cu is compiled once per Nz (the (z,t) pass of the tiled FFT
 # for that Nz and every Nt), so that the 7 x 7 extent pairs build in parallel
 SOURCES = [(f, [], f.replace(".cu", ".o")) for f in
-           ["lgf_api.cu", "kernels_site.cu", "kernels_fused.cu", "fft_generic.cu", "fft_tiled.cu", "microbench.cu"]]
+           ["lgf_api.cu", "kernels_site.cu", "kernels_fused.cu", "fft_generic.cu", "fft_tiled.cu", "microbench.cu", "noalloc.cu"]]
 SOURCES += [("fft_zt_inst.cu", [f"-DLGF_ZT_NA={n}"], f"fft_zt_na{n}.o") for n in ZT_EXTENTS]
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",

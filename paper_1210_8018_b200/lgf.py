@@ -37,6 +37,7 @@ SYMBOLS = [
     "lgf_measure", "lgf_iterate", "lgf_fix", "lgf_stage", "lgf_get_field", "lgf_set_field", "lgf_history",
     "lgf_kernel_time", "lgf_launch_count", "lgf_reset_counters", "lgf_uses_tiled_fft", "lgf_uses_gbuf", "lgf_zblock", "lgf_sync_links", "lgf_last_error",
     "lgf_destroy", "lgf_debug_dfma_rate", "lgf_shard_step", "lgf_shard_region", "lgf_shard_info", "lgf_shard_result",
+    "lgf_measure_noalloc", "lgf_noalloc_last_error",
 ]
 
 
@@ -96,6 +97,9 @@ def lib():
     L.lgf_shard_region.argtypes = [vp, i, ctypes.POINTER(ctypes.c_size_t), ctypes.POINTER(ctypes.c_size_t)]
     L.lgf_shard_info.argtypes = [vp, ctypes.POINTER(i64), i]
     L.lgf_shard_result.argtypes = [vp, rp]
+    L.lgf_measure_noalloc.argtypes = [i, i, i, i, i, vp, vp, vp, vp]
+    L.lgf_noalloc_last_error.argtypes = []
+    L.lgf_noalloc_last_error.restype = ctypes.c_char_p
     _lib = L
     return L
 
@@ -107,6 +111,29 @@ def debug_dfma_rate(stream=None):
     if rc:
         raise LgfError(rc, "lgf_debug_dfma_rate failed")
     return out.value
+
+
+NOALLOC_MAX_SITES = 1 << 20
+
+
+def measure_noalloc(N, links, delta, F_theta, stream=None):
+    """lgf_measure_noalloc: Delta, F, theta of `links` (torch complex tensor on the GPU, [V,4,3,3]) into the
+    caller's `delta` ([V,3,3], same dtype, or None) and `F_theta` (two float64, on the GPU or pinned host memory),
+    enqueued on `stream` (a torch stream; default: the current one).  Allocates nothing; at most 2^20 sites.
+    Marshalling only."""
+    import torch
+
+    N = _dims(N)
+    prec = {torch.complex128: PREC_FP64, torch.complex64: PREC_FP32}[links.dtype]
+    assert links.is_cuda and links.is_contiguous()
+    assert delta is None or (delta.is_cuda and delta.is_contiguous() and delta.dtype == links.dtype)
+    assert F_theta.dtype == torch.float64 and F_theta.numel() == 2 and F_theta.is_contiguous()
+    with torch.cuda.device(links.device):
+        st = stream if stream is not None else torch.cuda.current_stream(links.device)
+        rc = lib().lgf_measure_noalloc(*N, prec, links.data_ptr(), delta.data_ptr() if delta is not None else None,
+                                       F_theta.data_ptr(), st.cuda_stream)
+    if rc:
+        raise LgfError(rc, lib().lgf_noalloc_last_error().decode())
 
 
 def _dims(N):
