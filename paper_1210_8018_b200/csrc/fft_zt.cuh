@@ -13,6 +13,11 @@ namespace lgf {
 // shared (thread = (c, kz)): Dif(-), mask, Dit(+) -> shared; z-lines from shared: Dif(+),
 // stored straight to global.  p^2 = sum_mu 4 sin^2(pi k_mu/N_mu) (reading R5) from the
 // per-axis tables; the factor p_max^2/(p^2 V) is one FP64 division per mode.
+// Timing-only experiment on k_fft_zt (WRONG results; profiles/r02_zt_phases.md): 1 = memory only (every global and shared
+// load / store of the pass, no transform, no mask), 2 = arithmetic only (no global loads or stores; shared memory kept).
+#ifndef LGF_ZT_EXP
+#define LGF_ZT_EXP 0
+#endif
 #ifndef LGF_ZT_MAXB
 #define LGF_ZT_MAXB 2   /* 3 measured slower at 32^4 (47.6 vs 45.5 us: spills), equal at 48^4 */
 #endif
@@ -80,8 +85,8 @@ k_fft_zt(cx<T> *__restrict__ w, Geom geo, const double *__restrict__ ptab, doubl
         cx<T> v[LA::NL];
         const cx<T> *g = f + ca + st * ta;
 #pragma unroll
-        for (int i = 0; i < LA::NL; i++) v[i] = g[sz * LA::nat(i, ha)];
-        LA::template dif<-1>(v, ha, mz);
+        for (int i = 0; i < LA::NL; i++) v[i] = LGF_ZT_EXP == 2 ? mk<T>((T)(t + i) * (T)1e-3, (T)(i - t) * (T)1e-3) : g[sz * LA::nat(i, ha)];
+        if (LGF_ZT_EXP != 1) LA::template dif<-1>(v, ha, mz);
 #pragma unroll
         for (int q = 0; q < LA::NL; q++) sm[ta * TL::RS + LA::slot(q, ha) * C + ca] = v[q];
     }
@@ -90,14 +95,16 @@ k_fft_zt(cx<T> *__restrict__ w, Geom geo, const double *__restrict__ ptab, doubl
         cx<T> v[LB::NL];
 #pragma unroll
         for (int i = 0; i < LB::NL; i++) v[i] = sm[LB::nat(i, hb) * TL::RS + zb * C + cb];
-        LB::template dif<-1>(v, hb, mt);
+        if (LGF_ZT_EXP != 1) LB::template dif<-1>(v, hb, mt);
         const double pxyz = ptab[x0 + cb] + ptab[Nx + y] + ptab[Nx + Ny + zb];
+        if (LGF_ZT_EXP != 1) {
 #pragma unroll
         for (int q = 0; q < LB::NL; q++) {
             const T fac = (T)mask_factor(pmax2_over_V, pxyz + pt[LB::slot(q, hb)]);
             v[q] = cscale(v[q], fac);
         }
         LB::template dit<+1>(v, hb, mt);
+        }
 #pragma unroll
         for (int i = 0; i < LB::NL; i++) sm[LB::nat(i, hb) * TL::RS + zb * C + cb] = v[i];
     }
@@ -106,10 +113,10 @@ k_fft_zt(cx<T> *__restrict__ w, Geom geo, const double *__restrict__ ptab, doubl
         cx<T> v[LA::NL];
 #pragma unroll
         for (int i = 0; i < LA::NL; i++) v[i] = sm[ta * TL::RS + LA::nat(i, ha) * C + ca];
-        LA::template dif<+1>(v, ha, mz);
+        if (LGF_ZT_EXP != 1) LA::template dif<+1>(v, ha, mz);
         cx<T> *g = f + ca + st * ta;
 #pragma unroll
-        for (int q = 0; q < LA::NL; q++) g[sz * LA::slot(q, ha)] = v[q];
+        for (int q = 0; q < LA::NL; q++) if (LGF_ZT_EXP != 2 || v[q].x == (T)123456.789) g[sz * LA::slot(q, ha)] = v[q];
     }
 }
 
