@@ -258,7 +258,7 @@ def run_ours(args):
 
     gf = lgf.GaugeFixer(N, precision=prec, recon=recon, fft_batch=args.fft_batch, fft_path=args.fft_path,
                         fusion=args.fusion, l2_persist=args.l2_persist, accum_g=args.accum_g, gmap=args.gmap, graph=args.graph,
-                        zblock=args.zblock, zt_pipe=args.zt_pipe, link_tile=args.link_tile, tmarch=args.tmarch, device=f"cuda:{local}")
+                        zblock=args.zblock, zt_pipe=args.zt_pipe, link_tile=args.link_tile, link_stream=args.link_stream, tmarch=args.tmarch, device=f"cuda:{local}")
     K, W = args.steps, args.warmup
     stream = gf.stream
 
@@ -472,7 +472,7 @@ def run_ours(args):
         "ms_per_step": ms_all / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f64" if prec == "fp64" else "f32", "data": "synthetic",
         "config": {"workload": workload_label(args, prec, recon, gen.BASE_SEED + soff, sigma),
-                   "lattice": list(N), "zblock": gf.zblock(), "zt_pipe": args.zt_pipe, "link_tile": args.link_tile,
+                   "lattice": list(N), "zblock": gf.zblock(), "zt_pipe": args.zt_pipe, "link_tile": args.link_tile, "link_stream": args.link_stream,
                    "fft": "tiled register FFT, 3 passes" if tiled else "generic per-axis transform, 8 passes",
                    "l2": "working set (links + fields) exceeds the 126 MB L2" if V >= 32 ** 4 else
                          "working set fits in L2; latency/L2-bound by design (DESIGN.md section 6)",
@@ -591,6 +591,7 @@ def main():
     ap.add_argument("--pipeline", type=int, default=1, choices=[0, 1], help="also time the e2e step for a stream of lattices (ensemble.py)")
     ap.add_argument("--zblock", type=int, default=None, help="LGF_OPT_ZBLOCK (default: chosen from the L2 size)")
     ap.add_argument("--link-tile", type=int, default=None, help="LGF_OPT_LINK_TILE: 1 = site kernel, 128 / 256 / 512 = threads per 4D tile")
+    ap.add_argument("--link-stream", type=int, default=None, choices=[0, 1], help="LGF_OPT_LINK_STREAM: 1 = TMA-fed persistent link kernel")
     ap.add_argument("--tmarch", type=int, default=None, help="LGF_OPT_TMARCH")
     ap.add_argument("--zt-pipe", type=int, default=None, choices=[0, 1], help="LGF_OPT_ZT_PIPE")
     ap.add_argument("--launch-selftest", action="store_true", help="start the ranks, reduce one timing, print the rank count")

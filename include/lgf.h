@@ -162,7 +162,7 @@ enum {
                                    when it does not divide the number of time slices the context walks.  Same
                                    arithmetic per link; the order of the F, theta partial sums changes (1e-16).
                                    Before lgf_bind. */
-    LGF_OPT_LINK_TILE = 18      /* the fused link kernel on 4D tiles: 0 (default) or 1 = off (one thread per site in
+    LGF_OPT_LINK_TILE = 18,     /* the fused link kernel on 4D tiles: 0 (default) or 1 = off (one thread per site in
                                    walk order, k_update_measure), 128 / 256 / 512 = threads (sites) per tile.  A CTA
                                    owns an Nx x TDy x TDz x TDt tile; each thread forms its four new links
                                    U'_mu(x) = g(x) U_mu(x) g^dagger(x+mu) once (Alg. 1 lines 12-16) and
@@ -173,6 +173,16 @@ enum {
                                    the site kernel on B200 (profiles/r02_link_tile.md), hence off by default.
                                    Ignored (site kernel) for sharded contexts, with ACCUM_G, with FUSION = 0 and when
                                    Nx exceeds the tile.  Takes precedence over TMARCH.  Before lgf_bind. */
+    LGF_OPT_LINK_STREAM = 19    /* 1: the fused link kernel as a stream (k_update_measure_stream).  Persistent CTAs
+                                   walk tiles of 128 consecutive sites; a producer warp fetches the tile's own links
+                                   U_mu(x), the 4 x 6 or 4 x 9 SoA lines per site that must come from DRAM (Alg. 1
+                                   lines 12-16), with cp.async.bulk (the TMA engine) into a ring of
+                                   shared-memory stages, completion on an mbarrier, while four consumer warps do the
+                                   arithmetic of the previous tile.  Same links bit for bit; F and theta are summed
+                                   per CTA over its tiles (order of the sums only).  Needs the default path (FUSION = 1,
+                                   FFT_BATCH = 4, tiled FFT: the g buffer) and Nx Ny divisible by 128; ignored
+                                   otherwise, for sharded contexts and with ACCUM_G.  Takes precedence over LINK_TILE
+                                   and TMARCH.  0 (default): off.  Before lgf_bind. */
 };
 
 /* lgf_shard_step selectors: the kernels of one iteration of a sharded lattice, in the order of a step

@@ -293,7 +293,11 @@ k_update_measure(const cx<T> *__restrict__ lin, cx<T> *__restrict__ lout, const 
                 cx<T> g1[9], u[9], t[9], r[9];
                 load_g01<T, PACK, GBUF>(gsrc, V, sp, a, gexp, g1);
                 su3_row2(g1);
+#ifdef LGF_FUSED_FAKE_OWN   /* timing-only experiment: the thread's own links come from a cache-resident window (WRONG results) */
+                load_link_in<T, NE>(lin, V, mu, s & (int64_t)(LGF_FUSED_FAKE_OWN - 1), u);
+#else
                 load_link_in<T, NE>(lin, V, mu, s, u);
+#endif
                 mul_rows<2>(g0, u, t);
                 if (MARCH && mu == 3) {
 #pragma unroll
@@ -546,6 +550,227 @@ static void launch_update_measure_tile(const SiteArgs &a, const void *lin, void 
 #undef CALL_T
 }
 
+// ---------------------------------------------------------------- the link kernel as a stream (LGF_OPT_LINK_STREAM)
+// The same arithmetic as k_update_measure, site by site, with the thread's OWN links -- the 4 NE lines per site that
+// must come from DRAM -- fetched ahead of time by the TMA engine instead of by the thread: a persistent CTA walks
+// tiles of TS consecutive sites of the walk order (contiguous in memory when Nx Ny is a multiple of TS); its producer
+// warp issues one cp.async.bulk per SoA component array (TS x 16 bytes, contiguous) into a ring of shared-memory
+// stages, completion on an mbarrier, and the consumer warps take U_mu(x) -- and U_nu(x-nu) where x-nu lies in the
+// tile -- from shared memory.  g and the backward links outside the tile come through L1 / L2 as before.  Bytes in
+// flight per SM are then set by the ring (stages x 4 NE x TS x 16 B), not by the registers of 16 warps.
+// F and theta are accumulated per thread over all tiles of the CTA and reduced once at the end (one pair of partial
+// sums per CTA), so they differ from the site kernel's in the order of the sums only; links bitwise equal.
+// Default path only (g buffer, 4 packed fields); lattices with Nx Ny % TS != 0 and sharded slabs keep the site kernel.
+#ifndef LGF_STREAM_STAGES
+#define LGF_STREAM_STAGES 2
+#endif
+#ifdef LGF_STREAM_MINB_ALL   /* tuning sweeps: one CTA count for every instantiation (nvcc splits -D values at commas) */
+#define LGF_STREAM_MINB(T, NE) LGF_STREAM_MINB_ALL
+#endif
+#ifndef LGF_STREAM_MINB
+#define LGF_STREAM_MINB(T, NE) ((sizeof(T) == 8 && (NE) == 9) ? 1 : 2)
+#endif
+static const int STREAM_TS = 128;                    // sites per tile = consumer threads
+static const int STREAM_THREADS = STREAM_TS + 32;    // + one producer warp
+
+__device__ __forceinline__ unsigned smem_u32(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(unsigned long long *b, unsigned count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(b)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(unsigned long long *b, unsigned bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(b)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(unsigned long long *b)
+{
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(b)) : "memory");
+}
+__device__ __forceinline__ bool mbar_try_wait(unsigned long long *b, unsigned parity)
+{
+    unsigned ok;
+    asm volatile("{\n .reg .pred p;\n mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n selp.u32 %0, 1, 0, p;\n}"
+                 : "=r"(ok) : "r"(smem_u32(b)), "r"(parity) : "memory");
+    return ok != 0;
+}
+__device__ __forceinline__ void mbar_wait(unsigned long long *b, unsigned parity)
+{
+    while (!mbar_try_wait(b, parity)) {}
+}
+// global -> shared bulk copy by the TMA engine (UBLKCP in SASS); bytes: multiple of 16, both addresses 16-byte aligned
+__device__ __forceinline__ void bulk_g2s(void *dst, const void *src, unsigned bytes, unsigned long long *bar)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
+}
+
+template <typename T, int NE> struct StreamCfg {
+    static constexpr int NARR = 4 * NE;
+    static constexpr size_t STAGE = (size_t)NARR * STREAM_TS * sizeof(cx<T>);
+    static constexpr int NST = LGF_STREAM_STAGES;
+    static constexpr size_t SMEM = 128 + (size_t)NST * STAGE;     // barriers in the first 128 bytes
+    static constexpr int MINB = LGF_STREAM_MINB(T, NE);
+};
+
+// U_mu of site index s: from the stage when s lies in the tile [s0, s0 + TS), else from global memory
+template <typename T, int NE>
+__device__ __forceinline__ void load_link_stream(const cx<T> *__restrict__ lin, const cx<T> *stg, int64_t V, int mu, int64_t s, int64_t s0, cx<T> (&u)[9])
+{
+    const int64_t d = s - s0;
+    if ((unsigned long long)d < (unsigned long long)STREAM_TS) {
+        const cx<T> *p = stg + (size_t)mu * NE * STREAM_TS + d;
+#pragma unroll
+        for (int k = 0; k < NE; k++) u[k] = p[k * STREAM_TS];
+        if (NE == 6) su3_row2(u);
+    } else {
+        load_link_in<T, NE>(lin, V, mu, s, u);
+    }
+}
+
+template <typename T, int NE>
+__global__ void __launch_bounds__(STREAM_THREADS, (StreamCfg<T, NE>::MINB))
+k_update_measure_stream(const cx<T> *__restrict__ lin, cx<T> *__restrict__ lout, const cx<T> *__restrict__ gsrc,
+                        cx<T> *__restrict__ wout, Geom geo, int ntiles, Ctrl *ctrl, double *partials, double2 *hist, double eps)
+{
+    if (*(volatile int *)&ctrl->done) return;
+    typedef StreamCfg<T, NE> CF;
+    constexpr int TS = STREAM_TS, NST = CF::NST;
+    extern __shared__ __align__(128) unsigned char st_raw[];
+    unsigned long long *full = (unsigned long long *)st_raw, *empty = full + NST;
+    cx<T> *stage0 = (cx<T> *)(st_raw + 128);
+    const int tid = threadIdx.x;
+    const int64_t V = geo.V;
+    if (tid == 0) {
+        for (int i = 0; i < NST; i++) { mbar_init(full + i, 1); mbar_init(empty + i, TS / 32); }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+    }
+    __syncthreads();
+    double trF = 0, th = 0;
+    if (tid >= TS) {
+        // ---- producer warp: lane 0 keeps the ring full, the other lanes walk along (the warp stays converged)
+        int st = 0;
+        unsigned ph = 0;
+        for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
+            if (tid == TS) {
+                mbar_wait(empty + st, ph ^ 1u);                        // the consumers are done with this stage
+                int c[4];
+                const int64_t s0 = walk_site(geo, (int64_t)tile * TS, c);
+                cx<T> *dst = stage0 + (size_t)st * CF::NARR * TS;
+                mbar_expect_tx(full + st, (unsigned)CF::STAGE);
+#pragma unroll 4
+                for (int j = 0; j < CF::NARR; j++)
+                    bulk_g2s(dst + (size_t)j * TS, lin + (int64_t)j * V + s0, (unsigned)(TS * sizeof(cx<T>)), full + st);
+            }
+            __syncwarp();
+            if (++st == NST) { st = 0; ph ^= 1u; }
+        }
+    } else {
+        // ---- consumers: one site per thread and tile
+        int st = 0;
+        unsigned ph = 0;
+        for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
+            int c[4];
+            const int64_t s = walk_site(geo, (int64_t)tile * TS + tid, c);
+            const int64_t s0 = s - tid;
+            const cx<T> *stg = stage0 + (size_t)st * CF::NARR * TS;
+            // backward links, order t, z, y, x: t and z lie in other planes (global memory, issued before the wait);
+            // y and x are in the tile for most sites
+            cx<T> X[9];
+#pragma unroll
+            for (int k = 0; k < 9; k++) X[k] = mk<T>(0, 0);
+#pragma unroll
+            for (int q = 0; q < 4; q++) {
+                const int nu = 3 - q;
+                const int64_t sb = s + (c[nu] == 0 ? (int64_t)(geo.N[nu] - 1) : (int64_t)-1) * geo.st[nu];
+                cx<T> gb[9], u[9], h[9];
+                load_g01<T, 4, true>(gsrc, V, sb, (T)0, 0, gb);
+                if (nu >= 2) {
+                    load_link_in<T, NE>(lin, V, nu, sb, u);
+                } else {
+                    if (nu == 1) mbar_wait(full + st, ph);             // the tile's own links have landed
+                    load_link_stream<T, NE>(lin, stg, V, nu, sb, s0, u);
+                }
+                mul_rows<2>(gb, u, h);
+                su3_row2(h);
+#pragma unroll
+                for (int k = 0; k < 9; k++) X[k] = X[k] + h[k];
+            }
+            cx<T> g0[9];
+            load_g01<T, 4, true>(gsrc, V, s, (T)0, 0, g0);
+            su3_row2(g0);
+            T di[3] = {0, 0, 0};
+            cx<T> E[3] = {mk<T>(0, 0), mk<T>(0, 0), mk<T>(0, 0)};
+            {
+                cx<T> B[9];
+                mul_rows_dag<3>(X, g0, B);
+                acc_ah<T>(B, (T)1, di, E);
+            }
+            T tr = 0;
+#pragma unroll
+            for (int mu = 0; mu < 4; mu++) {
+                const int64_t sp = s + (c[mu] == geo.N[mu] - 1 ? -(int64_t)(geo.N[mu] - 1) : (int64_t)1) * geo.st[mu];
+                cx<T> g1[9], u[9], t[9], r[9];
+                load_g01<T, 4, true>(gsrc, V, sp, (T)0, 0, g1);
+                su3_row2(g1);
+                {
+                    const cx<T> *p = stg + (size_t)mu * NE * TS + tid;
+#pragma unroll
+                    for (int k = 0; k < NE; k++) u[k] = p[k * TS];
+                    if (NE == 6) su3_row2(u);
+                }
+                if (mu == 3) {                                         // last read of the stage: hand it back
+                    __syncwarp();
+                    if ((tid & 31) == 0) mbar_arrive(empty + st);
+                }
+                mul_rows<2>(g0, u, t);
+                mul_rows_dag<2>(t, g1, r);
+                su3_row2(r);
+                cx<T> *p = lout + (int64_t)mu * NE * V + s;
+#pragma unroll
+                for (int k = 0; k < NE; k++) st_link(p + (int64_t)k * V, r[k]);
+                tr += r[0].x + r[4].x + r[8].x;
+                acc_ah<T>(r, (T)-1, di, E);
+            }
+            trF += (double)tr;
+            th += store_delta<T, 4>(di, E, wout, V, s);
+            if (++st == NST) { st = 0; ph ^= 1u; }
+        }
+    }
+    finish_measure<STREAM_THREADS>(trF, th, geo.Vg, ctrl, partials, hist, eps, 1);
+}
+
+// 1 when the streamed link kernel applies to this geometry
+int link_stream_ok(const Geom &g)
+{
+    if (g.Vw != g.V) return 0;                                    // sharded slabs keep the site kernel
+    return ((int64_t)g.N[0] * g.N[1]) % STREAM_TS == 0 ? 1 : 0;
+}
+
+template <typename T, int NE>
+static void launch_stream_one(const SiteArgs &a, const void *lin, void *lout, const void *gsrc, void *wout, double eps, cudaStream_t st)
+{
+    typedef StreamCfg<T, NE> CF;
+    static int resident = 0;
+    if (resident == 0) {
+        int dev = 0, sms = 148, per = 1;
+        if (cudaFuncSetAttribute(k_update_measure_stream<T, NE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)CF::SMEM) != cudaSuccess) cudaGetLastError();
+        if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) { cudaGetLastError(); sms = 148; }
+        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per, k_update_measure_stream<T, NE>, STREAM_THREADS, CF::SMEM) != cudaSuccess || per < 1) { cudaGetLastError(); per = 1; }
+        resident = sms * per;
+    }
+    const int ntiles = (int)(a.geo.V / STREAM_TS);
+    const int nb = ntiles < resident ? ntiles : resident;
+    k_update_measure_stream<T, NE><<<nb, STREAM_THREADS, CF::SMEM, st>>>((const cx<T> *)lin, (cx<T> *)lout, (const cx<T> *)gsrc, (cx<T> *)wout,
+        a.geo, ntiles, a.ctrl, a.partials, a.hist, eps);
+}
+
+static void launch_update_measure_stream(const SiteArgs &a, const void *lin, void *lout, const void *gsrc, void *wout, double eps, cudaStream_t st)
+{
+    if (a.prec == 0) { if (a.recon == 12) launch_stream_one<double, 6>(a, lin, lout, gsrc, wout, eps, st); else launch_stream_one<double, 9>(a, lin, lout, gsrc, wout, eps, st); }
+    else             { if (a.recon == 12) launch_stream_one<float, 6>(a, lin, lout, gsrc, wout, eps, st); else launch_stream_one<float, 9>(a, lin, lout, gsrc, wout, eps, st); }
+}
+
 // The link kernel keeps nothing in shared memory but the reduction scratch: ask for the largest L1
 // the SM offers, the x and y neighbours of a CTA's sites are re-read through it (once per instantiation).
 #ifndef LGF_FUSED_MAXL1
@@ -569,6 +794,7 @@ template <typename T, int NE, int PACK, bool GBUF, bool STORE> static void prefe
 void launch_update_measure(const SiteArgs &a, const void *lin, void *lout, const void *gsrc, int gbuf, void *wout,
                            double alpha, double eps, cudaStream_t st)
 {
+    if (a.lstream > 0 && gbuf) { launch_update_measure_stream(a, lin, lout, gsrc, wout, eps, st); return; }
     if (a.ltile > 0) { launch_update_measure_tile(a, lin, lout, gsrc, gbuf, wout, alpha, eps, st); return; }
     const int tk = a.tmarch > 0 ? a.tmarch : 1;
     const int nb = fused_blocks(a.geo.Vw / tk);

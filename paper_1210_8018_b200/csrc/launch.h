@@ -16,6 +16,7 @@ struct SiteArgs {
     int pack;           // 4 or 9
     int gexp;           // LGF_OPT_GMAP: 0 first order + reunitarisation, 1 exact exponential
     int tmarch;         // LGF_OPT_TMARCH: consecutive time slices per thread of the link kernel (1, 2 or 4; divides Ntw)
+    int lstream;        // LGF_OPT_LINK_STREAM resolved: 1 = the streamed link kernel (k_update_measure_stream) where the path has a g buffer
     int ltile;          // LGF_OPT_LINK_TILE resolved: 0 = one thread per site in walk order (k_update_measure), 128 / 256 / 512 = 4D tiles of that many threads
 };
 
@@ -31,6 +32,8 @@ void launch_update_measure(const SiteArgs &a, const void *lin, void *lout, const
 int fused_blocks(int64_t V);
 // threads per CTA of the tiled link kernel for this geometry, 0 when it does not apply (want = 128, 256 or 512)
 int link_tile_threads(const Geom &g, int want);
+// 1 when the streamed link kernel (LGF_OPT_LINK_STREAM) applies to this geometry
+int link_stream_ok(const Geom &g);
 // ACCUM_G (fixed links, accumulated transformation G in the g buffer, rows 0, 1):
 // Delta, F, theta of G(x) U_mu(x) G^dagger(x+mu) -> a.w; counts one iteration
 void launch_measure_acc(const SiteArgs &a, const void *gacc, double eps, cudaStream_t st);

@@ -44,6 +44,7 @@ struct lgf_ctx {
     int fft_passes = 3;      // LGF_OPT_FFT_PASSES: 3 (fused middle), 4 (2D + 2D), 8 (4 x 1D)
     int tmarch = 0;          // LGF_OPT_TMARCH: time slices per thread of the link kernel (0 = auto)
     int link_tile = 0;       // LGF_OPT_LINK_TILE: 0 / 1 = off, 128 / 256 / 512 threads per tile
+    int link_stream = 0;     // LGF_OPT_LINK_STREAM: 1 = TMA-fed persistent link kernel
     // one lattice sharded in t-slabs over shard_world ranks (0 = off): V = sites of the interchange arrays (the
     // rank's own time slices), Vp = stored sites (with the two halo slices), Vg = sites of the whole lattice
     int shard_world = 0, shard_rank = 0;
@@ -477,7 +478,7 @@ int lgf_set_option(lgf_ctx *ctx, int key, int64_t value)
     if (!ctx) return LGF_ERR_INVALID_ARG;
     const bool layout_key = (key == LGF_OPT_RECON || key == LGF_OPT_FFT_BATCH || key == LGF_OPT_FFT_PATH || key == LGF_OPT_FUSION ||
                              key == LGF_OPT_L2_PERSIST || key == LGF_OPT_ACCUM_G || key == LGF_OPT_ZBLOCK || key == LGF_OPT_FFT_PASSES ||
-                             key == LGF_OPT_SHARD_WORLD || key == LGF_OPT_SHARD_RANK || key == LGF_OPT_TMARCH || key == LGF_OPT_LINK_TILE);
+                             key == LGF_OPT_SHARD_WORLD || key == LGF_OPT_SHARD_RANK || key == LGF_OPT_TMARCH || key == LGF_OPT_LINK_TILE || key == LGF_OPT_LINK_STREAM);
     if (layout_key && ctx->bound) return fail(ctx, LGF_ERR_INVALID_ARG, "this option must be set before lgf_bind");
     switch (key) {
     case LGF_OPT_RECON:
@@ -523,6 +524,9 @@ int lgf_set_option(lgf_ctx *ctx, int key, int64_t value)
         if (value != 0 && value != 1 && value != 128 && value != 256 && value != 512)
             return fail(ctx, LGF_ERR_INVALID_ARG, "LINK_TILE must be 0 or 1 (off), 128, 256 or 512");
         ctx->link_tile = (int)value; break;
+    case LGF_OPT_LINK_STREAM:
+        if (value != 0 && value != 1) return fail(ctx, LGF_ERR_INVALID_ARG, "LINK_STREAM must be 0 or 1");
+        ctx->link_stream = (int)value; break;
     case LGF_OPT_SHARD_WORLD:
         if (value < 0 || (value > 0 && (ctx->N[3] % value != 0 || ctx->N[1] % value != 0)))
             return fail(ctx, LGF_ERR_INVALID_ARG, "SHARD_WORLD must be 0 (off) or divide Nt and Ny");
@@ -589,6 +593,7 @@ int lgf_bind(lgf_ctx *ctx, void *dev_workspace, size_t bytes, void *cuda_stream)
     const int want = ctx->tmarch > 0 ? ctx->tmarch : ((ctx->prec == LGF_PREC_FP32 && !ctx->accum) ? 4 : 1);
     s.tmarch = (g.Ntw % want == 0) ? want : 1;
     s.ltile = (ctx->link_tile > 1 && ctx->fusion && !ctx->accum) ? link_tile_threads(g, ctx->link_tile) : 0;
+    s.lstream = (ctx->link_stream == 1 && ctx->fusion && !ctx->accum) ? link_stream_ok(g) : 0;
     for (int i = 0; i < 2; i++) { ctx->links_buf[i] = ctx->base + L.links[i]; ctx->w_buf[i] = ctx->base + L.w[i]; }
     ctx->gbuf = ctx->base + L.gbuf;
     ctx->cur = 0; ctx->wcur = 0;

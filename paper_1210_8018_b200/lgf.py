@@ -21,7 +21,7 @@ PREC_FP64, PREC_FP32 = 0, 1
 LAYOUT_AOS, LAYOUT_AOS12 = 0, 1
 OPT_RECON, OPT_FFT_BATCH, OPT_MAX_ITER, OPT_CHECK_INTERVAL, OPT_FFT_PATH, OPT_PROFILE, OPT_FUSION, OPT_L2_PERSIST = 1, 2, 3, 4, 5, 6, 7, 8
 OPT_GMAP, OPT_ACCUM_G, OPT_GRAPH, OPT_ZBLOCK, OPT_ZT_PIPE, OPT_FFT_PASSES = 9, 10, 11, 12, 13, 14
-OPT_SHARD_WORLD, OPT_SHARD_RANK, OPT_TMARCH, OPT_LINK_TILE = 15, 16, 17, 18
+OPT_SHARD_WORLD, OPT_SHARD_RANK, OPT_TMARCH, OPT_LINK_TILE, OPT_LINK_STREAM = 15, 16, 17, 18, 19
 (SHARD_MEASURE, SHARD_RESET, SHARD_XY_FWD, SHARD_PACK, SHARD_ZT, SHARD_UNPACK, SHARD_XY_INV_G, SHARD_LINK,
  SHARD_FINISH) = range(9)
 REGION_CTRL, REGION_XSEND, REGION_XRECV, REGION_G, REGION_LINKS = range(5)
@@ -150,7 +150,7 @@ class GaugeFixer:
 
     def __init__(self, N, precision="fp64", recon=18, fft_batch=4, fft_path=0, device="cuda:0",
                  stream=None, max_iter=None, check_interval=None, profile=False, fusion=None, l2_persist=None, gmap=None,
-                 accum_g=None, graph=None, zblock=None, zt_pipe=None, fft_passes=None, shard=None, tmarch=None, link_tile=None):
+                 accum_g=None, graph=None, zblock=None, zt_pipe=None, fft_passes=None, shard=None, tmarch=None, link_tile=None, link_stream=None):
         import torch
 
         self.torch = torch
@@ -189,6 +189,8 @@ class GaugeFixer:
             self.set_option(OPT_TMARCH, tmarch)
         if link_tile is not None:
             self.set_option(OPT_LINK_TILE, link_tile)
+        if link_stream is not None:
+            self.set_option(OPT_LINK_STREAM, link_stream)
         if shard is not None:
             self.set_option(OPT_SHARD_WORLD, shard[0])
             self.set_option(OPT_SHARD_RANK, shard[1])

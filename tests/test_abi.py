@@ -143,7 +143,7 @@ def test_round_2_options_validate_on_the_host(L):
     ctx = ctypes.c_void_p()
     assert L.lgf_create(16, 16, 12, 24, lgf.PREC_FP64, ctypes.byref(ctx)) == lgf.OK
     for key, good, bad in [(lgf.OPT_ZBLOCK, [0, 1, 3, 12], [-1, 5, 24]), (lgf.OPT_ZT_PIPE, [0, 1], [2]),
-                           (lgf.OPT_FFT_PASSES, [3, 4, 8], [0, 2, 5]), (lgf.OPT_TMARCH, [0, 1, 2, 4], [3, 8]), (lgf.OPT_LINK_TILE, [0, 1, 128, 256, 512], [-1, 2, 64, 1024]),
+                           (lgf.OPT_FFT_PASSES, [3, 4, 8], [0, 2, 5]), (lgf.OPT_TMARCH, [0, 1, 2, 4], [3, 8]), (lgf.OPT_LINK_TILE, [0, 1, 128, 256, 512], [-1, 2, 64, 1024]), (lgf.OPT_LINK_STREAM, [0, 1], [-1, 2]),
                            (lgf.OPT_SHARD_WORLD, [0, 1, 2, 4, 8], [5, 3, 16])]:
         for v in bad:
             assert L.lgf_set_option(ctx, key, v) == lgf.ERR_INVALID_ARG, (key, v)

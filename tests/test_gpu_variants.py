@@ -600,6 +600,72 @@ def test_link_tile_option_is_validated(lgf):
         lgf.GaugeFixer(8, link_tile=-1)
 
 
+# ------------------------------------------------------------------ LGF_OPT_LINK_STREAM: TMA-fed persistent link kernel
+STREAM_LATTICES = [(16, 16, 16, 16), (16, 8, 4, 6), (32, 32, 8, 8), (32, 4, 4, 32), (48, 48, 4, 4), (64, 64, 4, 4), (64, 8, 8, 4),
+                   (16, 16, 4, 24), (8, 8, 8, 8), (24, 24, 6, 8)]          # the last two: Nx Ny % 128 != 0, the option is ignored
+
+
+@pytest.mark.parametrize("var", [dict(recon=12), dict(recon=18), dict(recon=18, precision="fp32"), dict(recon=12, precision="fp32"),
+                                 dict(recon=12, zblock=2), dict(recon=12, gmap=1), dict(recon=12, graph=0)], ids=vid)
+def test_link_stream_gives_the_same_links(lgf, var):
+    """The streamed link kernel takes the thread's own links from a shared-memory ring filled by cp.async.bulk instead of
+    loading them itself: same arithmetic per site, so the links after 1 and 3 iterations are bitwise those of the site
+    kernel, F and theta agree to the order of the partial sums, and the first iteration matches the oracle."""
+    fp32 = var.get("precision") == "fp32"
+    for N in STREAM_LATTICES:
+        U = gen.gen_links(N, 0.5, 909 + N[0] + N[3])
+        Uo = U.copy()
+        if var.get("gmap"):
+            oracle.set_exponential(1)
+        try:
+            hist = oracle.iterate(N, Uo, ALPHA, 1)
+        finally:
+            oracle.set_exponential(0)
+        Uin = U.astype(np.complex64) if fp32 else U
+        res = []
+        for ls in (0, 1):
+            gf = lgf.GaugeFixer(N, link_stream=ls, tmarch=1, **var)
+            gf.load_links(Uin)
+            r1 = gf.iterate(ALPHA, 1)
+            U1 = gf.get_links()
+            assert np.abs(U1.astype(np.complex128) - Uo).max() < (1e-5 if fp32 else 1e-12), (N, ls)
+            assert abs(r1.F - hist[1, 0]) <= (1e-4 if fp32 else 1e-10) * abs(hist[1, 0]), (N, ls)
+            assert abs(r1.theta - hist[1, 1]) <= (1e-4 if fp32 else 1e-10) * hist[1, 1], (N, ls)
+            D1 = gf.get_field(lgf.FIELD_DELTA)
+            r3 = gf.iterate(ALPHA, 2)
+            res.append((U1, D1, gf.get_links(), r3.F, r3.theta))
+            gf.close()
+        assert np.array_equal(res[0][0], res[1][0]), N
+        if fp32:       # the FP32 site kernel adds the backward links in the order x, y, z, t, the streamed one in t, z, y, x
+            assert np.abs(res[0][1] - res[1][1]).max() <= 2e-5, N
+        else:
+            assert np.array_equal(res[0][1], res[1][1]), N             # Delta: the same sums per site
+        if fp32:       # a Delta that differs in the last place feeds the next g: the links stay equal to FP32 rounding
+            assert np.abs(res[0][2] - res[1][2]).max() <= 2e-5, N
+        else:
+            assert np.array_equal(res[0][2], res[1][2]), N
+        assert abs(res[0][3] - res[1][3]) <= (1e-6 if fp32 else 1e-14), N
+        assert abs(res[0][4] - res[1][4]) <= (1e-5 if fp32 else 1e-13) * res[0][4], N
+
+
+def test_link_stream_converges_to_the_golden_count(lgf):
+    """Algorithm 1 to theta <= 1e-15 with the streamed link kernel: the oracle's iteration count, final F and F history
+    (16^4 golden), with graph replay (default) and a stop decision taken by the persistent kernel's last CTA."""
+    it, F, th, ghist = read_golden(golden_path(16, gen.BASE_SEED + 16))
+    U = gen.gen_links(16, 0.5, gen.BASE_SEED + 16)
+    for recon in (12, 18):
+        gf = lgf.GaugeFixer(16, recon=recon, link_stream=1)
+        gf.load_links(U)
+        r = gf.fix(ALPHA, 1e-15)
+        assert r.converged == 1 and r.iterations == it
+        assert abs(r.F - F) < 1e-10
+        h = gf.history()
+        assert np.abs(h[:, 0] - ghist[:, 0]).max() < 1e-10
+        gf.close()
+    with pytest.raises(lgf.LgfError):
+        lgf.GaugeFixer(16, link_stream=2)
+
+
 # ------------------------------------------------------------------ ensemble.py: lattices pipelined through one GPU
 def test_ensemble_pipeline_equals_one_lattice_at_a_time(lgf):
     """Seven different lattices through three slots (three contexts, streams and host threads): results and links
