@@ -17,8 +17,6 @@ template <typename T> using cx = typename C2<T>::type;
 template <typename T> __host__ __device__ __forceinline__ cx<T> mk(T re, T im) { cx<T> r; r.x = re; r.y = im; return r; }
 __device__ __forceinline__ double2 operator+(double2 a, double2 b) { return make_double2(a.x + b.x, a.y + b.y); }
 __device__ __forceinline__ double2 operator-(double2 a, double2 b) { return make_double2(a.x - b.x, a.y - b.y); }
-__device__ __forceinline__ float2 operator+(float2 a, float2 b) { return make_float2(a.x + b.x, a.y + b.y); }
-__device__ __forceinline__ float2 operator-(float2 a, float2 b) { return make_float2(a.x - b.x, a.y - b.y); }
 // Complex products written as explicit fused multiply-adds: `acc.x += a.x*b.x - a.y*b.y` as plain
 // C++ costs DMUL + DFMA + DADD per component (the compiler may not reassociate), the forms
 // below cost two FMAs.  The FP64 pipe is the second roofline of this path.
@@ -76,6 +74,72 @@ template <typename V> __device__ __forceinline__ V cfmaconj(V a, V b, V acc)
     acc.y = fma_t(-a.y, b.x, fma_t(a.x, b.y, acc.y));
     return acc;
 }
+// ---------------------------------------------------------------- packed FP32 (sm_100: add / mul / fma .f32x2)
+// A complex number in FP32 is a register pair, and Blackwell has arithmetic on pairs (FADD2, FMUL2, FFMA2 in SASS):
+// a complex add is one instruction, a complex multiply-add two (the broadcasts {a.x, a.x} and the swaps {b.y, b.x}
+// become operand modifiers).  Same operations as the scalar forms above up to which of the two products of a
+// component is rounded first.  Measured on B200 (same-run A/B, profiles/r02_f32x2.md): 43 % fewer arithmetic
+// instructions in the FP32 FFT passes but register-pair moves in their place; the (x,y) passes on 32^2 planes get
+// 10-16 % faster, the 48^2 passes and the (z,t) pass do not change, the FP32 link kernel gets 8-9 % SLOWER.  So the
+// packed forms are compiled in the translation unit of the (x,y) passes only (fft_tiled.cu defines LGF_F32X2 1 before
+// it includes this header); -DLGF_F32X2=0 / 1 on the command line sets it everywhere.
+#ifndef LGF_F32X2
+#define LGF_F32X2 0
+#endif
+#if LGF_F32X2
+__device__ __forceinline__ unsigned long long pk2(float lo, float hi)
+{
+    unsigned long long r;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
+    return r;
+}
+__device__ __forceinline__ float2 un2(unsigned long long r)
+{
+    float2 v;
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(v.x), "=f"(v.y) : "l"(r));
+    return v;
+}
+__device__ __forceinline__ unsigned long long mul2(unsigned long long a, unsigned long long b)
+{
+    unsigned long long r;
+    asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
+    return r;
+}
+__device__ __forceinline__ unsigned long long fma2(unsigned long long a, unsigned long long b, unsigned long long c)
+{
+    unsigned long long r;
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c));
+    return r;
+}
+__device__ __forceinline__ float2 add2(float2 a, float2 b)
+{
+    unsigned long long r;
+    asm("add.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(pk2(a.x, a.y)), "l"(pk2(b.x, b.y)));
+    return un2(r);
+}
+__device__ __forceinline__ float2 sub2(float2 a, float2 b)
+{
+    unsigned long long r;
+    asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(pk2(a.x, a.y)), "l"(pk2(b.x, b.y)));
+    return un2(r);
+}
+// non-template overloads: preferred over the templates above for float2
+__device__ __forceinline__ float2 cmul(float2 a, float2 b) { return un2(fma2(pk2(a.x, a.x), pk2(b.x, b.y), mul2(pk2(a.y, a.y), pk2(-b.y, b.x)))); }
+__device__ __forceinline__ float2 cmulc(float2 a, float2 b) { return un2(fma2(pk2(a.x, a.x), pk2(b.x, -b.y), mul2(pk2(a.y, a.y), pk2(b.y, b.x)))); }
+__device__ __forceinline__ float2 cconjmul(float2 a, float2 b) { return un2(fma2(pk2(a.x, a.x), pk2(b.x, b.y), mul2(pk2(a.y, a.y), pk2(b.y, -b.x)))); }
+__device__ __forceinline__ float2 cfma(float2 a, float2 b, float2 acc) { return un2(fma2(pk2(a.y, a.y), pk2(-b.y, b.x), fma2(pk2(a.x, a.x), pk2(b.x, b.y), pk2(acc.x, acc.y)))); }
+__device__ __forceinline__ float2 cfms(float2 a, float2 b, float2 acc) { return un2(fma2(pk2(a.y, a.y), pk2(b.y, -b.x), fma2(pk2(-a.x, -a.x), pk2(b.x, b.y), pk2(acc.x, acc.y)))); }
+__device__ __forceinline__ float2 cfmac(float2 a, float2 b, float2 acc) { return un2(fma2(pk2(a.y, a.y), pk2(b.y, b.x), fma2(pk2(a.x, a.x), pk2(b.x, -b.y), pk2(acc.x, acc.y)))); }
+__device__ __forceinline__ float2 cfmaconj(float2 a, float2 b, float2 acc) { return un2(fma2(pk2(a.y, a.y), pk2(b.y, -b.x), fma2(pk2(a.x, a.x), pk2(b.x, b.y), pk2(acc.x, acc.y)))); }
+__device__ __forceinline__ float2 cscale(float2 a, float s) { return un2(mul2(pk2(a.x, a.y), pk2(s, s))); }
+#endif
+#if LGF_F32X2
+__device__ __forceinline__ float2 operator+(float2 a, float2 b) { return add2(a, b); }
+__device__ __forceinline__ float2 operator-(float2 a, float2 b) { return sub2(a, b); }
+#else
+__device__ __forceinline__ float2 operator+(float2 a, float2 b) { return make_float2(a.x + b.x, a.y + b.y); }
+__device__ __forceinline__ float2 operator-(float2 a, float2 b) { return make_float2(a.x - b.x, a.y - b.y); }
+#endif
 template <typename V> __device__ __forceinline__ V cconj(V a) { a.y = -a.y; return a; }
 template <typename V> __device__ __forceinline__ auto cnorm2(V a) -> decltype(a.x) { return a.x * a.x + a.y * a.y; }
 template <typename V, typename T> __device__ __forceinline__ V cscale(V a, T s) { a.x *= s; a.y *= s; return a; }

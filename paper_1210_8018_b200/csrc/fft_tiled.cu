@@ -19,6 +19,9 @@
 // addressing and for the mask.  Lines along the second axis of a tile go through shared
 // memory (padded rows, conflict-free for 16-byte accesses); the first axis of a pass is
 // loaded straight from global memory into registers and the last one stored straight back.
+#ifndef LGF_F32X2
+#define LGF_F32X2 1   /* packed FP32 complex arithmetic (common.cuh) for the (x,y) passes: measured faster here only */
+#endif
 #include "fft_lines.cuh"
 #include "su3.cuh"
 #include <cooperative_groups.h>
