@@ -16,6 +16,10 @@
 #include "reduce.cuh"
 #include <cstdio>
 #include <cstdlib>
+// 1: F and theta of the link kernel are summed in two levels (reduce.cuh, finish_measure_2l); 0: by the last block alone
+#ifndef LGF_REDUCE_2L
+#define LGF_REDUCE_2L 1
+#endif
 #ifndef LGF_FUSED_DUMMY_SMEM
 #define LGF_FUSED_DUMMY_SMEM 0   /* experiment: dynamic shared memory the site kernel does not use (what a smaller L1 costs) */
 #endif
@@ -169,7 +173,7 @@ __device__ __forceinline__ double store_delta(const T (&di)[3], const cx<T> (&E)
 template <typename T, int NE, int PACK, bool GBUF, bool STORE, bool MARCH = false>
 __global__ void __launch_bounds__(FUSED_THREADS, (STORE ? LGF_FUSED_MINB : LGF_ACC_MINB(NE, T)))
 k_update_measure(const cx<T> *__restrict__ lin, cx<T> *__restrict__ lout, const cx<T> *__restrict__ gsrc,
-                 cx<T> *__restrict__ wout, Geom geo, T a, int gexp, Ctrl *ctrl, double *partials, double2 *hist, double eps, int tk_arg)
+                 cx<T> *__restrict__ wout, Geom geo, T a, int gexp, Ctrl *ctrl, double *partials, void *gred, double2 *hist, double eps, int tk_arg)
 {
     const int tk = MARCH ? tk_arg : 1;
     if (*(volatile int *)&ctrl->done) return;
@@ -320,7 +324,11 @@ k_update_measure(const cx<T> *__restrict__ lin, cx<T> *__restrict__ lout, const 
           }
         }
     }
+#if LGF_REDUCE_2L
+    finish_measure_2l<FUSED_THREADS>(trF, th, geo.Vg, ctrl, partials, gred, hist, eps, 1);
+#else
     finish_measure<FUSED_THREADS>(trF, th, geo.Vg, ctrl, partials, hist, eps, 1);
+#endif
 }
 
 int fused_blocks(int64_t V) { return (int)((V + FUSED_THREADS - 1) / FUSED_THREADS); }
@@ -801,9 +809,9 @@ void launch_update_measure(const SiteArgs &a, const void *lin, void *lout, const
 #define CALL(T, NE, PACK, GB) \
     do { prefer_l1<T, NE, PACK, GB, true>();   \
     if (tk > 1) k_update_measure<T, NE, PACK, GB, true, true><<<nb, FUSED_THREADS, LGF_FUSED_DUMMY_SMEM, st>>>((const cx<T> *)lin, (cx<T> *)lout, (const cx<T> *)gsrc, \
-        (cx<T> *)wout, a.geo, (T)(alpha / 2.0), a.gexp, a.ctrl, a.partials, a.hist, eps, tk); \
+        (cx<T> *)wout, a.geo, (T)(alpha / 2.0), a.gexp, a.ctrl, a.partials, a.gred, a.hist, eps, tk); \
     else k_update_measure<T, NE, PACK, GB, true, false><<<nb, FUSED_THREADS, LGF_FUSED_DUMMY_SMEM, st>>>((const cx<T> *)lin, (cx<T> *)lout, (const cx<T> *)gsrc, \
-        (cx<T> *)wout, a.geo, (T)(alpha / 2.0), a.gexp, a.ctrl, a.partials, a.hist, eps, 1); } while (0)
+        (cx<T> *)wout, a.geo, (T)(alpha / 2.0), a.gexp, a.ctrl, a.partials, a.gred, a.hist, eps, 1); } while (0)
 #define CALL_NE(T, NE)                                           \
     do {                                                         \
         if (gbuf) { CALL(T, NE, 4, true); }                      \
@@ -824,9 +832,9 @@ void launch_measure_acc(const SiteArgs &a, const void *gacc, double eps, cudaStr
 #define CALL(T, NE) \
     do { prefer_l1<T, NE, 4, true, false>();  \
     if (tk > 1) k_update_measure<T, NE, 4, true, false, true><<<nb, FUSED_THREADS, 0, st>>>((const cx<T> *)a.links, (cx<T> *)nullptr, \
-        (const cx<T> *)gacc, (cx<T> *)a.w, a.geo, (T)0, 0, a.ctrl, a.partials, a.hist, eps, tk); \
+        (const cx<T> *)gacc, (cx<T> *)a.w, a.geo, (T)0, 0, a.ctrl, a.partials, a.gred, a.hist, eps, tk); \
     else k_update_measure<T, NE, 4, true, false, false><<<nb, FUSED_THREADS, 0, st>>>((const cx<T> *)a.links, (cx<T> *)nullptr, \
-        (const cx<T> *)gacc, (cx<T> *)a.w, a.geo, (T)0, 0, a.ctrl, a.partials, a.hist, eps, 1); } while (0)
+        (const cx<T> *)gacc, (cx<T> *)a.w, a.geo, (T)0, 0, a.ctrl, a.partials, a.gred, a.hist, eps, 1); } while (0)
     if (a.prec == 0) { if (a.recon == 12) CALL(double, 6); else CALL(double, 9); }
     else             { if (a.recon == 12) CALL(float, 6); else CALL(float, 9); }
 #undef CALL

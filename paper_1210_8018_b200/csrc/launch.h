@@ -10,6 +10,7 @@ struct SiteArgs {
     void *w;            // device: cx<T> [PACK][V]   (Delta, then w, in place)
     Ctrl *ctrl;         // device
     double *partials;   // device: 2 doubles per block of kernel (a)
+    void *gred;         // device: group partials and group tickets of the two-level reduction (reduce.cuh, reduce2l_bytes)
     double2 *hist;      // device: LGF_HIST_CAP pairs (F, theta)
     int prec;           // 0 = FP64, 1 = FP32
     int recon;          // 18 or 12

@@ -12,6 +12,7 @@
 
 #include "../../include/lgf.h"
 #include "launch.h"
+#include "reduce.cuh"
 
 using namespace lgf;
 
@@ -27,7 +28,7 @@ struct EvPair { cudaEvent_t a, b; int kind; };
 size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 
 struct Layout {
-    size_t links[2], w[2], gbuf, partials, ctrl, hist, ptab, tw, staging, xbuf[2], ptab_zt, total;
+    size_t links[2], w[2], gbuf, partials, gred, ctrl, hist, ptab, tw, staging, xbuf[2], ptab_zt, total;
     int64_t staging_sites;
 };
 
@@ -106,6 +107,7 @@ Layout make_layout(const lgf_ctx *c)
     // the tiled link kernel (LGF_OPT_LINK_TILE) may leave threads of a CTA idle: at most twice the CTAs (link_tile_threads checks)
     const int nblk = std::max(measure_blocks(Vl), 2 * fused_blocks(Vl) + 2);
     L.partials = off; off = align_up(off + (size_t)2 * nblk * sizeof(double), 256);
+    L.gred = off; off = align_up(off + reduce2l_bytes(fused_blocks(Vl)), 256);
     L.ctrl = off; off = align_up(off + sizeof(Ctrl), 256);
     L.hist = off; off = align_up(off + (size_t)LGF_HIST_CAP * sizeof(double2), 256);
     L.ptab = off; off = align_up(off + (size_t)sum_n(c) * sizeof(double), 256);
@@ -598,6 +600,7 @@ int lgf_bind(lgf_ctx *ctx, void *dev_workspace, size_t bytes, void *cuda_stream)
     ctx->gbuf = ctx->base + L.gbuf;
     ctx->cur = 0; ctx->wcur = 0;
     s.partials = (double *)(ctx->base + L.partials);
+    s.gred = ctx->base + L.gred;
     s.ctrl = (Ctrl *)(ctx->base + L.ctrl);
     s.hist = (double2 *)(ctx->base + L.hist);
     s.prec = ctx->prec; s.recon = ctx->recon; s.pack = ctx->pack; s.gexp = ctx->gmap;
@@ -643,6 +646,7 @@ int lgf_bind(lgf_ctx *ctx, void *dev_workspace, size_t bytes, void *cuda_stream)
         CK(cudaMemsetAsync(ctx->base, 0, L.partials, ctx->st));
         CK(cudaMemsetAsync(ctx->base + L.xbuf[0], 0, L.ptab_zt - L.xbuf[0], ctx->st));
     }
+    CK(cudaMemsetAsync(s.partials, 0, L.ctrl - L.partials, ctx->st));   // the group tickets of the two-level reduction start at zero
     CK(cudaMemsetAsync(s.ctrl, 0, sizeof(Ctrl), ctx->st));
     CK(cudaMemsetAsync(s.hist, 0, sizeof(double2) * LGF_HIST_CAP, ctx->st));
     CK(cudaStreamSynchronize(ctx->st)); // the host vectors above go out of scope

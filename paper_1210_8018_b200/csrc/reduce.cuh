@@ -53,6 +53,10 @@ __device__ __forceinline__ void finish_measure(double trF, double th, int64_t V,
         last = (tk == gridDim.x - 1);
     }
     __syncthreads();
+#ifdef LGF_REDUCE_SKIP   /* timing-only probe: no final sum (F, theta and the stop decision are NOT produced) */
+    if (last && threadIdx.x == 0) ctrl->iter += count_iter ? 1 : 0;
+    return;
+#endif
     if (!last) return;
     __threadfence();
     // One CTA adds gridDim.x pairs while the rest of the GPU idles (8192 pairs at 32^4, 131072 at 64^4), so the
@@ -71,6 +75,77 @@ __device__ __forceinline__ void finish_measure(double trF, double th, int64_t V,
     }
     for (; i < gridDim.x; i += THREADS) {
         const double2 v = __ldcg(pp + i);
+        f += v.x; t += v.y;
+    }
+    block_sum2<THREADS>(f, t);
+    if (threadIdx.x == 0) {
+        const double F = f / (12.0 * (double)V), theta = t / (3.0 * (double)V);
+        long long it = ctrl->iter + (count_iter ? 1 : 0);
+        ctrl->F = F; ctrl->theta = theta; ctrl->iter = it;
+        if (it < LGF_HIST_CAP) hist[it] = make_double2(F, theta);
+        if (!(theta == theta) || theta > 1.0e300) ctrl->done = 2;
+        else if (theta <= eps) ctrl->done = 1;
+    }
+}
+
+// The same in two levels, for the kernel of the inner loop.  In finish_measure ONE block adds the partial sums of the
+// whole grid while the rest of the GPU idles: 5.8 us of the 200 us of the link kernel at 32^4 (8192 blocks), 82 us at
+// 64^4 (131072 blocks; timing probe -DLGF_REDUCE_SKIP, profiles/r02_reduce.md).  Here the blocks form groups of
+// LGF_REDUCE_GROUP consecutive indices; the last block of a GROUP to arrive adds the group's partial sums (while other
+// groups are still at work), the last GROUP to finish adds the group sums.  Every sum runs over fixed indices in a
+// fixed order, so F and theta are bitwise reproducible whichever blocks happen to be last; they differ from the
+// one-level sums in the order of the additions only.
+// Scratch: `partials` holds the G block partials as before; `gred` is a region of its own (the one-level kernels,
+// whose grids differ, never write it): NG group partials (pairs of doubles) followed by NG unsigned group tickets,
+// NG = ceil(G / LGF_REDUCE_GROUP).  The tickets start at zero (lgf_bind clears the region) and wrap back to zero
+// with the last arrival of every launch.  reduce2l_bytes(G) is what the region must hold for grids up to G blocks.
+#ifndef LGF_REDUCE_GROUP
+#define LGF_REDUCE_GROUP 64
+#endif
+__host__ __device__ inline size_t reduce2l_bytes(int64_t max_blocks)
+{
+    const size_t ng = (size_t)((max_blocks + LGF_REDUCE_GROUP - 1) / LGF_REDUCE_GROUP) + 1;
+    return ng * (sizeof(double2) + sizeof(unsigned)) + 16;
+}
+template <int THREADS>
+__device__ __forceinline__ void finish_measure_2l(double trF, double th, int64_t V, Ctrl *ctrl, double *partials, void *gred,
+                                                  double2 *hist, double eps, int count_iter)
+{
+    static_assert(LGF_REDUCE_GROUP <= THREADS, "a group is summed by one pass of the block");
+    block_sum2<THREADS>(trF, th);
+    __shared__ int role;                                   // 0: done, 1: last block of its group, 2: last group
+    const unsigned G = gridDim.x, GS = LGF_REDUCE_GROUP, NG = (G + GS - 1) / GS;
+    double2 *bpart = (double2 *)partials, *gpart = (double2 *)gred;
+    unsigned *gtick = (unsigned *)(gpart + NG);
+    const unsigned grp = blockIdx.x / GS;
+    const unsigned gsize = (grp + 1) * GS <= G ? GS : G - grp * GS;
+    if (threadIdx.x == 0) {
+        bpart[blockIdx.x] = make_double2(trF, th);
+        __threadfence();
+        const unsigned tk = atomicInc(&gtick[grp], gsize - 1);
+        role = (tk == gsize - 1) ? 1 : 0;
+    }
+    __syncthreads();
+    if (!role) return;
+    __threadfence();
+    double f = 0, t = 0;
+    if (threadIdx.x < gsize) {
+        const double2 v = __ldcg(bpart + (size_t)grp * GS + threadIdx.x);
+        f = v.x; t = v.y;
+    }
+    block_sum2<THREADS>(f, t);
+    if (threadIdx.x == 0) {
+        gpart[grp] = make_double2(f, t);
+        __threadfence();
+        const unsigned tk = atomicInc(&ctrl->ticket, NG - 1);
+        role = (tk == NG - 1) ? 2 : 0;
+    }
+    __syncthreads();
+    if (role != 2) return;
+    __threadfence();
+    f = 0; t = 0;
+    for (unsigned i = threadIdx.x; i < NG; i += THREADS) {
+        const double2 v = __ldcg(gpart + i);
         f += v.x; t += v.y;
     }
     block_sum2<THREADS>(f, t);
