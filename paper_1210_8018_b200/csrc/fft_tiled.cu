@@ -296,19 +296,27 @@ k_fft_xy_inv_g(const cx<T> *__restrict__ w, cx<T> *__restrict__ gbuf, int64_t V,
 }
 
 // The same pass for planes whose four fields do not fit one SM's shared memory (64^2 in FP64:
-// 266 KB): a thread-block CLUSTER of two CTAs holds the plane, two fields each; after the
-// transforms each CTA builds g for half of the sites, reading its own two fields locally and
-// the other two from the peer's shared memory (DSMEM).
+// 266 KB): a thread-block CLUSTER of LGF_XYG_CLUSTER CTAs holds the plane, 4 / LGF_XYG_CLUSTER fields each; after the
+// transforms each CTA builds g for its share of the sites, reading its own fields locally and
+// the others from the peers' shared memory (DSMEM).
+// LGF_XYG_CLUSTER: CTAs per cluster, 2 (two fields per CTA, one CTA per SM for 64^2 FP64 planes) or 4 (one field per CTA,
+// three CTAs per SM; each CTA then reads three of the four fields of its quarter of the sites through DSMEM).
+// Same-run A/B in profiles/r02_xyg_cluster.md.
+#ifndef LGF_XYG_CLUSTER
+#define LGF_XYG_CLUSTER 4   /* 64^4 FP64: 792 us against 827 us with 2 (profiles/r02_xyg_cluster.md) */
+#endif
 template <typename T, int NA, int NB> struct XYG2Cfg {
     typedef Tile<NA, NB, 1, split_min<T>(NA, NB)> TL;
+    static constexpr int CS = LGF_XYG_CLUSTER, FPC = 4 / CS;  // cluster size, fields per CTA
+    static_assert(CS == 2 || CS == 4, "LGF_XYG_CLUSTER must be 2 or 4");
     static constexpr int TP = (TL::SA > 1 || TL::SB > 1) ? (TL::THREADS + 31) / 32 * 32 : TL::THREADS;
-    static constexpr int CTA = 2 * TP;                        // two fields per CTA
-    static constexpr size_t SMEM = (size_t)2 * TL::ELEMS * sizeof(cx<T>);
+    static constexpr int CTA = FPC * TP;
+    static constexpr size_t SMEM = (size_t)FPC * TL::ELEMS * sizeof(cx<T>);
     static constexpr bool FITS = SMEM <= 227 * 1024 && CTA <= 1024 && CTA >= 64;
 };
 
 template <typename T, int NA, int NB, bool ACC>
-__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__((XYG2Cfg<T, NA, NB>::CTA))
+__global__ void __cluster_dims__(LGF_XYG_CLUSTER, 1, 1) __launch_bounds__((XYG2Cfg<T, NA, NB>::CTA))
 k_fft_xy_inv_g2(const cx<T> *__restrict__ w, cx<T> *__restrict__ gbuf, int64_t V, T a, int gexp, const Ctrl *ctrl)
 {
     namespace cg = cooperative_groups;
@@ -319,12 +327,13 @@ k_fft_xy_inv_g2(const cx<T> *__restrict__ w, cx<T> *__restrict__ gbuf, int64_t V
     typedef Line<T, NB, TL::SB> LB;
     constexpr int TP = CF::TP;
     cg::cluster_group cluster = cg::this_cluster();
-    const int rank = (int)cluster.block_rank();              // 0: fields 0, 1;  1: fields 2, 3
+    constexpr int CS = CF::CS, FPC = CF::FPC;
+    const int rank = (int)cluster.block_rank();              // fields [rank FPC, (rank + 1) FPC)
     extern __shared__ __align__(16) unsigned char smem_raw[];
     cx<T> *smp = (cx<T> *)smem_raw;
     const int t = threadIdx.x, lf = t / TP, l = t % TP;
     cx<T> *sm = smp + (size_t)lf * TL::ELEMS;
-    const int64_t plane = blockIdx.x >> 1;
+    const int64_t plane = blockIdx.x / CS;
     const int64_t base = plane * (int64_t)(NA * NB);
     int xa, ha, yb, hb;
     line_of_thread<TL::SB>(l, xa, ha);
@@ -332,7 +341,7 @@ k_fft_xy_inv_g2(const cx<T> *__restrict__ w, cx<T> *__restrict__ gbuf, int64_t V
     const bool on_y = xa < NA && l < TL::SB * NA, on_x = yb < NB && l < TL::SA * NB;
     const unsigned my = __ballot_sync(0xffffffffu, on_y), mx = __ballot_sync(0xffffffffu, on_x);
     {
-        const cx<T> *f = w + (int64_t)(2 * rank + lf) * V + base;
+        const cx<T> *f = w + (int64_t)(FPC * rank + lf) * V + base;
 #pragma unroll
         for (int k = 0; k < (NA * NB + TP - 1) / TP; k++) {
             const int e = l + k * TP;
@@ -358,9 +367,11 @@ k_fft_xy_inv_g2(const cx<T> *__restrict__ w, cx<T> *__restrict__ gbuf, int64_t V
         for (int q = 0; q < LB::NL; q++) sm[LB::slot(q, ha) * TL::RS + xa] = v[q];
     }
     cluster.sync();                                          // all four fields of the plane are in place
-    const cx<T> *peer = cluster.map_shared_rank(smp, rank ^ 1);
-    const cx<T> *f01 = rank == 0 ? smp : peer, *f23 = rank == 0 ? peer : smp;
-    constexpr int HALF = NA * NB / 2;
+    // field k of the plane lives in CTA k / FPC at slot k % FPC (this CTA's own fields through its own mapping)
+    const cx<T> *fld[4];
+#pragma unroll
+    for (int k = 0; k < 4; k++) fld[k] = cluster.map_shared_rank(smp, k / FPC) + (size_t)(k % FPC) * TL::ELEMS;
+    constexpr int HALF = NA * NB / CS;                       // this CTA's share of the sites
     constexpr int EB = (ACC || LGF_EPI_ALL) ? LGF_EPI_BATCH : 1;
     for (int i0 = rank * HALF + t; i0 < (rank + 1) * HALF; i0 += EB * CF::CTA) {
         cx<T> Gold[EB][6];
@@ -378,7 +389,7 @@ k_fft_xy_inv_g2(const cx<T> *__restrict__ w, cx<T> *__restrict__ gbuf, int64_t V
             if (i < (rank + 1) * HALF) {
                 const int o = (i / NA) * TL::RS + (i % NA);
                 cx<T> g[9];
-                m_from_packed<T>(f01[o], f01[TL::ELEMS + o], f23[o], f23[TL::ELEMS + o], a, g);
+                m_from_packed<T>(fld[0][o], fld[1][o], fld[2][o], fld[3][o], a, g);
                 finish_g01<T>(g, gexp);
                 emit_g<T, ACC>(g, Gold[b], gbuf + base + i, V);
             }
@@ -496,8 +507,8 @@ template <typename T, int N> static int launch_inv_g_n(const FftArgs &a, void *g
         else k_fft_xy_inv_g<T, N, N, false><<<grid, X::CTA, X::SMEM, st>>>((const cx<T> *)a.w, (cx<T> *)gbuf, a.geo.V, nplanes, (T)(alpha / 2.0), gexp, a.ctrl);
     } else {
         typedef XYG2Cfg<T, N, N> X;                           // one cluster of two CTAs per plane
-        if (accum) k_fft_xy_inv_g2<T, N, N, true><<<(unsigned)(2 * nplanes), X::CTA, X::SMEM, st>>>((const cx<T> *)a.w, (cx<T> *)gbuf, a.geo.V, (T)(alpha / 2.0), gexp, a.ctrl);
-        else k_fft_xy_inv_g2<T, N, N, false><<<(unsigned)(2 * nplanes), X::CTA, X::SMEM, st>>>((const cx<T> *)a.w, (cx<T> *)gbuf, a.geo.V, (T)(alpha / 2.0), gexp, a.ctrl);
+        if (accum) k_fft_xy_inv_g2<T, N, N, true><<<(unsigned)(X::CS * nplanes), X::CTA, X::SMEM, st>>>((const cx<T> *)a.w, (cx<T> *)gbuf, a.geo.V, (T)(alpha / 2.0), gexp, a.ctrl);
+        else k_fft_xy_inv_g2<T, N, N, false><<<(unsigned)(X::CS * nplanes), X::CTA, X::SMEM, st>>>((const cx<T> *)a.w, (cx<T> *)gbuf, a.geo.V, (T)(alpha / 2.0), gexp, a.ctrl);
     }
     return 0;
 }
